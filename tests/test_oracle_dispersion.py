@@ -1,0 +1,324 @@
+"""Pins for the oracle's dispersion functions, gradients, equilibria and splines (CPU only).
+
+Each test pins oracle/ to something other than itself: numpy's determinant of the Cartesian dielectric
+matrix, Stix's biquadratic, the Appleton-Hartree formula, textbook cutoff / resonance frequencies built from
+scipy.constants, central differences, scipy's FITPACK splines, div B = 0 and the safety factor q(r).
+Pin numbers (P4, P7, P9) refer to DESIGN.md.
+"""
+import numpy as np
+import pytest
+import scipy.constants as sc
+
+from paper_2508_15967_b200 import inputs
+
+GHZ = 2 * np.pi * 1e9
+
+
+def _tok_points(n, seed=0, rho_lo=0.1, rho_hi=0.9):
+    rng = np.random.default_rng(seed)
+    t = inputs.TOKAMAK
+    rho = rng.uniform(rho_lo, rho_hi, n)
+    th = rng.uniform(0, 2 * np.pi, n)
+    ph = rng.uniform(0, 2 * np.pi, n)
+    R = t["R0"] + rho * t["a"] * np.cos(th)
+    Z = rho * t["a"] * np.sin(th)
+    x = np.stack([R * np.cos(ph), R * np.sin(ph), Z])
+    d = rng.normal(size=(3, n))
+    d /= np.linalg.norm(d, axis=0)
+    return x, d
+
+
+def _tok_eq():
+    return dict(kind="tokamak_circular", **inputs.TOKAMAK)
+
+
+def _slab_eq():
+    return inputs.config(3, n_rays=1).eq
+
+
+def _cart_matrix(S, Dx, P, b, n):
+    """eps + n n - n^2 I in Cartesian axes: eps = S (I - bb) + P bb + i Dx [b]x  (rotation of Eq. 7)."""
+    bx = np.array([[0, -b[2], b[1]], [b[2], 0, -b[0]], [-b[1], b[0], 0]])
+    eps = S * (np.eye(3) - np.outer(b, b)) + P * np.outer(b, b) + 1j * Dx * bx
+    return eps + np.outer(n, n) - (n @ n) * np.eye(3)
+
+
+# ---------------------------------------------------------------------------------------------- P7
+def test_stix_elements_match_textbook_cutoffs_and_resonance(oracle):
+    """Electrons only: right/left-hand cutoffs w_R,L = (sqrt(Wce^2 + 4 wpe^2) +- |Wce|)/2 give R = 0 / L = 0,
+    the upper hybrid w^2 = wpe^2 + Wce^2 gives S = 0, and w = wpe gives P = 0 (textbook closed forms; the
+    paper's Fig. 3 names exactly these surfaces, L157)."""
+    eq = _slab_eq()
+    eq["ion_mass"] = 0.0
+    x = np.array([[2.0], [0.0], [0.0]])
+    ne, B, _, _ = oracle.plasma(eq, x, 60 * GHZ)
+    wpe = np.sqrt(ne[0] * sc.e**2 / (sc.epsilon_0 * sc.m_e))
+    wce = sc.e * np.linalg.norm(B[:, 0]) / sc.m_e
+    assert ne[0] == pytest.approx(5e19 * 0.3 / 0.5, rel=1e-14)
+    assert B[2, 0] == pytest.approx(2.0 * 1.7 / 2.0, rel=1e-15)
+    w_R = 0.5 * (np.sqrt(wce**2 + 4 * wpe**2) + wce)
+    w_L = 0.5 * (np.sqrt(wce**2 + 4 * wpe**2) - wce)
+    w_UH = np.sqrt(wpe**2 + wce**2)
+    S, Dx, P = oracle.plasma(eq, x, w_R)[2][:, 0]
+    assert abs(S + Dx) < 1e-12 and abs(S - Dx) > 0.1          # R = S + Dx = 0 at the right-hand cutoff
+    S, Dx, P = oracle.plasma(eq, x, w_L)[2][:, 0]
+    assert abs(S - Dx) < 1e-12 and abs(S + Dx) > 0.1          # L = 0 at the left-hand cutoff
+    S, Dx, P = oracle.plasma(eq, x, w_UH)[2][:, 0]
+    assert abs(S) < 1e-12
+    S, Dx, P = oracle.plasma(eq, x, wpe)[2][:, 0]
+    assert abs(P) < 1e-12
+
+
+def test_stix_elements_two_species_against_scipy_constants(oracle):
+    """Eq. 8-10 with e + D, summed independently here in the R/L form 1 - sum wps^2/(w (w +- Ws))."""
+    eq = _tok_eq()
+    x, _ = _tok_points(50, seed=3)
+    w = 110 * GHZ
+    ne, B, sdp, ins = oracle.plasma(eq, x, w)
+    assert ins.all()
+    Bm = np.linalg.norm(B, axis=0)
+    mD = sc.physical_constants["deuteron mass"][0]
+    Rr = np.ones_like(ne)
+    Ll = np.ones_like(ne)
+    for q, m in ((-sc.e, sc.m_e), (sc.e, mD)):
+        wp2 = ne * q * q / (sc.epsilon_0 * m)
+        Om = q * Bm / m
+        Rr -= wp2 / (w * (w + Om))
+        Ll -= wp2 / (w * (w - Om))
+    np.testing.assert_allclose(sdp[0], 0.5 * (Rr + Ll), rtol=1e-12)
+    np.testing.assert_allclose(sdp[1], 0.5 * (Rr - Ll), rtol=1e-9, atol=1e-14)
+    np.testing.assert_allclose(sdp[2], 1 - ne * sc.e**2 / sc.epsilon_0 / w**2 * (1 / sc.m_e + 1 / mD), rtol=1e-12)
+
+
+def test_cold_full_equals_numpy_determinant_and_biquadratic(oracle):
+    """P7: oracle D == numpy.linalg.det of the complex Cartesian 3x3 == A n^4 - B n^2 + C."""
+    eq = _tok_eq()
+    w = 110 * GHZ
+    x, d = _tok_points(200, seed=1)
+    rng = np.random.default_rng(2)
+    nmag = rng.uniform(0.2, 1.3, x.shape[1])
+    k = d * nmag * w / inputs.C_LIGHT
+    D, _, ins = oracle.dispersion(eq, "cold_full", x, k, w)
+    ne, B, sdp, _ = oracle.plasma(eq, x, w)
+    assert ins.all()
+    for i in range(x.shape[1]):
+        S, Dx, P = sdp[:, i]
+        b = B[:, i] / np.linalg.norm(B[:, i])
+        n = d[:, i] * nmag[i]
+        det = np.linalg.det(_cart_matrix(S, Dx, P, b, n))
+        assert abs(det.imag) < 1e-13
+        assert D[i] == pytest.approx(det.real, abs=2e-13)
+        c2 = (n @ b) ** 2 / (n @ n)
+        s2 = 1 - c2
+        A = S * s2 + P * c2
+        Bq = (S * S - Dx * Dx) * s2 + P * S * (1 + c2)
+        C = P * (S * S - Dx * Dx)
+        n2 = n @ n
+        assert D[i] == pytest.approx(A * n2 * n2 - Bq * n2 + C, abs=2e-13)
+
+
+def test_cold_full_roots_at_special_angles_and_appleton_hartree(oracle):
+    """P7: theta = 90 deg -> n^2 in {P, RL/S}; theta = 0 -> n^2 in {R, L}; ions off -> Appleton-Hartree."""
+    eq = _tok_eq()
+    w = 110 * GHZ
+    x, d = _tok_points(40, seed=5)
+    ne, B, sdp, _ = oracle.plasma(eq, x, w)
+    b = B / np.linalg.norm(B, axis=0)
+    S, Dx, P = sdp
+    # perpendicular unit vectors
+    e = np.cross(b.T, d.T).T
+    e /= np.linalg.norm(e, axis=0)
+    for n2, dirv in ((P, e), ((S * S - Dx * Dx) / S, e), (S + Dx, b), (S - Dx, b)):
+        k = dirv * np.sqrt(n2) * w / inputs.C_LIGHT
+        D, _, _ = oracle.dispersion(eq, "cold_full", x, k, w)
+        assert np.abs(D).max() < 5e-14
+    # Appleton-Hartree (electrons only)
+    eq1 = dict(eq, ion_mass=0.0)
+    X = ne * sc.e**2 / (sc.epsilon_0 * sc.m_e * w * w)
+    Y = sc.e * np.linalg.norm(B, axis=0) / (sc.m_e * w)
+    ct = np.sum(d * b, axis=0)
+    st2 = 1 - ct * ct
+    for sign in (+1.0, -1.0):
+        den = 1 - X - 0.5 * Y**2 * st2 + sign * np.sqrt((0.5 * Y**2 * st2) ** 2 + (1 - X) ** 2 * Y**2 * ct**2)
+        n2 = 1 - X * (1 - X) / den
+        k = d * np.sqrt(n2) * w / inputs.C_LIGHT
+        D, _, _ = oracle.dispersion(eq1, "cold_full", x, k, w)
+        assert np.abs(D).max() < 5e-14
+
+
+def test_xmode_and_omode_values(oracle):
+    """XMODE D = S n^2 - RL and OMODE D = n^2 - 1 + X against the Stix elements / scipy.constants."""
+    eq = _slab_eq()
+    rng = np.random.default_rng(7)
+    n = 64
+    x = np.stack([rng.uniform(2.15, 2.3, n), rng.uniform(-0.2, 0.2, n), np.zeros(n)])
+    w = 60 * GHZ
+    nvec = rng.normal(size=(3, n)) * 0.5
+    k = nvec * w / sc.c
+    S, Dx, P = oracle.plasma(eq, x, w)[2]
+    D, _, _ = oracle.dispersion(eq, "xmode", x, k, w)
+    n2 = np.sum(nvec**2, axis=0)
+    np.testing.assert_allclose(D, S * n2 - (S + Dx) * (S - Dx), atol=1e-14)
+    ne = oracle.plasma(eq, x, w)[0]
+    D, _, _ = oracle.dispersion(eq, "omode", x, k, w)
+    np.testing.assert_allclose(D, n2 - 1 + ne * sc.e**2 / (sc.epsilon_0 * sc.m_e * w * w), atol=1e-14)
+
+
+# ---------------------------------------------------------------------------------------------- P4
+def _grid_eq_small():
+    return inputs.synth_grid(seed=11, eps=1e-3, nR=65, nZ=65, nPsi=65)
+
+
+@pytest.mark.parametrize("case", ["parabolic-omode", "slab-omode", "slab-xmode", "slab-cold", "tok-omode", "tok-xmode",
+                                  "tok-cold", "grid-cold"])
+def test_dual_number_gradients_match_central_differences(oracle, case):
+    """P4: all 7 partials (x, y, z, kx, ky, kz, w) against central differences of the plain-double D."""
+    eqname, disp = case.split("-")
+    disp = {"omode": "omode", "xmode": "xmode", "cold": "cold_full"}[disp]
+    n = 24
+    rng = np.random.default_rng(13)
+    if eqname == "parabolic":
+        w0 = inputs.config(1, n_rays=n)
+        eq, w, x = w0.eq, w0.omega, w0.x0 + rng.normal(size=(3, n)) * 0.05
+    elif eqname == "slab":
+        eq, w = _slab_eq(), 60 * GHZ
+        x = np.stack([rng.uniform(2.19, 2.29, n), rng.uniform(-0.2, 0.2, n), rng.uniform(-0.1, 0.1, n)])
+    elif eqname == "tok":
+        eq, w = _tok_eq(), 110 * GHZ
+        x, _ = _tok_points(n, seed=17)
+    else:
+        eq, w = oracle.Equilibrium(_grid_eq_small()), 110 * GHZ
+        x, _ = _tok_points(n, seed=19, rho_lo=0.2, rho_hi=0.85)
+    k = rng.normal(size=(3, n)) * 0.6 * w / sc.c
+    D, g, ins = oracle.dispersion(eq, disp, x, k, w)
+    assert ins.all() and np.isfinite(g).all()
+    # error scale: the partial itself, floored by 1e-3 of the largest partial of its group (x / k / w)
+    grp = [np.abs(g[0:3]).max(), np.abs(g[3:6]).max(), np.abs(g[6]).max()]
+    scale = np.stack([np.maximum(np.abs(g[j]), 1e-3 * grp[min(j // 3, 2)]) for j in range(7)])
+    for j in range(7):
+        if j < 3:
+            h = 1e-6
+            xp, xm = x.copy(), x.copy()
+            xp[j] += h
+            xm[j] -= h
+            fd = (oracle.dispersion_value(eq, disp, xp, k, w) - oracle.dispersion_value(eq, disp, xm, k, w)) / (2 * h)
+        elif j < 6:
+            h = 1e-6 * w / sc.c
+            kp, km = k.copy(), k.copy()
+            kp[j - 3] += h
+            km[j - 3] -= h
+            fd = (oracle.dispersion_value(eq, disp, x, kp, w) - oracle.dispersion_value(eq, disp, x, km, w)) / (2 * h)
+        else:
+            h = 1e-6 * w
+            fd = (oracle.dispersion_value(eq, disp, x, k, w + h) - oracle.dispersion_value(eq, disp, x, k, w - h)) / (2 * h)
+        err = np.abs(fd - g[j]) / scale[j]
+        assert err.max() < 2e-7, (case, j, err.max())
+
+
+def test_omega_derivative_closed_form_omode(oracle):
+    """SURVEY 8(c) step 2 check: O-mode w dD/dw = -2 (n^2 + X) (differentiating the full D, reading A4)."""
+    w0 = inputs.config(1, n_rays=16)
+    rng = np.random.default_rng(23)
+    k = rng.normal(size=(3, 16)) * w0.omega / sc.c
+    D, g, _ = oracle.dispersion(w0.eq, "omode", w0.x0, k, w0.omega)
+    n2 = np.sum((k * sc.c / w0.omega) ** 2, axis=0)
+    X = D - n2 + 1
+    np.testing.assert_allclose(g[6] * w0.omega, -2 * (n2 + X), rtol=1e-13)
+
+
+# ------------------------------------------------------------------------------------ equilibria
+def test_tokamak_field_is_divergence_free_and_has_the_stated_q(oracle):
+    """Reading A9: B = grad(phi) x grad(psi) + F grad(phi) is solenoidal; q(r) = r B_phi / (R0 B_theta) = 1 + 2 rho^2
+    on the midplane... in the cylindrical (large-aspect) definition used to build it."""
+    eq = _tok_eq()
+    t = inputs.TOKAMAK
+    x, _ = _tok_points(64, seed=29)
+    h = 1e-5
+    div = np.zeros(x.shape[1])
+    for j in range(3):
+        xp, xm = x.copy(), x.copy()
+        xp[j] += h
+        xm[j] -= h
+        div += (oracle.plasma(eq, xp, 1e11)[1][j] - oracle.plasma(eq, xm, 1e11)[1][j]) / (2 * h)
+    assert np.abs(div).max() < 1e-8
+    ne, B, _, _ = oracle.plasma(eq, x, 1e11)
+    R = np.hypot(x[0], x[1])
+    r = np.hypot(R - t["R0"], x[2])
+    Bphi = (-B[0] * x[1] + B[1] * x[0]) / R
+    BR = (B[0] * x[0] + B[1] * x[1]) / R
+    Bpol = np.hypot(BR, B[2])
+    np.testing.assert_allclose(r * Bphi / (t["R0"] * Bpol), 1 + 2 * (r / t["a"]) ** 2, rtol=1e-12)
+    np.testing.assert_allclose(Bphi, t["B0"] * t["R0"] / R, rtol=1e-14)
+    np.testing.assert_allclose(ne, 5e19 * (1 - (r / t["a"]) ** 2) ** 1.5, rtol=1e-12)
+    # B_poloidal is tangent to the flux surface (circles about the axis): B . grad(r) = 0
+    assert np.abs(BR * (R - t["R0"]) + B[2] * x[2]).max() < 1e-15
+
+
+def test_domain_flags(oracle):
+    eq = _tok_eq()
+    t = inputs.TOKAMAK
+    x = np.array([[t["R0"] + 0.97 * t["a"], t["R0"] + 0.985 * t["a"], t["R0"]], [0, 0, 0], [0, 0, 0.99 * t["a"]]], float)
+    ins = oracle.plasma(eq, x, 1e11)[3]
+    assert list(ins) == [1, 0, 0]
+    eqs = _slab_eq()
+    ins = oracle.plasma(eqs, np.array([[1.0, -1.0], [0, 0], [0, 0]], float), 1e11)[3]
+    assert list(ins) == [1, 0]
+
+
+# ---------------------------------------------------------------------------------------------- P9
+def test_bicubic_pieces_reproduce_a_bicubic_polynomial_exactly(oracle):
+    """P9: a not-a-knot tensor spline of samples of a bicubic polynomial is that polynomial."""
+    rng = np.random.default_rng(31)
+    c = rng.normal(size=(4, 4))
+    R = np.linspace(1.0, 2.0, 9)
+    Z = np.linspace(-0.5, 0.5, 11)
+    f = sum(c[p, q] * R[:, None] ** p * Z[None, :] ** q for p in range(4) for q in range(4))
+    pp = oracle.fit_bicubic_pp(f, R, Z)
+    Rq, Zq = rng.uniform(1, 2, 200), rng.uniform(-0.5, 0.5, 200)
+    iR = np.minimum(((Rq - 1.0) / (R[1] - R[0])).astype(int), 7)
+    iZ = np.minimum(((Zq + 0.5) / (Z[1] - Z[0])).astype(int), 9)
+    dR, dZ = Rq - R[iR], Zq - Z[iZ]
+    val = sum(pp[iR, iZ, p, q] * dR**p * dZ**q for p in range(4) for q in range(4))
+    ref = sum(c[p, q] * Rq**p * Zq**q for p in range(4) for q in range(4))
+    np.testing.assert_allclose(val, ref, rtol=0, atol=1e-12)
+
+
+def test_grid_equilibrium_matches_fitpack_splines(oracle):
+    """P9: B_R = -psi_Z/R, B_Z = psi_R/R, B_phi = F(psi)/R, n_e(psi) from the oracle's spline pieces against
+    scipy's RectBivariateSpline(kx=ky=3, s=0) / CubicSpline evaluated independently (FITPACK B-splines)."""
+    from scipy.interpolate import CubicSpline, RectBivariateSpline
+    g = _grid_eq_small()
+    R = g["Rmin"] + np.arange(g["nR"]) * (g["Rmax"] - g["Rmin"]) / (g["nR"] - 1)
+    Z = g["Zmin"] + np.arange(g["nZ"]) * (g["Zmax"] - g["Zmin"]) / (g["nZ"] - 1)
+    Pg = np.linspace(g["psi_min"], g["psi_max"], g["nPsi"])
+    rbs = RectBivariateSpline(R, Z, g["psi_RZ"], kx=3, ky=3, s=0)
+    x, _ = _tok_points(300, seed=37, rho_lo=0.05, rho_hi=0.95)
+    Rq, Zq = np.hypot(x[0], x[1]), x[2]
+    ne, B, _, ins = oracle.plasma(oracle.Equilibrium(g), x, 1e11)
+    assert ins.all()
+    BR = (B[0] * x[0] + B[1] * x[1]) / Rq
+    Bphi = (-B[0] * x[1] + B[1] * x[0]) / Rq
+    np.testing.assert_allclose(BR, -rbs.ev(Rq, Zq, dy=1) / Rq, atol=1e-11)
+    np.testing.assert_allclose(B[2], rbs.ev(Rq, Zq, dx=1) / Rq, atol=1e-11)
+    psi = rbs.ev(Rq, Zq)
+    np.testing.assert_allclose(Bphi, CubicSpline(Pg, g["F_psi"])(psi) / Rq, rtol=1e-12)
+    np.testing.assert_allclose(ne, CubicSpline(Pg, g["ne_psi"])(psi), rtol=1e-10, atol=1e8)
+
+
+def test_grid_second_derivatives_match_fitpack(oracle):
+    """P9: d(B_Z R)/dR = psi_RR etc. (by central differences of the oracle's field) against FITPACK's dx=2."""
+    from scipy.interpolate import RectBivariateSpline
+    g = _grid_eq_small()
+    R = g["Rmin"] + np.arange(g["nR"]) * (g["Rmax"] - g["Rmin"]) / (g["nR"] - 1)
+    Z = g["Zmin"] + np.arange(g["nZ"]) * (g["Zmax"] - g["Zmin"]) / (g["nZ"] - 1)
+    rbs = RectBivariateSpline(R, Z, g["psi_RZ"], kx=3, ky=3, s=0)
+    eq = oracle.Equilibrium(g)
+    rng = np.random.default_rng(41)
+    Rq, Zq = rng.uniform(1.3, 2.1, 100), rng.uniform(-0.4, 0.4, 100)
+    h = 1e-6
+    zeros = np.zeros_like(Rq)
+    f = lambda r, z: oracle.plasma(eq, np.stack([r, zeros, z]), 1e11)[1]
+    psi_RR = (f(Rq + h, Zq)[2] * (Rq + h) - f(Rq - h, Zq)[2] * (Rq - h)) / (2 * h)
+    psi_ZZ = -(f(Rq, Zq + h)[0] - f(Rq, Zq - h)[0]) * Rq / (2 * h)
+    np.testing.assert_allclose(psi_RR, rbs.ev(Rq, Zq, dx=2), atol=2e-6)
+    np.testing.assert_allclose(psi_ZZ, rbs.ev(Rq, Zq, dy=2), atol=2e-6)
