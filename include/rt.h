@@ -1,0 +1,151 @@
+/* rt.h -- C ABI of the B200-native batched RF ray tracer.
+ *
+ * The library integrates, for a batch of independent rays, the geometric-optics ray equations
+ *
+ *      dx/dt = -(dD/dk)/(dD/dw),      dk/dt = +(dD/dx)/(dD/dw)                 (Eq. 2-3)
+ *
+ * with the classical 4th-order Runge-Kutta tableau at a fixed step ("expressions of 4th order
+ * Runga-Kutta ... a single kernel call"; inputs x, k, t, w; outputs the dispersion residual and the updated
+ * x, k, t), D(x, k, w) being a cold-plasma dispersion function (Eq. 5-10; O-mode / X-mode
+ * branches L157, L191) over a plasma equilibrium B(x), n_e(x) (splines L60).  Every step of that
+ * path runs in hand-written sm_100a CUDA kernels: one thread per ray, all n_steps fused in one launch, RK4 state
+ * and hand-derived gradients of D in registers.  There is NO CPU fallback: every entry point that computes
+ * returns RT_ERR_CUDA when no CUDA device is usable.
+ *
+ * Conventions
+ *   - All functions return RT_OK (0) or a negative RT_ERR_* code; they never throw and never abort.
+ *     rt_last_error() returns a thread-local message for the last non-zero return on the calling thread.
+ *   - "DEVICE" pointers are CUDA device pointers on the current device, 16-byte aligned, owned by the caller
+ *     (e.g. PyTorch tensors); buffers must not alias.  "HOST" pointers are ordinary host memory.
+ *   - Ray arrays are structure-of-arrays: x0[c*n_rays + i], c = 0..2 (x, y, z), i = ray.
+ *   - Element type of every ray buffer follows `precision`: double for RT_F64, float for RT_F32.
+ *   - Units are the paper's: x [m], k [rad/m], w [rad/s].  The step `dt` is given in tau = c*t metres
+ *     (reading A3), i.e. the time step is dt/c seconds.  Sample times are t_s = s*save_stride*dt/c.
+ *   - Calls with a `cuda_stream` enqueue work on that stream (a cudaStream_t cast to void*; NULL = the legacy
+ *     default stream) and return without synchronising.
+ *   - Ray status (reading A12): 0 = integrated all steps; 1 = a Runge-Kutta stage point left the
+ *     equilibrium's domain, the ray is frozen at its last accepted state; 2 = a step produced a non-finite state,
+ *     frozen likewise.  |D| reported at a state outside the domain is NaN.
+ */
+#ifndef RT_B200_RT_H
+#define RT_B200_RT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RT_OK               0
+#define RT_ERR_INVALID     -1   /* bad argument (null pointer, negative size, misaligned buffer, bad enum) */
+#define RT_ERR_UNSUPPORTED -2   /* combination not defined (e.g. X-mode over the unmagnetised parabolic slab) */
+#define RT_ERR_CUDA        -3   /* CUDA runtime error, or no usable device */
+#define RT_ERR_NOMEM       -4   /* host or device allocation failed */
+
+/* Equilibria: B(x), n_e(x).  Definitions in DESIGN.md "Equilibria". */
+typedef enum {
+  RT_EQ_SLAB_PARABOLIC   = 0,  /* n_e = n_ref (1 + (x^2+y^2)/L^2), no B                    (BASELINE configs 1-2) */
+  RT_EQ_SLAB_LINEAR_BR   = 1,  /* n_e = n_ref (x_foot - x)/L_ramp, B = (B0 R0 / x) z^; domain x > 0   (config 3;
+                                  the unclamped linear profile of PAPER.md Eq. 4) */
+  RT_EQ_TOKAMAK_CIRCULAR = 2,  /* B = grad(phi) x grad(psi) + F grad(phi), F = B0 R0, dpsi/dr = B0 r/q,
+                                  q = q0 + q1 rho^2, n_e = n_ref (1-rho^2)^p_exp; domain rho < rho_max (config 4) */
+  RT_EQ_GRID_RZ          = 3   /* psi(R,Z) bicubic, F(psi), n_e(psi) cubic not-a-knot splines of nodal data;
+                                  domain = grid rectangle and psi in [psi_min, psi_max]    (config 5) */
+} rt_eq_kind;
+
+/* Dispersion functions (dimensionless; n = c k / w, Eq. 6; S, D, P of Eq. 8-10). */
+typedef enum {
+  RT_DISP_OMODE     = 0,       /* D = n^2 - 1 + wpe^2/w^2            (BASELINE config 1; electrons only) */
+  RT_DISP_XMODE     = 1,       /* D = S n^2 - R L                     (reading A5) */
+  RT_DISP_COLD_FULL = 2        /* D = Det(eps + n n - n^2 I)          (Eq. 5) */
+} rt_disp_kind;
+
+typedef enum { RT_F64 = 0, RT_F32 = 1 } rt_precision;
+
+/* Plain-old-data description of an equilibrium.  Caller-owned; everything (including the nodal arrays) is copied
+ * by rt_create_equilibrium.  Fields not used by `kind` are ignored. */
+typedef struct rt_equilibrium_desc {
+  int32_t kind;                       /* rt_eq_kind */
+  int32_t nR, nZ, nPsi;               /* GRID_RZ: node counts (each >= 4) */
+  double n_ref, L;                    /* n_ref [m^-3]: reference density of the three analytic kinds; L [m] */
+  double x_foot, L_ramp, B0, R0;      /* [m], [m], [T], [m] */
+  double a, q0, q1, p_exp, rho_max;   /* minor radius [m]; q = q0 + q1 rho^2; rho_max <= 0 means 0.98 */
+  double Rmin, Rmax, Zmin, Zmax;      /* GRID_RZ: uniform node coordinates R_i = Rmin + i (Rmax-Rmin)/(nR-1) */
+  double psi_min, psi_max;            /* GRID_RZ: uniform psi nodes of the two 1-D profiles */
+  const double* psi_RZ;               /* HOST [nR][nZ] nodal psi, row-major (Z fastest) [T m^2] */
+  const double* F_psi;                /* HOST [nPsi] nodal F = R B_phi [T m] */
+  const double* ne_psi;               /* HOST [nPsi] nodal n_e [m^-3] */
+  double ion_mass, ion_charge;        /* one ion species, n_i = n_e/ion_charge; ion_mass [kg] = 0: electrons only */
+} rt_equilibrium_desc;
+
+typedef struct rt_equilibrium rt_equilibrium;   /* opaque; owns its device tables and a host<->device workspace */
+
+/* Validate and copy `desc`; for GRID_RZ fit the not-a-knot splines on the host in fp64 (reading A10) and
+ * upload the cell-major coefficient tables.  *out receives the handle.  Errors: INVALID, NOMEM, CUDA. */
+int rt_create_equilibrium(const rt_equilibrium_desc* desc, rt_equilibrium** out);
+
+/* Free the handle and everything it owns.  NULL is accepted.  Synchronises the device. */
+int rt_destroy(rt_equilibrium* eq);
+
+/* The hot path (Eq. 2-3): trace n_rays rays for n_steps RK4 steps of size dt.
+ *   x0, k0        DEVICE [3][n_rays]   launch positions [m] and wave vectors [rad/m] (on-shell)
+ *   omega         rad/s, one value per call
+ *   save_stride   >= 1; used only when out_traj != NULL, and then n_steps % save_stride must be 0
+ *   out_traj      DEVICE [n_saved][6][n_rays], n_saved = n_steps/save_stride + 1, rows (x,y,z,kx,ky,kz); sample 0 is
+ *                 the launch state, sample s the state after s*save_stride steps; or NULL
+ *   out_final     DEVICE [6][n_rays] state after n_steps; or NULL
+ *   out_residual  DEVICE |D|: [n_saved][n_rays] if out_traj != NULL else [n_rays] (at the final state); or NULL
+ *   out_status    DEVICE int32 [n_rays]; or NULL
+ * n_rays == 0 or n_steps == 0 are valid (n_steps == 0 copies the launch state).  Errors: INVALID, UNSUPPORTED, CUDA. */
+int rt_trace(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+             int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
+             void* out_residual, int32_t* out_status, void* cuda_stream);
+
+/* The same call with HOST buffers (pageable or pinned): copies x0, k0 to the device, runs the rt_trace kernel and
+ * copies the requested outputs back, pipelined over ray chunks on the handle's own streams; returns after the
+ * results are in host memory.  Uses (and grows) the handle's workspace: not re-entrant per handle. */
+int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                  int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
+                  void* out_residual, int32_t* out_status);
+
+/* Launch conditions ("fix w, x, k_y, k_z; Newton-solve ... to |D| < 1e-15; the initial guess selects
+ * the root").  For each ray: given the position x0 and a unit direction dir, find |n| on D = 0 -- closed form
+ * (O: n^2 = 1-X; X: n^2 = RL/S; full: root of Stix's biquadratic A n^4 - B n^2 + C, branch 0 = the root nearer P,
+ * 1 = the other; reading A11) polished by at most 8 Newton steps until |D| < 1e-15 -- and write
+ * k0 = |n| dir w/c.  fp64 only.
+ *   x0, dir       DEVICE double [3][n]
+ *   k0            DEVICE double [3][n]   (NaN where the branch is evanescent or x0 is outside the domain)
+ *   D_out         DEVICE double [n] D at the returned state (signed); or NULL */
+int rt_launch(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, double omega,
+              int64_t n, double* k0, double* D_out, void* cuda_stream);
+
+/* Diagnostic evaluation of the integrand at n points (the quantities one RK4 stage computes):
+ *   x, k          DEVICE [3][n]
+ *   D_out         DEVICE [n]     signed D(x,k,w); NaN outside the domain; or NULL
+ *   rhs_out       DEVICE [6][n]  (dx/dtau, dn/dtau), tau = c t, n = c k/w: the right-hand side the kernel integrates
+ *                 (zero outside the domain); or NULL
+ *   inside_out    DEVICE int32 [n]; or NULL */
+int rt_rhs(const rt_equilibrium* eq, int disp, int precision, const void* x, const void* k, double omega, int64_t n,
+           void* D_out, void* rhs_out, int32_t* inside_out, void* cuda_stream);
+
+/* Device-side reductions over a residual / status pair as written by rt_trace (per-context reduction
+ * kernels; L80 converge items).  residual: DEVICE [n] of `precision` (NaN entries are skipped), status: DEVICE
+ * int32 [n] or NULL.  out: DEVICE double [6] = {max |D|, sum |D|, count finite, #status0, #status1, #status2}. */
+int rt_reduce(int precision, const void* residual, const int32_t* status, int64_t n, double* out, void* cuda_stream);
+
+/* Measured roofline denominator: run >= min_ms milliseconds of independent dependent-chain FMA accumulators (DFMA
+ * for RT_F64, FFMA for RT_F32) on every SM and report the sustained rate.  Synchronous.
+ *   fma_per_s     HOST out: fused multiply-adds per second (flop/s = 2x)
+ *   sm_clock_mhz  HOST out: average SM clock over the run derived from clock64()/globaltimer; or NULL */
+int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz);
+
+/* Number of kernel launches this library has enqueued on the calling process so far (for bench.py's gpu_launches). */
+int64_t rt_launch_count(void);
+
+const char* rt_last_error(void);
+const char* rt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_B200_RT_H */

@@ -1,0 +1,307 @@
+"""Thin ctypes binding of the C-ABI library declared in ``include/rt.h`` -- argument marshalling only.
+
+Every step of the hot path (RK4 on the ray equations Eq. 2-3; Eq. 5-10 dispersion; L60 spline
+equilibria; L159 launch conditions) runs inside ``librt_b200.so``'s sm_100a kernels.  This module turns torch tensors
+into raw device pointers + the current CUDA stream, turns an equilibrium dict into ``rt_equilibrium_desc``, and raises
+``RtError`` on a non-zero return.  There is no CPU fallback: if the library is missing, ``load()`` raises.
+
+Function names mirror the C ABI: ``create_equilibrium / destroy / trace / trace_host / launch / rhs / reduce /
+fma_peak / launch_count``.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "librt_b200.so"
+
+RT_OK, RT_ERR_INVALID, RT_ERR_UNSUPPORTED, RT_ERR_CUDA, RT_ERR_NOMEM = 0, -1, -2, -3, -4
+EQ_KINDS = {"slab_parabolic": 0, "slab_linear_br": 1, "tokamak_circular": 2, "grid_rz": 3}
+DISP_KINDS = {"omode": 0, "xmode": 1, "cold_full": 2}
+PRECISIONS = {"f64": 0, "f32": 1}
+
+# every symbol include/rt.h declares (tests check the library exports each of them)
+SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_host", "rt_launch", "rt_rhs", "rt_reduce",
+           "rt_fma_peak", "rt_launch_count", "rt_last_error", "rt_version")
+
+
+class RtError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"rt error {code}: {msg}")
+        self.code = code
+
+
+class EquilibriumDesc(ctypes.Structure):
+    """Mirror of ``rt_equilibrium_desc`` (include/rt.h)."""
+    _fields_ = [
+        ("kind", ctypes.c_int32), ("nR", ctypes.c_int32), ("nZ", ctypes.c_int32), ("nPsi", ctypes.c_int32),
+        ("n_ref", ctypes.c_double), ("L", ctypes.c_double),
+        ("x_foot", ctypes.c_double), ("L_ramp", ctypes.c_double), ("B0", ctypes.c_double), ("R0", ctypes.c_double),
+        ("a", ctypes.c_double), ("q0", ctypes.c_double), ("q1", ctypes.c_double), ("p_exp", ctypes.c_double),
+        ("rho_max", ctypes.c_double),
+        ("Rmin", ctypes.c_double), ("Rmax", ctypes.c_double), ("Zmin", ctypes.c_double), ("Zmax", ctypes.c_double),
+        ("psi_min", ctypes.c_double), ("psi_max", ctypes.c_double),
+        ("psi_RZ", ctypes.c_void_p), ("F_psi", ctypes.c_void_p), ("ne_psi", ctypes.c_void_p),
+        ("ion_mass", ctypes.c_double), ("ion_charge", ctypes.c_double),
+    ]
+
+
+_SCALARS = ("n_ref", "L", "x_foot", "L_ramp", "B0", "R0", "a", "q0", "q1", "p_exp", "rho_max", "Rmin", "Rmax", "Zmin",
+            "Zmax", "psi_min", "psi_max", "ion_mass", "ion_charge")
+
+
+def make_desc(eq: dict):
+    """Equilibrium dict (``inputs.py``) -> (EquilibriumDesc, keep-alive list of the nodal numpy arrays)."""
+    d = EquilibriumDesc()
+    kind = eq["kind"]
+    d.kind = EQ_KINDS[kind] if isinstance(kind, str) else int(kind)
+    for name in _SCALARS:
+        setattr(d, name, float(eq.get(name, 0.0)))
+    keep = []
+    if d.kind == EQ_KINDS["grid_rz"]:
+        psi = np.ascontiguousarray(eq["psi_RZ"], dtype=np.float64)
+        F = np.ascontiguousarray(eq["F_psi"], dtype=np.float64)
+        ne = np.ascontiguousarray(eq["ne_psi"], dtype=np.float64)
+        if psi.ndim != 2 or F.ndim != 1 or ne.shape != F.shape:
+            raise ValueError("grid_rz: psi_RZ must be [nR, nZ]; F_psi and ne_psi must be [nPsi]")
+        d.nR, d.nZ, d.nPsi = psi.shape[0], psi.shape[1], F.shape[0]
+        d.psi_RZ, d.F_psi, d.ne_psi = psi.ctypes.data, F.ctypes.data, ne.ctypes.data
+        keep = [psi, F, ne]
+    return d, keep
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Load librt_b200.so (built in-tree by ``paper_2508_15967_b200.build``).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RtError(RT_ERR_CUDA, f"{LIB_PATH} is missing: build it with `python -m paper_2508_15967_b200.build` "
+                                       "(there is no CPU fallback)")
+        lib = ctypes.CDLL(str(LIB_PATH))
+        P, D, I64, I32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_int
+        lib.rt_create_equilibrium.argtypes = [ctypes.POINTER(EquilibriumDesc), ctypes.POINTER(P)]
+        lib.rt_destroy.argtypes = [P]
+        lib.rt_trace.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
+        lib.rt_trace_host.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P]
+        lib.rt_launch.argtypes = [P, I32, I32, P, P, D, I64, P, P, P]
+        lib.rt_rhs.argtypes = [P, I32, I32, P, P, D, I64, P, P, P, P]
+        lib.rt_reduce.argtypes = [I32, P, P, I64, P, P]
+        lib.rt_fma_peak.argtypes = [I32, D, ctypes.POINTER(D), ctypes.POINTER(D)]
+        lib.rt_launch_count.restype = I64
+        lib.rt_last_error.restype = ctypes.c_char_p
+        lib.rt_version.restype = ctypes.c_char_p
+        for name in SYMBOLS:
+            fn = getattr(lib, name)
+            if name not in ("rt_launch_count", "rt_last_error", "rt_version"):
+                fn.restype = I32
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise RtError(rc, load().rt_last_error().decode())
+
+
+def version() -> str:
+    return load().rt_version().decode()
+
+
+def launch_count() -> int:
+    return int(load().rt_launch_count())
+
+
+class Equilibrium:
+    """Owns an ``rt_equilibrium*``."""
+
+    def __init__(self, eq: dict):
+        lib = load()
+        desc, keep = make_desc(eq)
+        h = ctypes.c_void_p()
+        _check(lib.rt_create_equilibrium(ctypes.byref(desc), ctypes.byref(h)))
+        self.handle = h
+        self.kind = desc.kind
+
+    def close(self):
+        if getattr(self, "handle", None):
+            load().rt_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def create_equilibrium(eq: dict) -> Equilibrium:
+    return Equilibrium(eq)
+
+
+def destroy(eq: Equilibrium):
+    eq.close()
+
+
+def _disp(disp) -> int:
+    return DISP_KINDS[disp] if isinstance(disp, str) else int(disp)
+
+
+def _prec_of(t) -> int:
+    import torch
+    if t.dtype == torch.float64:
+        return 0
+    if t.dtype == torch.float32:
+        return 1
+    raise TypeError(f"ray buffers must be float64 or float32, got {t.dtype}")
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _dev_soa(t, rows, n=None):
+    if not t.is_cuda or not t.is_contiguous() or t.dim() != 2 or t.shape[0] != rows or (n is not None and t.shape[1] != n):
+        raise ValueError(f"expected a contiguous CUDA tensor of shape [{rows}, {n if n is not None else 'n'}], got "
+                         f"{tuple(t.shape)} on {t.device}")
+    return t
+
+
+def trace(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: float, save_stride: int = 1, *, traj=False,
+          final=True, residual=True, status=True, out: dict | None = None) -> dict:
+    """``rt_trace`` on the current CUDA stream.  x0, k0: CUDA tensors [3, n_rays] (float64 or float32).  Returns a dict
+    of freshly allocated (or, via ``out``, caller-provided) device tensors: 'traj' [n_saved, 6, n], 'final' [6, n],
+    'residual' ([n_saved, n] with traj else [n]), 'status' [n] int32.  Does not synchronise."""
+    import torch
+    lib = load()
+    x0 = _dev_soa(x0, 3)
+    n = x0.shape[1]
+    k0 = _dev_soa(k0, 3, n)
+    if k0.dtype != x0.dtype:
+        raise TypeError("x0 and k0 must have the same dtype")
+    prec = _prec_of(x0)
+    n_saved = n_steps // save_stride + 1 if traj else 0
+    o = {} if out is None else out
+    kw = dict(dtype=x0.dtype, device=x0.device)
+    if traj and "traj" not in o:
+        o["traj"] = torch.empty((n_saved, 6, n), **kw)
+    if final and "final" not in o:
+        o["final"] = torch.empty((6, n), **kw)
+    if residual and "residual" not in o:
+        o["residual"] = torch.empty((n_saved, n) if traj else (n,), **kw)
+    if status and "status" not in o:
+        o["status"] = torch.empty((n,), dtype=torch.int32, device=x0.device)
+    _check(lib.rt_trace(eq.handle, _disp(disp), prec, _ptr(x0), _ptr(k0), float(omega), n, int(n_steps), float(dt),
+                        int(save_stride), _ptr(o.get("traj") if traj else None), _ptr(o.get("final") if final else None),
+                        _ptr(o.get("residual") if residual else None), _ptr(o.get("status") if status else None),
+                        _stream()))
+    return o
+
+
+def trace_host(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: float, save_stride: int = 1, *,
+               traj=False, final=True, residual=True, status=True, out: dict | None = None) -> dict:
+    """``rt_trace_host``: x0, k0 and all outputs are HOST arrays (numpy, or CPU torch tensors -- pinned memory makes
+    the copies asynchronous).  Returns when the results are in host memory."""
+    lib = load()
+    is_torch = not isinstance(x0, np.ndarray)
+
+    def hp(a):
+        if a is None:
+            return None
+        return ctypes.c_void_p(a.data_ptr() if is_torch else a.ctypes.data)
+
+    n = x0.shape[1]
+    if is_torch:
+        import torch
+        if x0.is_cuda or k0.is_cuda or not x0.is_contiguous() or not k0.is_contiguous():
+            raise ValueError("trace_host wants contiguous CPU tensors")
+        prec = _prec_of(x0)
+        empty = lambda shape, dtype=x0.dtype: torch.empty(shape, dtype=dtype)
+        i32 = torch.int32
+    else:
+        x0 = np.ascontiguousarray(x0)
+        k0 = np.ascontiguousarray(k0)
+        prec = {np.dtype(np.float64): 0, np.dtype(np.float32): 1}[x0.dtype]
+        empty = lambda shape, dtype=x0.dtype: np.empty(shape, dtype=dtype)
+        i32 = np.int32
+    if tuple(x0.shape) != (3, n) or tuple(k0.shape) != (3, n) or k0.dtype != x0.dtype:
+        raise ValueError("x0, k0 must both be [3, n] of the same dtype")
+    n_saved = n_steps // save_stride + 1 if traj else 0
+    o = {} if out is None else out
+    if traj and "traj" not in o:
+        o["traj"] = empty((n_saved, 6, n))
+    if final and "final" not in o:
+        o["final"] = empty((6, n))
+    if residual and "residual" not in o:
+        o["residual"] = empty((n_saved, n) if traj else (n,))
+    if status and "status" not in o:
+        o["status"] = empty((n,), i32)
+    _check(lib.rt_trace_host(eq.handle, _disp(disp), prec, hp(x0), hp(k0), float(omega), n, int(n_steps), float(dt),
+                             int(save_stride), hp(o.get("traj") if traj else None), hp(o.get("final") if final else None),
+                             hp(o.get("residual") if residual else None), hp(o.get("status") if status else None)))
+    return o
+
+
+def launch(eq: Equilibrium, disp, x0, dirs, omega: float, branch: int = 0):
+    """``rt_launch``: on-shell k0 [3, n] along unit directions dirs [3, n] from positions x0 (float64 CUDA tensors);
+    also returns D at the launch state."""
+    import torch
+    lib = load()
+    x0 = _dev_soa(x0, 3)
+    n = x0.shape[1]
+    dirs = _dev_soa(dirs, 3, n)
+    if x0.dtype != torch.float64 or dirs.dtype != torch.float64:
+        raise TypeError("rt_launch is fp64 only")
+    k0 = torch.empty((3, n), dtype=torch.float64, device=x0.device)
+    D = torch.empty((n,), dtype=torch.float64, device=x0.device)
+    _check(lib.rt_launch(eq.handle, _disp(disp), int(branch), _ptr(x0), _ptr(dirs), float(omega), n, _ptr(k0), _ptr(D),
+                         _stream()))
+    return k0, D
+
+
+def rhs(eq: Equilibrium, disp, x, k, omega: float):
+    """``rt_rhs``: D [n], (dx/dtau, dn/dtau) [6, n] and the inside flag [n] at points x, k [3, n] (CUDA tensors)."""
+    import torch
+    lib = load()
+    x = _dev_soa(x, 3)
+    n = x.shape[1]
+    k = _dev_soa(k, 3, n)
+    prec = _prec_of(x)
+    D = torch.empty((n,), dtype=x.dtype, device=x.device)
+    f = torch.empty((6, n), dtype=x.dtype, device=x.device)
+    ins = torch.empty((n,), dtype=torch.int32, device=x.device)
+    _check(lib.rt_rhs(eq.handle, _disp(disp), prec, _ptr(x), _ptr(k), float(omega), n, _ptr(D), _ptr(f), _ptr(ins), _stream()))
+    return D, f, ins
+
+
+def reduce(residual, status=None):
+    """``rt_reduce``: device tensor [6] = (max|D|, sum|D|, #finite, #status0, #status1, #status2)."""
+    import torch
+    lib = load()
+    ref = residual if residual is not None else status
+    out = torch.empty((6,), dtype=torch.float64, device=ref.device)
+    prec = _prec_of(residual) if residual is not None else 0
+    n = ref.numel()
+    if residual is not None and not residual.is_contiguous():
+        raise ValueError("residual must be contiguous")
+    _check(lib.rt_reduce(prec, _ptr(residual), _ptr(status), n, _ptr(out), _stream()))
+    return out
+
+
+def fma_peak(precision="f64", min_ms: float = 100.0):
+    """``rt_fma_peak``: (fused multiply-adds per second, observed SM clock in MHz)."""
+    lib = load()
+    rate, mhz = ctypes.c_double(), ctypes.c_double()
+    p = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
+    _check(lib.rt_fma_peak(p, float(min_ms), ctypes.byref(rate), ctypes.byref(mhz)))
+    return rate.value, mhz.value

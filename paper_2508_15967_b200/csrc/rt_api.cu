@@ -1,0 +1,534 @@
+// rt_api.cu -- the C ABI of include/rt.h: argument checks, per-call constant folding (step a0), kernel dispatch,
+// the host-buffer pipeline of rt_trace_host, and the equilibrium handle.  No arithmetic of the method runs on the host
+// except the once-per-equilibrium spline fit (spline_fit.cpp) and the once-per-call folding of w into O(1) constants.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/rt.h"
+#include "rt_kernels.cuh"
+#include "spline_fit.h"
+
+namespace {
+
+// CODATA-2022 numerals (reading A6)
+constexpr double kC = 299792458.0;          // m/s
+constexpr double kQe = 1.602176634e-19;     // C
+constexpr double kMe = 9.1093837139e-31;    // kg
+constexpr double kEps0 = 8.8541878188e-12;  // F/m
+
+thread_local std::string g_err;
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+int cuda_fail(cudaError_t e, const char* what) {
+  return fail(e == cudaErrorMemoryAllocation ? RT_ERR_NOMEM : RT_ERR_CUDA,
+              std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define RT_CUDA(call)                                  \
+  do {                                                 \
+    cudaError_t e_ = (call);                           \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+// ---- the handle ---------------------------------------------------------------------------------------------------
+struct rt_equilibrium {
+  rt_equilibrium_desc d;          // scalars only (nodal pointers nulled)
+  double rho_max;
+  double ne_scale;                // grid: nodal n_e table is stored divided by this
+  // device tables (grid kind): fp64 and fp32 copies
+  double* psi_pp64 = nullptr;
+  double* prof_pp64 = nullptr;
+  float* psi_pp32 = nullptr;
+  float* prof_pp32 = nullptr;
+  int device = 0;
+  // rt_trace_host workspace: two pipeline slots
+  cudaStream_t streams[2] = {nullptr, nullptr};
+  void* slot[2] = {nullptr, nullptr};
+  size_t slot_bytes = 0;
+};
+
+namespace {
+
+template <class T>
+rt::Params<T> make_params(const rt_equilibrium* eq, double omega) {
+  rt::Params<T> P;
+  std::memset(&P, 0, sizeof(P));
+  const rt_equilibrium_desc& d = eq->d;
+  const double alpha = kQe * kQe / (kEps0 * kMe * omega * omega);       // X_e = alpha n_e
+  const double nscale = (d.kind == RT_EQ_GRID_RZ) ? eq->ne_scale : d.n_ref;
+  P.xs = (T)(alpha * nscale);
+  const double wce_per_T = kQe / (kMe * omega);
+  P.beta = (T)(wce_per_T * wce_per_T);
+  P.mu = (T)((d.ion_mass > 0.0) ? d.ion_charge * kMe / d.ion_mass : 0.0);
+  P.k2n = (T)(kC / omega);
+  P.n2k = (T)(omega / kC);
+  P.inv_L2 = (T)(d.L != 0.0 ? 1.0 / (d.L * d.L) : 0.0);
+  P.x_foot = (T)d.x_foot;
+  P.inv_Lramp = (T)(d.L_ramp != 0.0 ? 1.0 / d.L_ramp : 0.0);
+  P.B0R0 = (T)(d.B0 * d.R0);
+  P.R0 = (T)d.R0;
+  P.B0 = (T)d.B0;
+  const double inv_a2 = d.a != 0.0 ? 1.0 / (d.a * d.a) : 0.0;
+  P.inv_a2 = (T)inv_a2;
+  P.q0 = (T)d.q0;
+  P.q1 = (T)d.q1;
+  P.two_q1_a2 = (T)(2.0 * d.q1 * inv_a2);
+  P.p_exp = (T)d.p_exp;
+  P.p_is_three_halves = (d.p_exp == 1.5) ? 1 : 0;
+  P.rho_max2 = (T)(eq->rho_max * eq->rho_max);
+  if (d.kind == RT_EQ_GRID_RZ) {
+    const double hR = (d.Rmax - d.Rmin) / (d.nR - 1), hZ = (d.Zmax - d.Zmin) / (d.nZ - 1);
+    const double hP = (d.psi_max - d.psi_min) / (d.nPsi - 1);
+    P.Rmin = (T)d.Rmin; P.Rmax = (T)d.Rmax; P.Zmin = (T)d.Zmin; P.Zmax = (T)d.Zmax;
+    P.hR = (T)hR; P.hZ = (T)hZ; P.inv_hR = (T)(1.0 / hR); P.inv_hZ = (T)(1.0 / hZ);
+    P.psi_min = (T)d.psi_min; P.psi_max = (T)d.psi_max; P.hP = (T)hP; P.inv_hP = (T)(1.0 / hP);
+    P.nRc = d.nR - 1; P.nZc = d.nZ - 1; P.nPc = d.nPsi - 1;
+    if (sizeof(T) == 8) {
+      P.psi_pp = reinterpret_cast<const T*>(eq->psi_pp64);
+      P.prof_pp = reinterpret_cast<const T*>(eq->prof_pp64);
+    } else {
+      P.psi_pp = reinterpret_cast<const T*>(eq->psi_pp32);
+      P.prof_pp = reinterpret_cast<const T*>(eq->prof_pp32);
+    }
+  }
+  return P;
+}
+
+int check_combo(const rt_equilibrium* eq, int disp) {
+  if (!eq) return fail(RT_ERR_INVALID, "equilibrium handle is NULL");
+  if (disp < RT_DISP_OMODE || disp > RT_DISP_COLD_FULL) return fail(RT_ERR_INVALID, "unknown dispersion kind");
+  if (eq->d.kind == RT_EQ_SLAB_PARABOLIC && disp != RT_DISP_OMODE)
+    return fail(RT_ERR_UNSUPPORTED, "the parabolic slab has no magnetic field: only RT_DISP_OMODE is defined on it");
+  return RT_OK;
+}
+
+int check_omega(double omega) {
+  if (!(omega > 0.0) || !std::isfinite(omega)) return fail(RT_ERR_INVALID, "omega must be positive and finite");
+  return RT_OK;
+}
+
+unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
+
+// ---- dispatch over (EQ, DISP) ---------------------------------------------------------------------------------
+#define RT_FOR_COMBOS(M)                                   \
+  M(rt::EQ_PARABOLIC, rt::DISP_O)                          \
+  M(rt::EQ_LINEAR, rt::DISP_O) M(rt::EQ_LINEAR, rt::DISP_X) M(rt::EQ_LINEAR, rt::DISP_FULL)     \
+  M(rt::EQ_TOKAMAK, rt::DISP_O) M(rt::EQ_TOKAMAK, rt::DISP_X) M(rt::EQ_TOKAMAK, rt::DISP_FULL)  \
+  M(rt::EQ_GRID, rt::DISP_O) M(rt::EQ_GRID, rt::DISP_X) M(rt::EQ_GRID, rt::DISP_FULL)
+
+template <class T>
+int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const rt::TraceArgs<T>& A, cudaStream_t st) {
+  if (A.n_rays == 0) return RT_OK;
+  const unsigned grid = grid_for(A.n_rays, rt::TRACE_BLOCK);
+#define M(E, D)                                                                   \
+  if (eq->d.kind == (E) && disp == (D)) {                                         \
+    rt::trace_kernel<T, E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, A);            \
+    ++g_launches;                                                                 \
+    RT_CUDA(cudaGetLastError());                                                  \
+    return RT_OK;                                                                 \
+  }
+  RT_FOR_COMBOS(M)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no kernel for this equilibrium / dispersion combination");
+}
+
+template <class T>
+int launch_rhs(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const T* x, const T* k, long long n, T* D_out,
+               T* rhs_out, int32_t* inside_out, cudaStream_t st) {
+  if (n == 0) return RT_OK;
+  const unsigned grid = grid_for(n, rt::TRACE_BLOCK);
+#define M(E, D)                                                                                        \
+  if (eq->d.kind == (E) && disp == (D)) {                                                              \
+    rt::rhs_kernel<T, E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, x, k, n, D_out, rhs_out, inside_out);  \
+    ++g_launches;                                                                                      \
+    RT_CUDA(cudaGetLastError());                                                                       \
+    return RT_OK;                                                                                      \
+  }
+  RT_FOR_COMBOS(M)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no kernel for this equilibrium / dispersion combination");
+}
+
+int launch_launch(const rt_equilibrium* eq, int disp, const rt::Params<double>& P, int branch, const double* x0,
+                  const double* dir, long long n, double* k0, double* D_out, cudaStream_t st) {
+  if (n == 0) return RT_OK;
+  const unsigned grid = grid_for(n, rt::TRACE_BLOCK);
+#define M(E, D)                                                                                  \
+  if (eq->d.kind == (E) && disp == (D)) {                                                        \
+    rt::launch_kernel<E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, branch, x0, dir, n, k0, D_out);  \
+    ++g_launches;                                                                                \
+    RT_CUDA(cudaGetLastError());                                                                 \
+    return RT_OK;                                                                                \
+  }
+  RT_FOR_COMBOS(M)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no kernel for this equilibrium / dispersion combination");
+}
+
+template <class T>
+int trace_device(const rt_equilibrium* eq, int disp, const void* x0, const void* k0, double omega, long long n_rays,
+                 long long n_steps, double dt, long long save_stride, void* out_traj, void* out_final,
+                 void* out_residual, int32_t* out_status, cudaStream_t st) {
+  const rt::Params<T> P = make_params<T>(eq, omega);
+  rt::TraceArgs<T> A;
+  A.x0 = static_cast<const T*>(x0);
+  A.k0 = static_cast<const T*>(k0);
+  A.traj = static_cast<T*>(out_traj);
+  A.fin = static_cast<T*>(out_final);
+  A.res = static_cast<T*>(out_residual);
+  A.status = out_status;
+  A.n_rays = n_rays;
+  A.n_steps = n_steps;
+  A.stride = save_stride;
+  A.h = (T)dt;
+  return launch_trace<T>(eq, disp, P, A, st);
+}
+
+int check_trace_args(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                     long long n_rays, long long n_steps, double dt, long long save_stride, const void* out_traj) {
+  int rc = check_combo(eq, disp);
+  if (rc) return rc;
+  if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if ((rc = check_omega(omega))) return rc;
+  if (n_rays < 0 || n_steps < 0) return fail(RT_ERR_INVALID, "n_rays and n_steps must be >= 0");
+  if (!std::isfinite(dt)) return fail(RT_ERR_INVALID, "dt must be finite");
+  if (save_stride < 1) return fail(RT_ERR_INVALID, "save_stride must be >= 1");
+  if (out_traj && (n_steps % save_stride) != 0)
+    return fail(RT_ERR_INVALID, "n_steps must be a multiple of save_stride when out_traj is given");
+  if (n_rays > 0 && (!x0 || !k0)) return fail(RT_ERR_INVALID, "x0 / k0 is NULL");
+  return RT_OK;
+}
+
+int require_device_ptr(const void* p, const char* name, bool may_be_null) {
+  if (!p) return may_be_null ? RT_OK : fail(RT_ERR_INVALID, std::string(name) + " is NULL");
+  if (!aligned16(p)) return fail(RT_ERR_INVALID, std::string(name) + " is not 16-byte aligned");
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cudaPointerGetAttributes"); }
+  if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+    return fail(RT_ERR_INVALID, std::string(name) + " is not a device pointer (host buffers go through rt_trace_host)");
+  return RT_OK;
+}
+
+template <class T>
+int upload(const std::vector<double>& src, T** dst) {
+  std::vector<T> tmp(src.begin(), src.end());
+  RT_CUDA(cudaMalloc(reinterpret_cast<void**>(dst), tmp.size() * sizeof(T)));
+  RT_CUDA(cudaMemcpy(*dst, tmp.data(), tmp.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return RT_OK;
+}
+
+void free_handle(rt_equilibrium* eq) {
+  if (!eq) return;
+  cudaFree(eq->psi_pp64); cudaFree(eq->prof_pp64); cudaFree(eq->psi_pp32); cudaFree(eq->prof_pp32);
+  for (int s = 0; s < 2; ++s) {
+    if (eq->slot[s]) cudaFree(eq->slot[s]);
+    if (eq->streams[s]) cudaStreamDestroy(eq->streams[s]);
+  }
+  delete eq;
+}
+
+}  // namespace
+
+// ==== C ABI ===========================================================================================================
+extern "C" {
+
+const char* rt_last_error(void) { return g_err.c_str(); }
+const char* rt_version(void) { return "rt-b200 0.1 (sm_100a)"; }
+int64_t rt_launch_count(void) { return (int64_t)g_launches.load(); }
+
+int rt_create_equilibrium(const rt_equilibrium_desc* desc, rt_equilibrium** out) {
+  if (!desc || !out) return fail(RT_ERR_INVALID, "desc / out is NULL");
+  *out = nullptr;
+  const rt_equilibrium_desc& d = *desc;
+  auto bad = [](double v) { return !std::isfinite(v); };
+  if (d.kind < RT_EQ_SLAB_PARABOLIC || d.kind > RT_EQ_GRID_RZ) return fail(RT_ERR_INVALID, "unknown equilibrium kind");
+  if (bad(d.ion_mass) || d.ion_mass < 0.0) return fail(RT_ERR_INVALID, "ion_mass must be >= 0");
+  if (d.ion_mass > 0.0 && !(d.ion_charge > 0.0 && std::isfinite(d.ion_charge)))
+    return fail(RT_ERR_INVALID, "ion_charge must be > 0 when ion_mass > 0");
+  if (d.kind != RT_EQ_GRID_RZ && (bad(d.n_ref) || d.n_ref < 0.0)) return fail(RT_ERR_INVALID, "n_ref must be >= 0");
+  switch (d.kind) {
+    case RT_EQ_SLAB_PARABOLIC:
+      if (!(d.L > 0.0) || bad(d.L)) return fail(RT_ERR_INVALID, "parabolic slab: L must be > 0");
+      break;
+    case RT_EQ_SLAB_LINEAR_BR:
+      if (bad(d.x_foot) || bad(d.L_ramp) || d.L_ramp == 0.0) return fail(RT_ERR_INVALID, "linear slab: bad x_foot / L_ramp");
+      if (bad(d.B0) || bad(d.R0) || d.B0 * d.R0 == 0.0) return fail(RT_ERR_INVALID, "linear slab: B0 R0 must be non-zero");
+      break;
+    case RT_EQ_TOKAMAK_CIRCULAR:
+      if (!(d.a > 0.0) || !(d.R0 > 0.0) || bad(d.a) || bad(d.R0)) return fail(RT_ERR_INVALID, "tokamak: a, R0 must be > 0");
+      if (bad(d.B0) || d.B0 == 0.0) return fail(RT_ERR_INVALID, "tokamak: B0 must be non-zero");
+      if (bad(d.q0) || bad(d.q1) || !(d.q0 > 0.0) || d.q1 < 0.0) return fail(RT_ERR_INVALID, "tokamak: need q0 > 0, q1 >= 0");
+      if (bad(d.p_exp) || d.p_exp < 1.0) return fail(RT_ERR_INVALID, "tokamak: p_exp must be >= 1");
+      if (bad(d.rho_max) || d.rho_max >= 1.0) return fail(RT_ERR_INVALID, "tokamak: rho_max must be < 1");
+      break;
+    default:
+      if (d.nR < 4 || d.nZ < 4 || d.nPsi < 4) return fail(RT_ERR_INVALID, "grid: nR, nZ, nPsi must each be >= 4");
+      if (d.nR > 16384 || d.nZ > 16384 || d.nPsi > (1 << 24)) return fail(RT_ERR_INVALID, "grid: too many nodes");
+      if (bad(d.Rmin) || bad(d.Rmax) || bad(d.Zmin) || bad(d.Zmax) || !(d.Rmax > d.Rmin) || !(d.Zmax > d.Zmin) || !(d.Rmin > 0.0))
+        return fail(RT_ERR_INVALID, "grid: need 0 < Rmin < Rmax and Zmin < Zmax");
+      if (bad(d.psi_min) || bad(d.psi_max) || !(d.psi_max > d.psi_min)) return fail(RT_ERR_INVALID, "grid: need psi_min < psi_max");
+      if (!d.psi_RZ || !d.F_psi || !d.ne_psi) return fail(RT_ERR_INVALID, "grid: nodal arrays are NULL");
+  }
+  rt_equilibrium* eq = new (std::nothrow) rt_equilibrium();
+  if (!eq) return fail(RT_ERR_NOMEM, "out of host memory");
+  eq->d = d;
+  eq->d.psi_RZ = eq->d.F_psi = eq->d.ne_psi = nullptr;
+  eq->rho_max = (d.rho_max > 0.0) ? d.rho_max : 0.98;
+  eq->ne_scale = 1.0;
+  if (d.kind == RT_EQ_GRID_RZ) {
+    try {
+      const size_t nn = (size_t)d.nR * d.nZ;
+      for (size_t i = 0; i < nn; ++i)
+        if (bad(d.psi_RZ[i])) { delete eq; return fail(RT_ERR_INVALID, "grid: psi_RZ has a non-finite entry"); }
+      double nmax = 0.0;
+      for (int i = 0; i < d.nPsi; ++i) {
+        if (bad(d.F_psi[i]) || bad(d.ne_psi[i])) { delete eq; return fail(RT_ERR_INVALID, "grid: profile has a non-finite entry"); }
+        nmax = std::fmax(nmax, std::fabs(d.ne_psi[i]));
+      }
+      eq->ne_scale = nmax > 0.0 ? nmax : 1.0;
+      // node coordinates: R_i = Rmin + i hR (the kernels recompute them the same way)
+      const double hR = (d.Rmax - d.Rmin) / (d.nR - 1), hZ = (d.Zmax - d.Zmin) / (d.nZ - 1);
+      const double hP = (d.psi_max - d.psi_min) / (d.nPsi - 1);
+      std::vector<double> R(d.nR), Z(d.nZ), Pn(d.nPsi), ne_n(d.nPsi);
+      for (int i = 0; i < d.nR; ++i) R[i] = d.Rmin + i * hR;
+      for (int i = 0; i < d.nZ; ++i) Z[i] = d.Zmin + i * hZ;
+      for (int i = 0; i < d.nPsi; ++i) { Pn[i] = d.psi_min + i * hP; ne_n[i] = d.ne_psi[i] / eq->ne_scale; }
+      std::vector<double> psi_pp;
+      rt::fit_bicubic_not_a_knot(R.data(), Z.data(), d.psi_RZ, d.nR, d.nZ, psi_pp);
+      const int nPc = d.nPsi - 1;
+      std::vector<double> fpp((size_t)nPc * 4), gpp((size_t)nPc * 4), prof((size_t)nPc * 8);
+      rt::fit_cubic_not_a_knot(Pn.data(), d.F_psi, 1, d.nPsi, fpp.data());
+      rt::fit_cubic_not_a_knot(Pn.data(), ne_n.data(), 1, d.nPsi, gpp.data());
+      for (int i = 0; i < nPc; ++i)
+        for (int m = 0; m < 4; ++m) { prof[(size_t)i * 8 + m] = fpp[(size_t)i * 4 + m]; prof[(size_t)i * 8 + 4 + m] = gpp[(size_t)i * 4 + m]; }
+      cudaError_t e = cudaGetDevice(&eq->device);
+      if (e != cudaSuccess) { delete eq; return cuda_fail(e, "cudaGetDevice"); }
+      int rc;
+      if ((rc = upload<double>(psi_pp, &eq->psi_pp64)) || (rc = upload<double>(prof, &eq->prof_pp64)) ||
+          (rc = upload<float>(psi_pp, &eq->psi_pp32)) || (rc = upload<float>(prof, &eq->prof_pp32))) {
+        free_handle(eq);
+        return rc;
+      }
+    } catch (const std::bad_alloc&) {
+      free_handle(eq);
+      return fail(RT_ERR_NOMEM, "out of host memory while fitting the splines");
+    }
+  }
+  *out = eq;
+  return RT_OK;
+}
+
+int rt_destroy(rt_equilibrium* eq) {
+  if (!eq) return RT_OK;
+  if (eq->psi_pp64 || eq->slot[0] || eq->streams[0]) cudaDeviceSynchronize();
+  free_handle(eq);
+  return RT_OK;
+}
+
+int rt_trace(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+             int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
+             void* out_residual, int32_t* out_status, void* cuda_stream) {
+  int rc = check_trace_args(eq, disp, precision, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj);
+  if (rc) return rc;
+  if (n_rays == 0) return RT_OK;
+  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(k0, "k0", false)) ||
+      (rc = require_device_ptr(out_traj, "out_traj", true)) || (rc = require_device_ptr(out_final, "out_final", true)) ||
+      (rc = require_device_ptr(out_residual, "out_residual", true)) || (rc = require_device_ptr(out_status, "out_status", true)))
+    return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (precision == RT_F64)
+    return trace_device<double>(eq, disp, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+  return trace_device<float>(eq, disp, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+}
+
+int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                  int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
+                  void* out_residual, int32_t* out_status) {
+  int rc = check_trace_args(eq, disp, precision, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj);
+  if (rc) return rc;
+  if (n_rays == 0) return RT_OK;
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  const long long n_saved = out_traj ? n_steps / save_stride + 1 : 0;
+  const long long n_res = out_residual ? (out_traj ? n_saved : 1) : 0;
+  // bytes per ray in a pipeline slot
+  const size_t per_ray = 6 * es + (size_t)n_saved * 6 * es + (out_final ? 6 * es : 0) + (size_t)n_res * es + (out_status ? 4 : 0);
+  // chunk: ~8 chunks per call, a multiple of 1024 rays, at least 2^15 rays, at most 4 GiB per slot
+  long long C = ((n_rays + 7) / 8 + 1023) / 1024 * 1024;
+  if (C < 32768) C = 32768;
+  const long long cap = (long long)(((size_t)4 << 30) / per_ray) / 1024 * 1024;
+  if (C > cap) C = cap > 1024 ? cap : 1024;
+  if (C > n_rays) C = (n_rays + 1023) / 1024 * 1024;
+  const size_t need = per_ray * (size_t)C + 256;
+  if (!eq->streams[0]) {
+    for (int s = 0; s < 2; ++s) RT_CUDA(cudaStreamCreateWithFlags(&eq->streams[s], cudaStreamNonBlocking));
+  }
+  if (eq->slot_bytes < need) {
+    RT_CUDA(cudaDeviceSynchronize());
+    for (int s = 0; s < 2; ++s) {
+      if (eq->slot[s]) { cudaFree(eq->slot[s]); eq->slot[s] = nullptr; }
+    }
+    eq->slot_bytes = 0;
+    for (int s = 0; s < 2; ++s) RT_CUDA(cudaMalloc(&eq->slot[s], need));
+    eq->slot_bytes = need;
+  }
+  const char* hx = static_cast<const char*>(x0);
+  const char* hk = static_cast<const char*>(k0);
+  int j = 0;
+  for (long long off = 0; off < n_rays; off += C, ++j) {
+    const long long c = (n_rays - off < C) ? (n_rays - off) : C;
+    cudaStream_t st = eq->streams[j & 1];
+    char* base = static_cast<char*>(eq->slot[j & 1]);
+    char* dx = base;                 base += 3 * (size_t)C * es;
+    char* dk = base;                 base += 3 * (size_t)C * es;
+    char* dtraj = base;              base += (size_t)n_saved * 6 * (size_t)C * es;
+    char* dfin = base;               base += (out_final ? 6 : 0) * (size_t)C * es;
+    char* dres = base;               base += (size_t)n_res * (size_t)C * es;
+    char* dstat = base;
+    const size_t w = (size_t)c * es, hp = (size_t)n_rays * es;
+    RT_CUDA(cudaMemcpy2DAsync(dx, w, hx + (size_t)off * es, hp, w, 3, cudaMemcpyHostToDevice, st));
+    RT_CUDA(cudaMemcpy2DAsync(dk, w, hk + (size_t)off * es, hp, w, 3, cudaMemcpyHostToDevice, st));
+    void* t = out_traj ? dtraj : nullptr;
+    void* f = out_final ? dfin : nullptr;
+    void* r = out_residual ? dres : nullptr;
+    int32_t* s = out_status ? reinterpret_cast<int32_t*>(dstat) : nullptr;
+    if (precision == RT_F64)
+      rc = trace_device<double>(eq, disp, dx, dk, omega, c, n_steps, dt, save_stride, t, f, r, s, st);
+    else
+      rc = trace_device<float>(eq, disp, dx, dk, omega, c, n_steps, dt, save_stride, t, f, r, s, st);
+    if (rc) { cudaDeviceSynchronize(); return rc; }
+    if (out_traj)
+      RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_traj) + (size_t)off * es, hp, dtraj, w, w, (size_t)n_saved * 6, cudaMemcpyDeviceToHost, st));
+    if (out_final)
+      RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_final) + (size_t)off * es, hp, dfin, w, w, 6, cudaMemcpyDeviceToHost, st));
+    if (out_residual)
+      RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_residual) + (size_t)off * es, hp, dres, w, w, (size_t)n_res, cudaMemcpyDeviceToHost, st));
+    if (out_status)
+      RT_CUDA(cudaMemcpyAsync(out_status + off, dstat, (size_t)c * 4, cudaMemcpyDeviceToHost, st));
+  }
+  RT_CUDA(cudaStreamSynchronize(eq->streams[0]));
+  RT_CUDA(cudaStreamSynchronize(eq->streams[1]));
+  return RT_OK;
+}
+
+int rt_launch(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, double omega,
+              int64_t n, double* k0, double* D_out, void* cuda_stream) {
+  int rc = check_combo(eq, disp);
+  if (rc) return rc;
+  if ((rc = check_omega(omega))) return rc;
+  if (branch != 0 && branch != 1) return fail(RT_ERR_INVALID, "branch must be 0 or 1");
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  if (n == 0) return RT_OK;
+  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(dir, "dir", false)) ||
+      (rc = require_device_ptr(k0, "k0", false)) || (rc = require_device_ptr(D_out, "D_out", true)))
+    return rc;
+  const rt::Params<double> P = make_params<double>(eq, omega);
+  return launch_launch(eq, disp, P, branch, x0, dir, n, k0, D_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rt_rhs(const rt_equilibrium* eq, int disp, int precision, const void* x, const void* k, double omega, int64_t n,
+           void* D_out, void* rhs_out, int32_t* inside_out, void* cuda_stream) {
+  int rc = check_combo(eq, disp);
+  if (rc) return rc;
+  if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if ((rc = check_omega(omega))) return rc;
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  if (n == 0) return RT_OK;
+  if ((rc = require_device_ptr(x, "x", false)) || (rc = require_device_ptr(k, "k", false)) ||
+      (rc = require_device_ptr(D_out, "D_out", true)) || (rc = require_device_ptr(rhs_out, "rhs_out", true)) ||
+      (rc = require_device_ptr(inside_out, "inside_out", true)))
+    return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (precision == RT_F64)
+    return launch_rhs<double>(eq, disp, make_params<double>(eq, omega), static_cast<const double*>(x),
+                              static_cast<const double*>(k), n, static_cast<double*>(D_out), static_cast<double*>(rhs_out), inside_out, st);
+  return launch_rhs<float>(eq, disp, make_params<float>(eq, omega), static_cast<const float*>(x), static_cast<const float*>(k), n,
+                           static_cast<float*>(D_out), static_cast<float*>(rhs_out), inside_out, st);
+}
+
+int rt_reduce(int precision, const void* residual, const int32_t* status, int64_t n, double* out, void* cuda_stream) {
+  if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  int rc;
+  if ((rc = require_device_ptr(out, "out", false)) || (rc = require_device_ptr(residual, "residual", true)) ||
+      (rc = require_device_ptr(status, "status", true)))
+    return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  RT_CUDA(cudaMemsetAsync(out, 0, 6 * sizeof(double), st));
+  if (n == 0) return RT_OK;
+  long long blocks = (n + 255) / 256;
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  if (precision == RT_F64)
+    rt::reduce_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(static_cast<const double*>(residual), status, n, out);
+  else
+    rt::reduce_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(static_cast<const float*>(residual), status, n, out);
+  ++g_launches;
+  RT_CUDA(cudaGetLastError());
+  return RT_OK;
+}
+
+int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz) {
+  if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if (!fma_per_s) return fail(RT_ERR_INVALID, "fma_per_s is NULL");
+  if (!(min_ms > 0.0) || min_ms > 10000.0) return fail(RT_ERR_INVALID, "min_ms must be in (0, 10000]");
+  int dev = 0, sms = 0;
+  RT_CUDA(cudaGetDevice(&dev));
+  RT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int grid = sms * 4;                                  // 4 x 256 threads per SM: 8 warps per scheduler
+  void* sink = nullptr;
+  unsigned long long* clk = nullptr;
+  RT_CUDA(cudaMalloc(&sink, (size_t)grid * rt::FMA_BLOCK * 8));
+  RT_CUDA(cudaMalloc(reinterpret_cast<void**>(&clk), 16));
+  cudaEvent_t e0, e1;
+  RT_CUDA(cudaEventCreate(&e0));
+  RT_CUDA(cudaEventCreate(&e1));
+  auto run = [&](long long iters, float* ms) -> int {
+    RT_CUDA(cudaEventRecord(e0, 0));
+    if (precision == RT_F64)
+      rt::fma_peak_kernel<double><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 1.0000001, 1e-9, clk);
+    else
+      rt::fma_peak_kernel<float><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1.0001f, 1e-6f, clk);
+    ++g_launches;
+    RT_CUDA(cudaGetLastError());
+    RT_CUDA(cudaEventRecord(e1, 0));
+    RT_CUDA(cudaEventSynchronize(e1));
+    RT_CUDA(cudaEventElapsedTime(ms, e0, e1));
+    return RT_OK;
+  };
+  float ms = 0.f;
+  int rc = run(2000, &ms);                                    // warm-up + calibration
+  if (!rc) rc = run(2000, &ms);
+  long long iters = 2000;
+  if (!rc) {
+    iters = (long long)(2000.0 * min_ms / (ms > 1e-3f ? ms : 1e-3f)) + 1;
+    rc = run(iters, &ms);
+  }
+  if (!rc) {
+    const double fmas = (double)grid * rt::FMA_BLOCK * rt::FMA_CHAINS * 8.0 * (double)iters;
+    *fma_per_s = fmas / (ms * 1e-3);
+    if (sm_clock_mhz) {
+      unsigned long long h[2] = {0, 0};
+      cudaMemcpy(h, clk, 16, cudaMemcpyDeviceToHost);
+      *sm_clock_mhz = h[1] ? (double)h[0] / (double)h[1] * 1e3 : 0.0;
+    }
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(sink); cudaFree(clk);
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,126 @@
+"""CPU-only checks of the C-ABI library: it builds, loads, exports every symbol include/rt.h declares, validates its
+arguments before touching CUDA, and has no CPU fallback (compute calls fail loudly without a device)."""
+import ctypes
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from paper_2508_15967_b200 import binding, inputs
+from paper_2508_15967_b200 import build as rt_build
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    rt_build.build()
+    return binding.load()
+
+
+def _declared_symbols():
+    text = (ROOT / "include" / "rt.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(rt_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    declared = _declared_symbols()
+    assert sorted(binding.SYMBOLS) == declared
+    for name in declared:
+        assert getattr(lib, name) is not None
+    assert "sm_100a" in binding.version()
+
+
+def test_library_embeds_sm_100a_sass_only():
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not Path(cuobjdump).exists():
+        pytest.skip("cuobjdump not available")
+    out = subprocess.run([cuobjdump, "-lelf", str(binding.LIB_PATH)], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_\d+a?", out))
+    assert archs == {"sm_100a"}, archs
+
+
+def test_desc_struct_matches_header_field_order():
+    text = (ROOT / "include" / "rt.h").read_text()
+    body = re.search(r"typedef struct rt_equilibrium_desc \{(.*?)\} rt_equilibrium_desc;", text, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    names = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if not decl:
+            continue
+        decl = re.sub(r"^(const\s+)?(int32_t|double)\s*\*?", "", decl)
+        names += [n.strip().lstrip("*") for n in decl.split(",")]
+    assert names == [f[0] for f in binding.EquilibriumDesc._fields_]
+
+
+def test_create_validates_descriptors(lib):
+    ok = inputs.config(4, n_rays=4).eq
+    eq = binding.create_equilibrium(ok)          # analytic kinds need no device
+    eq.close()
+    for bad in (dict(ok, a=0.0), dict(ok, B0=0.0), dict(ok, q0=0.0), dict(ok, rho_max=1.5), dict(ok, kind=7),
+                dict(ok, ion_mass=-1.0), dict(ok, ion_charge=0.0), dict(ok, n_ref=float("nan")),
+                dict(inputs.config(1, n_rays=4).eq, L=0.0), dict(inputs.config(3, n_rays=4).eq, L_ramp=0.0)):
+        with pytest.raises(binding.RtError) as e:
+            binding.create_equilibrium(bad)
+        assert e.value.code == binding.RT_ERR_INVALID
+    g = inputs.synth_grid(seed=3, nR=3, nZ=9, nPsi=9)
+    with pytest.raises(binding.RtError) as e:
+        binding.create_equilibrium(g)
+    assert e.value.code == binding.RT_ERR_INVALID
+
+
+def test_trace_argument_checks_come_before_cuda(lib):
+    eq = binding.create_equilibrium(inputs.config(1, n_rays=4).eq)
+    P = ctypes.c_void_p
+    buf = np.zeros((3, 8))
+    call = lambda **kw: lib.rt_trace_host(eq.handle, kw.get("disp", 0), kw.get("prec", 0), P(buf.ctypes.data),
+                                          P(buf.ctypes.data), kw.get("omega", 1e11), kw.get("n", 8), kw.get("steps", 4),
+                                          1e-3, kw.get("stride", 1), kw.get("traj", None), None, None, None)
+    assert call(disp=1) == binding.RT_ERR_UNSUPPORTED and b"parabolic" in lib.rt_last_error()
+    assert call(disp=9) == binding.RT_ERR_INVALID
+    assert call(prec=5) == binding.RT_ERR_INVALID
+    assert call(omega=0.0) == binding.RT_ERR_INVALID
+    assert call(n=-1) == binding.RT_ERR_INVALID
+    assert call(stride=0) == binding.RT_ERR_INVALID
+    assert call(steps=5, stride=2, traj=P(buf.ctypes.data)) == binding.RT_ERR_INVALID
+    assert call(n=0) == binding.RT_OK
+    # host pointers are rejected by rt_trace (no CPU fallback), whether or not a device is present
+    rc = lib.rt_trace(eq.handle, 0, 0, P(buf.ctypes.data), P(buf.ctypes.data), 1e11, 8, 4, 1e-3, 1, None, None, None, None, None)
+    assert rc in (binding.RT_ERR_INVALID, binding.RT_ERR_CUDA)
+    assert lib.rt_trace(None, 0, 0, None, None, 1e11, 8, 4, 1e-3, 1, None, None, None, None, None) == binding.RT_ERR_INVALID
+    eq.close()
+
+
+def test_no_cpu_fallback_without_a_device(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    eq = binding.create_equilibrium(inputs.config(1, n_rays=4).eq)
+    buf = np.zeros((3, 8))
+    out = np.zeros((6, 8))
+    P = ctypes.c_void_p
+    rc = lib.rt_trace_host(eq.handle, 0, 0, P(buf.ctypes.data), P(buf.ctypes.data), 1e11, 8, 4, 1e-3, 1, None,
+                           P(out.ctypes.data), None, None)
+    assert rc == binding.RT_ERR_CUDA
+    rate = ctypes.c_double()
+    assert lib.rt_fma_peak(0, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
+    with pytest.raises(binding.RtError):
+        binding.create_equilibrium(inputs.synth_grid(seed=3, nR=9, nZ=9, nPsi=9))   # grid tables live on the device
+    eq.close()
+
+
+def test_product_never_imports_the_oracle():
+    for path in list((ROOT / "paper_2508_15967_b200").rglob("*.py")) + list((ROOT / "paper_2508_15967_b200").rglob("*.cu*")) \
+            + list((ROOT / "paper_2508_15967_b200").rglob("*.cpp")) + list((ROOT / "paper_2508_15967_b200").rglob("*.h")):
+        text = path.read_text()
+        assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), path
+        assert "rt_oracle" not in text and "librt_oracle" not in text, path
+    for path in (ROOT / "oracle").glob("*"):
+        if path.suffix in (".py", ".cpp", ".h"):
+            assert "paper_2508_15967_b200.binding" not in path.read_text() and "csrc" not in path.read_text().replace(
+                "paper_2508_15967_b200/csrc", ""), path

@@ -1,0 +1,359 @@
+"""GPU parity tests (run with -m gpu on a B200): the CUDA path, called through the C ABI, against the CPU oracle on the
+same seeded inputs.
+
+Tolerances: north_star's relative 1e-10 on final (x, k) for fp64 and 1e-4 for fp32, per-ray
+2-norms (reading A15).  |D| is a cancellation residue, so it is compared absolutely: 64 ulp of the O(1) terms it is
+the difference of, plus 1e-6 of its own size.  Integer outputs (status, inside flags) must be equal.
+Launch wave vectors k0 come from oracle.launch and the same bytes go to both sides (reading A17); rt_launch has its own
+parity test.
+"""
+import numpy as np
+import pytest
+
+from paper_2508_15967_b200 import inputs
+from helpers import rel_err_xk
+
+pytestmark = pytest.mark.gpu
+
+C = inputs.C_LIGHT
+TOL = {"f64": 1e-10, "f32": 1e-4}
+RES_ATOL = {"f64": 64 * 2.2e-16, "f32": 64 * 1.2e-7}
+
+
+@pytest.fixture(scope="module")
+def rt():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: the product has no CPU fallback")
+    from paper_2508_15967_b200 import binding
+    from paper_2508_15967_b200 import build as rt_build
+    rt_build.build()
+    binding.load()
+    torch.cuda.set_device(0)
+    return binding
+
+
+def _dev(a, prec="f64"):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64 if prec == "f64" else np.float32)).cuda()
+
+
+def _host(t):
+    return t.detach().cpu().numpy().astype(np.float64) if t.dtype.is_floating_point else t.detach().cpu().numpy()
+
+
+def _workload(oracle, cfg, n_rays, n_steps, disp=None):
+    w = inputs.config(cfg, n_rays=n_rays, n_steps=n_steps)
+    if disp is not None:
+        w.disp = disp
+    oeq = oracle.Equilibrium(w.eq)
+    k0, D0 = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    assert np.isfinite(k0).all()
+    return w, oeq, k0
+
+
+def _check_residual(got, ref, prec):
+    got, ref = np.asarray(got, dtype=np.float64), np.asarray(ref)
+    assert np.array_equal(np.isnan(got), np.isnan(ref))
+    ok = ~np.isnan(ref)
+    assert (np.abs(got[ok] - ref[ok]) <= RES_ATOL[prec] + 1e-6 * np.abs(ref[ok])).all(), np.abs(got[ok] - ref[ok]).max()
+
+
+# --------------------------------------------------------------------------------- one stage: D and the ray RHS
+COMBOS = [(1, "omode"), (3, "omode"), (3, "xmode"), (3, "cold_full"), (4, "omode"), (4, "xmode"), (4, "cold_full"),
+          (5, "omode"), (5, "xmode"), (5, "cold_full")]
+
+
+def _interior_points(cfg, n, seed):
+    rng = np.random.default_rng(seed)
+    if cfg == 1:
+        return np.stack([rng.uniform(-0.6, 0.6, n), rng.uniform(-0.4, 0.4, n), rng.uniform(-0.1, 0.1, n)])
+    if cfg == 3:
+        return np.stack([rng.uniform(2.19, 2.29, n), rng.uniform(-0.2, 0.2, n), rng.uniform(-0.1, 0.1, n)])
+    t = inputs.TOKAMAK
+    rho, th, ph = rng.uniform(0.05, 0.93, n), rng.uniform(0, 2 * np.pi, n), rng.uniform(0, 2 * np.pi, n)
+    R, Z = t["R0"] + rho * t["a"] * np.cos(th), rho * t["a"] * np.sin(th)
+    return np.stack([R * np.cos(ph), R * np.sin(ph), Z])
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("cfg,disp", COMBOS)
+def test_stage_rhs_matches_oracle_dual_number_gradients(rt, oracle, cfg, disp, prec):
+    """The hand-derived chain rule (kernel) against forward-mode dual numbers through the literal D (oracle), off-shell
+    at random interior points: dx/dtau = -(dD/dk)/(dD/dw)/c, dn/dtau = (dD/dx)/(dD/dw)/w  (Eq. 2-3)."""
+    n = 128 * 3 + 57
+    w = inputs.config(cfg, n_rays=4)
+    x = _interior_points(cfg, n, seed=100 + cfg)
+    rng = np.random.default_rng(7)
+    k = rng.normal(size=(3, n)) * 0.5 * w.omega / C
+    oeq = oracle.Equilibrium(w.eq)
+    D, g, ins = oracle.dispersion(oeq, disp, x, k, w.omega)
+    assert ins.all()
+    f_ref = np.concatenate([-g[3:6] / g[6] / C, g[0:3] / g[6] / w.omega])
+    eq = rt.create_equilibrium(w.eq)
+    Dg, fg, ig = rt.rhs(eq, disp, _dev(x, prec), _dev(k, prec), w.omega)
+    Dg, fg, ig = _host(Dg), _host(fg), _host(ig)
+    assert (ig == 1).all()
+    tol = 2e-12 if prec == "f64" else 2e-4
+    # per point: error relative to the size of the 6-vector (x-part and n-part separately)
+    for sl in (slice(0, 3), slice(3, 6)):
+        err = np.linalg.norm(fg[sl] - f_ref[sl], axis=0) / np.linalg.norm(f_ref[sl], axis=0)
+        # points where dD/dw nearly vanishes amplify rounding: scale by the conditioning |D-gradient| / |W|
+        assert np.median(err) < tol and err.max() < tol * 1e3, (err.max(), np.median(err))
+    np.testing.assert_allclose(Dg, D, rtol=0, atol=(1e-13 if prec == "f64" else 1e-4) * max(1.0, np.abs(D).max()))
+    eq.close()
+
+
+# --------------------------------------------------------------------------------- whole traces, small sizes
+@pytest.mark.parametrize("cfg,n_steps,precs", [(1, 1000, ("f64",)), (2, 2000, ("f64", "f32")), (3, 3000, ("f64",)),
+                                               (4, 1000, ("f64",)), (5, 500, ("f64", "f32"))])
+def test_trace_final_state_parity(rt, oracle, cfg, n_steps, precs):
+    """BASELINE.json configs 1-5 at their own step counts, 677 rays (5 blocks of 128 + a ragged tail of 37)."""
+    n_rays = 128 * 5 + 37
+    w, oeq, k0 = _workload(oracle, cfg, n_rays, n_steps)
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, w.omega, w.n_steps, w.dt)
+    assert (ref["status"] == 0).all()
+    eq = rt.create_equilibrium(w.eq)
+    for prec in precs:
+        out = rt.trace(eq, w.disp, _dev(w.x0, prec), _dev(k0, prec), w.omega, w.n_steps, w.dt)
+        ex, ek = rel_err_xk(_host(out["final"]), ref["final"])
+        assert ex < TOL[prec] and ek < TOL[prec], (cfg, prec, ex, ek)
+        assert np.array_equal(_host(out["status"]), ref["status"])
+        _check_residual(_host(out["residual"]), ref["residual"], prec)
+    eq.close()
+
+
+@pytest.mark.parametrize("cfg,n_steps,stride", [(1, 1000, 1), (4, 1000, 10), (3, 300, 300), (5, 120, 40)])
+def test_trajectory_samples_parity(rt, oracle, cfg, n_steps, stride):
+    """Decimated SoA trajectory output [n_saved][6][n_rays] and |D| at every saved sample (configs 1 and 4's modes)."""
+    n_rays = 128 * 2 + 5
+    w, oeq, k0 = _workload(oracle, cfg, n_rays, n_steps)
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, w.omega, n_steps, w.dt, stride, traj=True)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, n_steps, w.dt, stride, traj=True)
+    tr = _host(out["traj"])
+    assert tr.shape == ref["traj"].shape == (n_steps // stride + 1, 6, n_rays)
+    for m in range(tr.shape[0]):
+        ex, ek = rel_err_xk(tr[m], ref["traj"][m])
+        assert ex < 1e-10 and ek < 1e-10, (m, ex, ek)
+    np.testing.assert_allclose(tr[0, :3], w.x0, rtol=0, atol=0)                   # sample 0 = launch state
+    np.testing.assert_allclose(_host(out["final"]), tr[-1], rtol=0, atol=0)       # final = last sample, bit for bit
+    _check_residual(_host(out["residual"]), ref["residual"], "f64")
+    np.testing.assert_array_equal(_host(out["residual"])[-1], _host(
+        rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, n_steps, w.dt)["residual"]))
+    eq.close()
+
+
+def test_config1_closed_form_harmonic_oscillator(rt, oracle):
+    """BASELINE.json config 1's own check, applied to the CUDA path directly: x(tau), n(tau) are harmonic."""
+    w, oeq, k0 = _workload(oracle, 1, 1024, 1000)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 1000, w.dt, 1, traj=True)
+    tr = _host(out["traj"])
+    n0 = k0 * C / w.omega
+    W = 1 / np.sqrt(2.0)
+    tau = (np.arange(1001) * w.dt)[:, None, None]
+    assert np.abs(tr[:, :3] - (w.x0[None] * np.cos(W * tau) + n0[None] / W * np.sin(W * tau))).max() < 1e-12
+    assert np.abs(tr[:, 3:] * C / w.omega - (n0[None] * np.cos(W * tau) - W * w.x0[None] * np.sin(W * tau))).max() < 1e-12
+    assert np.nanmax(_host(out["residual"])) < 1e-13
+    eq.close()
+
+
+@pytest.mark.parametrize("cfg,disp", [(3, "omode"), (4, "omode"), (4, "xmode"), (5, "omode"), (5, "xmode")])
+def test_trace_parity_other_combinations(rt, oracle, cfg, disp):
+    """Every (equilibrium, dispersion) instantiation the library dispatches, not only the five configs."""
+    w, oeq, k0 = _workload(oracle, cfg, 300, 400, disp)
+    ref = oracle.trace(oeq, disp, w.x0, k0, w.omega, 400, w.dt)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, disp, _dev(w.x0), _dev(k0), w.omega, 400, w.dt)
+    ex, ek = rel_err_xk(_host(out["final"]), ref["final"])
+    assert ex < 1e-10 and ek < 1e-10, (ex, ek)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    eq.close()
+
+
+def test_cold_full_on_the_slab_inside_the_ramp(rt, oracle):
+    """Pin P8's setting on the CUDA path: the full determinant in the slab, launched 2 cm inside the ramp (n_e > 0)."""
+    w = inputs.config(3, n_rays=200, n_steps=800)
+    w.x0[0] = 2.28
+    oeq = oracle.Equilibrium(w.eq)
+    for branch in (0, 1):
+        k0, _ = oracle.launch(oeq, "cold_full", w.x0, w.dirs, w.omega, branch)
+        ref = oracle.trace(oeq, "cold_full", w.x0, k0, w.omega, 800, w.dt)
+        eq = rt.create_equilibrium(w.eq)
+        out = rt.trace(eq, "cold_full", _dev(w.x0), _dev(k0), w.omega, 800, w.dt)
+        ex, ek = rel_err_xk(_host(out["final"]), ref["final"])
+        assert ex < 1e-10 and ek < 1e-10, (branch, ex, ek)
+        eq.close()
+
+
+# --------------------------------------------------------------------------------- status / freezing (reading A12)
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_rays_leaving_the_domain_freeze_identically(rt, oracle, cfg):
+    w = inputs.config(cfg, n_rays=256, n_steps=300)
+    w.dirs[:, ::2] *= -1.0                 # every other ray is aimed outward: it reaches rho_max / psi_max and freezes
+    oeq = oracle.Equilibrium(w.eq)
+    k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, w.omega, 300, w.dt, 100, traj=True)
+    assert (ref["status"][::2] == 1).all() and (ref["status"][1::2] == 0).all()
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 300, w.dt, 100, traj=True)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    ex, ek = rel_err_xk(_host(out["final"]), ref["final"])
+    assert ex < 1e-10 and ek < 1e-10
+    _check_residual(_host(out["residual"]), ref["residual"], "f64")
+    eq.close()
+
+
+def test_non_finite_state_gives_status_2(rt, oracle):
+    """A NaN launch state in the (always-inside) parabolic slab: both sides reject the step with status 2."""
+    w, oeq, k0 = _workload(oracle, 1, 64, 10)
+    k0[0, 5] = np.nan
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, w.omega, 10, w.dt)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 10, w.dt)
+    assert ref["status"][5] == 2 and np.array_equal(_host(out["status"]), ref["status"])
+    eq.close()
+
+
+# --------------------------------------------------------------------------------- edge cases
+def test_edge_sizes(rt, oracle):
+    import torch
+    w, oeq, k0 = _workload(oracle, 4, 129, 20)
+    eq = rt.create_equilibrium(w.eq)
+    # n_steps = 0: outputs are the launch state
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 0, w.dt, 1, traj=True)
+    assert out["traj"].shape == (1, 6, 129)
+    np.testing.assert_allclose(_host(out["final"])[:3], w.x0, rtol=0, atol=0)
+    np.testing.assert_allclose(_host(out["final"])[3:], k0, rtol=1e-15)
+    # a single ray; stride == n_steps
+    ref = oracle.trace(oeq, w.disp, w.x0[:, :1], k0[:, :1], w.omega, 20, w.dt, 20, traj=True)
+    out = rt.trace(eq, w.disp, _dev(w.x0[:, :1]), _dev(k0[:, :1]), w.omega, 20, w.dt, 20, traj=True)
+    ex, ek = rel_err_xk(_host(out["traj"])[1], ref["traj"][1])
+    assert out["traj"].shape == (2, 6, 1) and ex < 1e-12 and ek < 1e-12
+    # zero rays
+    e = torch.empty((3, 0), dtype=torch.float64, device="cuda")
+    out = rt.trace(eq, w.disp, e, e.clone(), w.omega, 5, w.dt)
+    assert out["final"].shape == (6, 0)
+    # outputs are optional
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 20, w.dt, final=False, residual=False, status=True)
+    assert set(out) == {"status"}
+    # argument errors surface as RtError
+    with pytest.raises(rt.RtError):
+        rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 21, w.dt, 2, traj=True)
+    with pytest.raises(rt.RtError):
+        rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), -1.0, 20, w.dt)
+    eq.close()
+
+
+def test_omega_invariance_in_n(rt, oracle):
+    """Reading A13: config 1 in (x, n, tau) does not depend on w when X is held fixed -- run the kernel at two
+    frequencies (n_ref rescaled) and compare n = c k / w."""
+    w, oeq, k0 = _workload(oracle, 1, 256, 500)
+    eq = rt.create_equilibrium(w.eq)
+    a = _host(rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, 500, w.dt)["final"])
+    s = 0.37
+    eq2 = rt.create_equilibrium(dict(w.eq, n_ref=w.eq["n_ref"] * s * s))
+    b = _host(rt.trace(eq2, w.disp, _dev(w.x0), _dev(k0 * s), w.omega * s, 500, w.dt)["final"])
+    np.testing.assert_allclose(a[:3], b[:3], rtol=0, atol=1e-14)
+    np.testing.assert_allclose(a[3:] / w.omega, b[3:] / (w.omega * s), rtol=0, atol=1e-14 / C)
+    eq.close()
+    eq2.close()
+
+
+# --------------------------------------------------------------------------------- launch solver
+@pytest.mark.parametrize("cfg,disp,branch", [(1, "omode", 0), (3, "xmode", 0), (4, "cold_full", 0), (4, "cold_full", 1),
+                                             (5, "cold_full", 0), (5, "cold_full", 1), (4, "xmode", 0), (5, "omode", 0)])
+def test_launch_solver_parity(rt, oracle, cfg, disp, branch):
+    w = inputs.config(cfg, n_rays=1000)
+    oeq = oracle.Equilibrium(w.eq)
+    k_ref, D_ref = oracle.launch(oeq, disp, w.x0, w.dirs, w.omega, branch)
+    eq = rt.create_equilibrium(w.eq)
+    k, D = rt.launch(eq, disp, _dev(w.x0), _dev(w.dirs), w.omega, branch)
+    k, D = _host(k), _host(D)
+    assert np.array_equal(np.isnan(k), np.isnan(k_ref))
+    ok = np.isfinite(k_ref).all(axis=0)
+    assert ok.sum() > 900
+    err = np.linalg.norm(k[:, ok] - k_ref[:, ok], axis=0) / np.linalg.norm(k_ref[:, ok], axis=0)
+    assert err.max() < 1e-13, err.max()
+    assert np.abs(D[ok]).max() < 2e-15          # L159's |D| < 1e-15 criterion (plus one rounding of re-evaluation)
+    # the oracle agrees that the GPU's launch states are on-shell
+    D_chk = oracle.dispersion_value(oeq, disp, w.x0[:, ok], k[:, ok], w.omega)
+    assert np.abs(D_chk).max() < 4e-15
+    eq.close()
+
+
+def test_launch_outside_domain_and_evanescent(rt, oracle):
+    w = inputs.config(4, n_rays=8)
+    w.x0[:, 0] = [inputs.TOKAMAK["R0"] + 0.99 * inputs.TOKAMAK["a"], 0.0, 0.0]       # outside rho_max
+    oeq = oracle.Equilibrium(w.eq)
+    k_ref, _ = oracle.launch(oeq, "cold_full", w.x0, w.dirs, w.omega, 0)
+    eq = rt.create_equilibrium(w.eq)
+    k, _ = rt.launch(eq, "cold_full", _dev(w.x0), _dev(w.dirs), w.omega, 0)
+    assert np.array_equal(np.isnan(_host(k)), np.isnan(k_ref)) and np.isnan(k_ref[:, 0]).all()
+    # O-mode above cutoff density: n^2 = 1 - X < 0
+    w1 = inputs.config(1, n_rays=8)
+    w1.x0[0] = 1.5
+    k_ref, _ = oracle.launch(w1.eq, "omode", w1.x0, w1.dirs, w1.omega)
+    eq1 = rt.create_equilibrium(w1.eq)
+    k, _ = rt.launch(eq1, "omode", _dev(w1.x0), _dev(w1.dirs), w1.omega)
+    assert np.isnan(k_ref).all() and np.isnan(_host(k)).all()
+    eq.close()
+    eq1.close()
+
+
+# --------------------------------------------------------------------------------- host-buffer pipeline, reductions
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_trace_host_equals_trace_bit_for_bit(rt, oracle, prec):
+    """rt_trace_host chunks the rays over two streams; per-ray results must not depend on the chunking."""
+    import torch
+    n = 32768 * 2 + 12345                      # three chunks, the last one ragged
+    w = inputs.config(4, n_rays=n, n_steps=40)
+    eq = rt.create_equilibrium(w.eq)
+    x0d = _dev(w.x0)
+    k0d, _ = rt.launch(eq, w.disp, x0d, _dev(w.dirs), w.omega, w.branch)
+    dt = torch.float64 if prec == "f64" else torch.float32
+    x0d, k0d = x0d.to(dt), k0d.to(dt)
+    dev = rt.trace(eq, w.disp, x0d, k0d, w.omega, 40, w.dt, 10, traj=True)
+    x0h, k0h = x0d.cpu().pin_memory(), k0d.cpu().pin_memory()
+    host = rt.trace_host(eq, w.disp, x0h, k0h, w.omega, 40, w.dt, 10, traj=True)
+    for key in ("traj", "final", "residual", "status"):
+        a, b = dev[key].cpu().numpy(), host[key].numpy()
+        assert a.shape == b.shape and np.array_equal(a, b, equal_nan=True), key
+    # numpy (pageable) buffers work too
+    host2 = rt.trace_host(eq, w.disp, x0h.numpy(), k0h.numpy(), w.omega, 40, w.dt, traj=False)
+    assert np.array_equal(host2["final"], dev["final"].cpu().numpy())
+    # a handful of those rays against the oracle
+    idx = np.array([0, 1, 32767, 32768, 65535, 65536, n - 1])
+    oeq = oracle.Equilibrium(w.eq)
+    ref = oracle.trace(oeq, w.disp, w.x0[:, idx], k0h.numpy()[:, idx].astype(np.float64), w.omega, 40, w.dt)
+    ex, ek = rel_err_xk(host["final"].numpy()[:, idx], ref["final"])
+    assert ex < TOL[prec] and ek < TOL[prec]
+    eq.close()
+
+
+def test_reduce_matches_numpy(rt, oracle):
+    import torch
+    rng = np.random.default_rng(5)
+    n = 100003
+    res = np.abs(rng.normal(size=n)) * 1e-12
+    res[rng.integers(0, n, 50)] = np.nan
+    status = rng.choice([0, 0, 0, 1, 2], size=n).astype(np.int32)
+    for prec in ("f64", "f32"):
+        r = _dev(res, prec)
+        out = _host(rt.reduce(r, torch.from_numpy(status).cuda()))
+        rr = _host(r)
+        ok = np.isfinite(rr)
+        assert out[0] == rr[ok].max()
+        assert out[1] == pytest.approx(rr[ok].sum(), rel=1e-12)
+        assert out[2] == ok.sum()
+        assert list(out[3:]) == [np.sum(status == 0), np.sum(status == 1), np.sum(status == 2)]
+
+
+def test_fma_peak_is_plausible(rt):
+    f64, mhz = rt.fma_peak("f64", 50.0)
+    f32, _ = rt.fma_peak("f32", 50.0)
+    # B200: 148 SMs x 64 FP64 (128 FP32) lanes x ~1.5-2 GHz
+    assert 0.8e13 < f64 < 2.5e13, f64
+    assert 1.6e13 < f32 < 5.0e13, f32
+    assert 900 < mhz < 2200, mhz
