@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- ray-steps/s of the batched RF ray tracer on B200 (BASELINE.json's metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--precision f64] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one pass of the whole hot path over one batch: one ``rt_trace`` call that loads the launch states, runs all
+RK4 steps of every ray and writes the config's outputs.  The default workload is BASELINE.json
+config 4 -- the configuration the north-star target is quoted on (2^20 rays x 1000 steps, full Stix determinant,
+analytic tokamak, fp64, trajectories decimated every 10 steps).  Inputs are seeded and synthetic (inputs.py) and are
+resident in HBM when the timed region starts; launch wave vectors come from the library's own ``rt_launch`` kernel.
+
+`value`        = n_gpus * n_rays * n_steps * K / (max-over-ranks device time of K steps)
+`e2e`          = the same metric through ``rt_trace_host`` with pinned HOST buffers (H2D + kernel + D2H per step)
+`roofline`     = bound "alu": algorithmic flops per launch / mean kernel time (CUDA events on the launch stream) against
+                 2 x the DFMA (FFMA) rate measured by ``rt_fma_peak`` in this process
+`cpu_baseline` = the CPU oracle, as it stands, on a bounded sample of the same workload (rank 0, N = 1 only)
+``--impl reference`` times the oracle alone (the reference arm of this tier).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+from paper_2508_15967_b200 import inputs  # noqa: E402
+
+METRIC = "ray_steps_per_s"
+UNIT = "ray-steps/s"
+
+# Algorithmic flops per ray-step: adds + multiplies + divisions + square roots of the
+# hand-derived formulation, one RK4 step = 4 right-hand sides + the tableau; a fused multiply-add counts 2.
+FLOPS_PER_RAY_STEP = {1: 263, 2: 263, 3: 571, 4: 1067, 5: 1507}
+# DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None
+NCU_DRAM_BYTES = {}
+
+WORKLOAD_NAMES = {
+    1: "cfg1: O-mode, parabolic slab, 1024 rays x 1000 steps, full trajectory",
+    2: "cfg2: O-mode, parabolic slab, 2^20 rays x 2000 steps, final state + |D|",
+    3: "cfg3: X-mode, e+D, B0R0/R slab with linear density ramp, 2^18 rays x 3000 steps, final state + |D|",
+    4: "cfg4: full Stix determinant, e+D, analytic circular tokamak, 2^20 rays x 1000 steps, trajectory every 10 steps + |D|",
+    5: "cfg5: full Stix determinant, e+D, 257x257 bicubic-spline R-Z grid, 2^24 rays x 500 steps, final state + |D|",
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n-rays", type=int, default=None, help="override the config's ray count (debugging only)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the secondary per-config table")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons while the timed region runs (nvidia-smi, the profiling recipe's line)."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        # "under load": samples at or above half the maximum power seen
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        thr = 0.5 * max(pw)
+        load = [s for s, p in zip(sm, pw) if p >= thr] or sm
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle legs
+def oracle_rate(cfg: int, target_s: float, n_threads: int = 0):
+    """Time the CPU oracle, as it stands, on a bounded sample of config `cfg`: the first n rays of the seeded launch set
+    at the config's full step count, n sized from a short calibration so the run takes about `target_s` seconds."""
+    import oracle
+    oracle.build()
+    cores = oracle.max_threads() if n_threads <= 0 else n_threads
+    n_steps = inputs.FULL_SIZES[cfg][1]
+    probe_n = 8 * cores
+    w = inputs.config(cfg, n_rays=probe_n, n_steps=n_steps)
+    oeq = oracle.Equilibrium(w.eq)
+    k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    oracle.trace(oeq, w.disp, w.x0, k0, w.omega, max(1, n_steps // 10), w.dt, n_threads=cores)   # thread start-up
+    t0 = time.perf_counter()
+    oracle.trace(oeq, w.disp, w.x0, k0, w.omega, n_steps, w.dt, n_threads=cores)
+    t_probe = time.perf_counter() - t0
+    n = int(max(probe_n, min(inputs.FULL_SIZES[cfg][0], probe_n * target_s / max(t_probe, 1e-6))))
+    n = max(cores, n // cores * cores)
+    w = inputs.config(cfg, n_rays=n, n_steps=n_steps)
+    k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    stride = w.save_stride if w.save_stride > 0 else 1
+
+    def run_once():
+        t0 = time.perf_counter()
+        oracle.trace(oeq, w.disp, w.x0, k0, w.omega, n_steps, w.dt, stride, traj=w.save_stride > 0, n_threads=cores)
+        return time.perf_counter() - t0
+
+    return run_once, n, n_steps, cores
+
+
+def cpu_baseline(cfg: int) -> dict:
+    run_once, n, n_steps, cores = oracle_rate(cfg, target_s=15.0)
+    t = run_once()
+    return {"value": n * n_steps / t, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": round(t, 2),
+            "sample": f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps (fp64, OpenMP over rays)"}
+
+
+def run_reference(args) -> int:
+    """--impl reference: the oracle timed on the host cores, same metric / config; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    cfg = args.config
+    run_once, n, n_steps, cores = oracle_rate(cfg, target_s=3.0)
+    for _ in range(args.warmup):
+        run_once()
+    t = sum(run_once() for _ in range(args.steps))
+    value = n * n_steps * args.steps / t
+    sample = f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps per step (fp64, OpenMP over rays)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[cfg], "n_rays_per_step": n, "n_steps": n_steps},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ the CUDA arm
+class Job:
+    """One config resident on the current device: equilibrium handle, launch states, preallocated outputs."""
+
+    def __init__(self, rt, torch, cfg: int, prec: str, n_rays, rank: int):
+        self.rt, self.torch, self.cfg, self.prec = rt, torch, cfg, prec
+        seed = 1000 + cfg + 7919 * rank                       # rank r traces its own batch (weak scaling, no exchange)
+        self.w = w = inputs.config(cfg, n_rays=n_rays, seed=seed)
+        self.eq = rt.create_equilibrium(w.eq)
+        dt = torch.float64 if prec == "f64" else torch.float32
+        x0 = torch.from_numpy(w.x0).cuda()
+        k0, D0 = rt.launch(self.eq, w.disp, x0, torch.from_numpy(w.dirs).cuda(), w.omega, w.branch)
+        if not bool(torch.isfinite(k0).all()):
+            raise RuntimeError("rt_launch returned non-finite launch states for a bench workload")
+        self.launch_residual = float(D0.abs().max())
+        self.x0, self.k0 = x0.to(dt).contiguous(), k0.to(dt).contiguous()
+        self.traj = w.save_stride > 0
+        self.stride = w.save_stride if self.traj else 1
+        self.out = {}
+        self.es = 8 if prec == "f64" else 4
+
+    @property
+    def ray_steps(self) -> int:
+        return self.w.n_rays * self.w.n_steps
+
+    def step(self):
+        w = self.w
+        return self.rt.trace(self.eq, w.disp, self.x0, self.k0, w.omega, w.n_steps, w.dt, self.stride, traj=self.traj,
+                             out=self.out)
+
+    def host_buffers(self):
+        torch, w = self.torch, self.w
+        x0h, k0h = self.x0.cpu().pin_memory(), self.k0.cpu().pin_memory()
+        n, dt = w.n_rays, self.x0.dtype
+        n_saved = w.n_steps // self.stride + 1
+        out = {"final": torch.empty((6, n), dtype=dt, pin_memory=True),
+               "residual": torch.empty((n_saved, n) if self.traj else (n,), dtype=dt, pin_memory=True),
+               "status": torch.empty((n,), dtype=torch.int32, pin_memory=True)}
+        if self.traj:
+            out["traj"] = torch.empty((n_saved, 6, n), dtype=dt, pin_memory=True)
+        h2d = x0h.numel() * self.es + k0h.numel() * self.es
+        d2h = sum(t.numel() * t.element_size() for t in out.values())
+        return x0h, k0h, out, h2d, d2h
+
+    def step_host(self, x0h, k0h, out):
+        w = self.w
+        return self.rt.trace_host(self.eq, w.disp, x0h, k0h, w.omega, w.n_steps, w.dt, self.stride, traj=self.traj, out=out)
+
+    def close(self):
+        self.out = {}
+        self.eq.close()
+
+
+def time_steps(torch, job: Job, steps: int, warmup: int, flush, barrier=None):
+    """W warm-up steps, then exactly K steps bracketed by barrier + synchronize; L2 is flushed between steps by
+    overwriting a buffer larger than L2.  Returns (total ms over the bracket, mean kernel ms from per-step events)."""
+    for _ in range(warmup):
+        job.step()
+        flush.zero_()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for a, b in ev:
+        a.record()
+        job.step()
+        b.record()
+        flush.zero_()
+    t1.record()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    return t0.elapsed_time(t1), statistics.fmean(a.elapsed_time(b) for a, b in ev)
+
+
+def run_ours(args) -> int:
+    import torch
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device -- the product has no CPU fallback", file=sys.stderr)
+        return 2
+    from paper_2508_15967_b200 import binding as rt
+    from paper_2508_15967_b200 import build as rt_build
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if rank == 0:
+        rt_build.build()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    rt.load()
+    barrier = (lambda: dist.barrier()) if dist else None
+    cfg, prec = args.config, args.precision
+    n_rays = args.n_rays if args.n_rays else inputs.FULL_SIZES[cfg][0]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB of L2
+    job = Job(rt, torch, cfg, prec, n_rays, rank)
+
+    peak_before, _ = rt.fma_peak(prec, 200.0)
+    sampler = ClockSampler(local)
+    launches0 = rt.launch_count()
+    sampler.start()
+    total_ms, kernel_ms = time_steps(torch, job, args.steps, args.warmup, flush, barrier)
+    clocks = sampler.stop()
+    launches = rt.launch_count() - launches0 - args.warmup
+    peak_after, peak_mhz = rt.fma_peak(prec, 200.0)
+
+    # a reduction over the last step's outputs: the run's own correctness summary (max |D|, status counts)
+    red = rt.reduce(job.out["residual"].reshape(-1), job.out["status"]).cpu().tolist()
+
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    value = world * job.ray_steps * args.steps / (total_ms_max * 1e-3)
+
+    e2e = None
+    if not args.no_e2e:
+        x0h, k0h, hout, h2d, d2h = job.host_buffers()
+        job.step_host(x0h, k0h, hout)                                       # warm-up (allocates the pipeline workspace)
+        k_e2e = max(1, min(args.steps, 3))
+        torch.cuda.synchronize()
+        if barrier:
+            barrier()
+        w0 = time.perf_counter()
+        for _ in range(k_e2e):
+            job.step_host(x0h, k0h, hout)
+        torch.cuda.synchronize()
+        te = torch.tensor([time.perf_counter() - w0], dtype=torch.float64, device="cuda")
+        if dist:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * job.ray_steps * k_e2e / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": k_e2e, "api": "rt_trace_host (pinned host buffers, 2-stream chunk pipeline)"}
+        del x0h, k0h, hout
+
+    flops = FLOPS_PER_RAY_STEP[cfg] * job.ray_steps
+    launch_residual = job.launch_residual
+    peak = 2.0 * peak_after
+    achieved = flops / (kernel_ms * 1e-3)
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": NCU_DRAM_BYTES.get((cfg, prec)), "kernel": f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
+                "kernel_ms": kernel_ms, "flops_per_ray_step": FLOPS_PER_RAY_STEP[cfg],
+                "peak_source": f"rt_fma_peak({prec}) measured in this process after the timed region: "
+                               f"{peak_after / 1e12:.3f} T{'D' if prec == 'f64' else 'F'}FMA/s at {peak_mhz:.0f} MHz "
+                               f"(before: {peak_before / 1e12:.3f})"}
+    extra = None
+    if rank == 0 and world == 1 and not args.no_extra and not args.n_rays:
+        job.close()
+        del job
+        torch.cuda.empty_cache()
+        extra = []
+        for c, p in ((2, "f64"), (2, "f32"), (3, "f64"), (4, "f32"), (5, "f64"), (5, "f32")):
+            if (c, p) == (cfg, prec):
+                continue
+            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 0)
+            _, kms = time_steps(torch, j, 3, 1, flush)
+            pk, _ = rt.fma_peak(p, 100.0)
+            extra.append({"workload": f"cfg{c}", "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
+                          "roofline_frac": FLOPS_PER_RAY_STEP[c] * j.ray_steps / (kms * 1e-3) / (2.0 * pk)})
+            j.close()
+            del j
+            torch.cuda.empty_cache()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(cfg)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": prec, "data": "synthetic",
+                "config": {"workload": WORKLOAD_NAMES[cfg], "n_rays_per_gpu": n_rays, "n_steps": inputs.FULL_SIZES[cfg][1],
+                           "l2": "flushed between steps (256 MiB memset)", "sharding": "independent ray batches per GPU, no collective",
+                           "launch_states": "rt_launch kernel, max |D0| = %.1e" % launch_residual},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "checks": {"max_abs_D": red[0], "mean_abs_D": red[1] / max(red[2], 1.0), "status_counts": red[3:6]},
+                "cpu_baseline": cpu, "other_configs": extra}
+        print(json.dumps(line))
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main() -> int:
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -2,8 +2,8 @@
 same seeded inputs.
 
 Tolerances: north_star's relative 1e-10 on final (x, k) for fp64 and 1e-4 for fp32, per-ray
-2-norms (reading A15).  |D| is a cancellation residue, so it is compared absolutely: 64 ulp of the O(1) terms it is
-the difference of, plus 1e-6 of its own size.  Integer outputs (status, inside flags) must be equal.
+2-norms (reading A15).  |D| is a cancellation residue of O(1) terms, so it is compared absolutely and at one and the
+same state (see _check_residual): 64 ulp.  Integer outputs (status, inside flags) must be equal.
 Launch wave vectors k0 come from oracle.launch and the same bytes go to both sides (reading A17); rt_launch has its own
 parity test.
 """
@@ -52,11 +52,19 @@ def _workload(oracle, cfg, n_rays, n_steps, disp=None):
     return w, oeq, k0
 
 
-def _check_residual(got, ref, prec):
-    got, ref = np.asarray(got, dtype=np.float64), np.asarray(ref)
-    assert np.array_equal(np.isnan(got), np.isnan(ref))
+def _check_residual(oracle, oeq, w, states, got, ref, prec):
+    """|D| is a cancellation residue of O(1) terms, so it can only be compared at one and the same state: the oracle's
+    plain-double D is evaluated AT THE STATES THE KERNEL WROTE ([..., 6, n]) and must match the kernel's |D| to 64 ulp of
+    those O(1) terms.  Against the oracle's own residual (taken at the oracle's states, which differ from the kernel's
+    by the allowed state error times |grad D|) only NaN pattern and magnitude are asserted."""
+    got, ref, states = np.asarray(got, dtype=np.float64), np.asarray(ref), np.asarray(states, dtype=np.float64)
+    assert got.shape == ref.shape and np.array_equal(np.isnan(got), np.isnan(ref))
+    st = np.moveaxis(states, -2, 0).reshape(6, -1)
+    D_at = np.abs(oracle.dispersion_value(oeq, w.disp, st[:3], st[3:], w.omega)).reshape(got.shape)
     ok = ~np.isnan(ref)
-    assert (np.abs(got[ok] - ref[ok]) <= RES_ATOL[prec] + 1e-6 * np.abs(ref[ok])).all(), np.abs(got[ok] - ref[ok]).max()
+    assert np.array_equal(np.isnan(D_at), ~ok)
+    assert (np.abs(got[ok] - D_at[ok]) <= RES_ATOL[prec]).all(), np.abs(got[ok] - D_at[ok]).max()
+    assert np.abs(got[ok] - ref[ok]).max() <= (1e-11 if prec == "f64" else 1e-3)
 
 
 # --------------------------------------------------------------------------------- one stage: D and the ray RHS
@@ -119,7 +127,7 @@ def test_trace_final_state_parity(rt, oracle, cfg, n_steps, precs):
         ex, ek = rel_err_xk(_host(out["final"]), ref["final"])
         assert ex < TOL[prec] and ek < TOL[prec], (cfg, prec, ex, ek)
         assert np.array_equal(_host(out["status"]), ref["status"])
-        _check_residual(_host(out["residual"]), ref["residual"], prec)
+        _check_residual(oracle, oeq, w, _host(out["final"]), _host(out["residual"]), ref["residual"], prec)
     eq.close()
 
 
@@ -138,7 +146,7 @@ def test_trajectory_samples_parity(rt, oracle, cfg, n_steps, stride):
         assert ex < 1e-10 and ek < 1e-10, (m, ex, ek)
     np.testing.assert_allclose(tr[0, :3], w.x0, rtol=0, atol=0)                   # sample 0 = launch state
     np.testing.assert_allclose(_host(out["final"]), tr[-1], rtol=0, atol=0)       # final = last sample, bit for bit
-    _check_residual(_host(out["residual"]), ref["residual"], "f64")
+    _check_residual(oracle, oeq, w, tr, _host(out["residual"]), ref["residual"], "f64")
     np.testing.assert_array_equal(_host(out["residual"])[-1], _host(
         rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), w.omega, n_steps, w.dt)["residual"]))
     eq.close()
@@ -201,7 +209,7 @@ def test_rays_leaving_the_domain_freeze_identically(rt, oracle, cfg):
     assert np.array_equal(_host(out["status"]), ref["status"])
     ex, ek = rel_err_xk(_host(out["final"]), ref["final"])
     assert ex < 1e-10 and ek < 1e-10
-    _check_residual(_host(out["residual"]), ref["residual"], "f64")
+    _check_residual(oracle, oeq, w, _host(out["traj"]), _host(out["residual"]), ref["residual"], "f64")
     eq.close()
 
 
