@@ -294,6 +294,8 @@ def reduce(residual, status=None):
     n = ref.numel()
     if residual is not None and not residual.is_contiguous():
         raise ValueError("residual must be contiguous")
+    if status is not None and (status.numel() != n or status.dtype != torch.int32 or not status.is_contiguous()):
+        raise ValueError("status must be a contiguous int32 tensor with as many entries as residual")
     _check(lib.rt_reduce(prec, _ptr(residual), _ptr(status), n, _ptr(out), _stream()))
     return out
 
