@@ -499,9 +499,9 @@ int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_cloc
   auto run = [&](long long iters, float* ms) -> int {
     RT_CUDA(cudaEventRecord(e0, 0));
     if (precision == RT_F64)
-      rt::fma_peak_kernel<double><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 1.0000001, 1e-9, clk);
+      rt::fma_peak_kernel<double><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 1e-9, clk);
     else
-      rt::fma_peak_kernel<float><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1.0001f, 1e-6f, clk);
+      rt::fma_peak_kernel<float><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1e-7f, clk);
     ++g_launches;
     RT_CUDA(cudaGetLastError());
     RT_CUDA(cudaEventRecord(e1, 0));

@@ -210,11 +210,16 @@ def test_rays_leaving_the_domain_freeze_identically(rt, oracle, cfg):
     fin = _host(out["final"])
     ex, ek = rel_err_xk(fin[:, 1::2], ref["final"][:, 1::2])
     assert ex < 1e-10 and ek < 1e-10, (ex, ek)
-    # the frozen rays stopped on the same step (a one-step difference would be ~1e-3).  Their last stretch runs where
-    # n_e -> 0 and the two roots of the full determinant merge (hard part 6): the right-hand side is
-    # ill-conditioned there, so rounding differences are amplified beyond the 1e-10 of well-conditioned rays.
+    # The frozen rays stopped on the same step (a one-step difference would be ~1e-3).  Their last stretch runs where
+    # n_e -> 0 (X ~ 1e-6 at rho -> 1 on the grid) and the two roots of the full determinant merge (hard
+    # part 6): the right-hand side is ill-conditioned there.  The tolerance is therefore derived from the oracle's own
+    # sensitivity: re-run it with the launch positions perturbed by 1e-15 relative and allow 50x that spread.
+    x1 = w.x0 * (1.0 + 1e-15 * np.random.default_rng(0).normal(size=w.x0.shape))
+    ref1 = oracle.trace(oeq, w.disp, x1, k0, w.omega, 300, w.dt)
+    sx, sk = rel_err_xk(ref1["final"][:, ::2], ref["final"][:, ::2])
     ex, ek = rel_err_xk(fin[:, ::2], ref["final"][:, ::2])
-    assert ex < 1e-7 and ek < 1e-7, (ex, ek)
+    assert ex < max(1e-10, 50 * sx) and ek < max(1e-10, 50 * sk), (ex, ek, sx, sk)
+    assert ex < 1e-4 and ek < 1e-4
     _check_residual(oracle, oeq, w, _host(out["traj"]), _host(out["residual"]), ref["residual"], "f64")
     eq.close()
 
@@ -289,7 +294,9 @@ def test_launch_solver_parity(rt, oracle, cfg, disp, branch):
     ok = np.isfinite(k_ref).all(axis=0)
     assert ok.sum() > 900
     err = np.linalg.norm(k[:, ok] - k_ref[:, ok], axis=0) / np.linalg.norm(k_ref[:, ok], axis=0)
-    assert err.max() < 1e-13, err.max()
+    # the two sides stop Newton at slightly different |D| < 1e-15; |n| then differs by that over |dD/d|n||, which is
+    # small where the O and X roots nearly merge (root splitting 1.8e-3 at rho = 0.95)
+    assert err.max() < 1e-12, err.max()
     assert np.abs(D[ok]).max() < 2e-15          # L159's |D| < 1e-15 criterion (plus one rounding of re-evaluation)
     # the oracle agrees that the GPU's launch states are on-shell
     D_chk = oracle.dispersion_value(oeq, disp, w.x0[:, ok], k[:, ok], w.omega)
@@ -368,6 +375,6 @@ def test_fma_peak_is_plausible(rt):
     f64, mhz = rt.fma_peak("f64", 50.0)
     f32, _ = rt.fma_peak("f32", 50.0)
     # B200: 148 SMs x 64 FP64 (128 FP32) lanes x ~1.5-2 GHz
-    assert 0.8e13 < f64 < 2.5e13, f64
-    assert 1.6e13 < f32 < 5.0e13, f32
+    assert 1.4e13 < f64 < 2.0e13, f64          # nominal 64 x 148 x 1.965e9 = 1.86e13
+    assert 2.8e13 < f32 < 4.0e13, f32
     assert 900 < mhz < 2200, mhz
