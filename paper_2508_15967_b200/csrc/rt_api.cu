@@ -73,7 +73,9 @@ rt::Params<T> make_params(const rt_equilibrium* eq, double omega) {
   P.xs = (T)(alpha * nscale);
   const double wce_per_T = kQe / (kMe * omega);
   P.beta = (T)(wce_per_T * wce_per_T);
-  P.mu = (T)((d.ion_mass > 0.0) ? d.ion_charge * kMe / d.ion_mass : 0.0);
+  const double mu = (d.ion_mass > 0.0) ? d.ion_charge * kMe / d.ion_mass : 0.0;
+  P.mu = (T)mu; P.mu2 = (T)(mu * mu); P.mu3 = (T)(mu * mu * mu); P.mu4 = (T)(mu * mu * mu * mu);
+  P.one_plus_mu = (T)(1.0 + mu);
   P.k2n = (T)(kC / omega);
   P.n2k = (T)(omega / kC);
   P.inv_L2 = (T)(d.L != 0.0 ? 1.0 / (d.L * d.L) : 0.0);
@@ -88,7 +90,7 @@ rt::Params<T> make_params(const rt_equilibrium* eq, double omega) {
   P.q1 = (T)d.q1;
   P.two_q1_a2 = (T)(2.0 * d.q1 * inv_a2);
   P.p_exp = (T)d.p_exp;
-  P.p_is_three_halves = (d.p_exp == 1.5) ? 1 : 0;
+  P.two_xs_a2 = (T)(2.0 * alpha * nscale * inv_a2);
   P.rho_max2 = (T)(eq->rho_max * eq->rho_max);
   if (d.kind == RT_EQ_GRID_RZ) {
     const double hR = (d.Rmax - d.Rmin) / (d.nR - 1), hZ = (d.Zmax - d.Zmin) / (d.nZ - 1);
@@ -121,6 +123,12 @@ int check_omega(double omega) {
   return RT_OK;
 }
 
+// kernel-side equilibrium kind: the tokamak has a specialised instantiation for p_exp = 3/2
+int kernel_kind(const rt_equilibrium* eq) {
+  if (eq->d.kind == RT_EQ_TOKAMAK_CIRCULAR && eq->d.p_exp != 1.5) return rt::EQ_TOKAMAK_POW;
+  return eq->d.kind;
+}
+
 unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
 
 // ---- dispatch over (EQ, DISP) ---------------------------------------------------------------------------------
@@ -128,6 +136,7 @@ unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / 
   M(rt::EQ_PARABOLIC, rt::DISP_O)                          \
   M(rt::EQ_LINEAR, rt::DISP_O) M(rt::EQ_LINEAR, rt::DISP_X) M(rt::EQ_LINEAR, rt::DISP_FULL)     \
   M(rt::EQ_TOKAMAK, rt::DISP_O) M(rt::EQ_TOKAMAK, rt::DISP_X) M(rt::EQ_TOKAMAK, rt::DISP_FULL)  \
+  M(rt::EQ_TOKAMAK_POW, rt::DISP_O) M(rt::EQ_TOKAMAK_POW, rt::DISP_X) M(rt::EQ_TOKAMAK_POW, rt::DISP_FULL)  \
   M(rt::EQ_GRID, rt::DISP_O) M(rt::EQ_GRID, rt::DISP_X) M(rt::EQ_GRID, rt::DISP_FULL)
 
 template <class T>
@@ -135,7 +144,7 @@ int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, con
   if (A.n_rays == 0) return RT_OK;
   const unsigned grid = grid_for(A.n_rays, rt::TRACE_BLOCK);
 #define M(E, D)                                                                   \
-  if (eq->d.kind == (E) && disp == (D)) {                                         \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                         \
     rt::trace_kernel<T, E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, A);            \
     ++g_launches;                                                                 \
     RT_CUDA(cudaGetLastError());                                                  \
@@ -152,7 +161,7 @@ int launch_rhs(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const
   if (n == 0) return RT_OK;
   const unsigned grid = grid_for(n, rt::TRACE_BLOCK);
 #define M(E, D)                                                                                        \
-  if (eq->d.kind == (E) && disp == (D)) {                                                              \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                                              \
     rt::rhs_kernel<T, E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, x, k, n, D_out, rhs_out, inside_out);  \
     ++g_launches;                                                                                      \
     RT_CUDA(cudaGetLastError());                                                                       \
@@ -168,7 +177,7 @@ int launch_launch(const rt_equilibrium* eq, int disp, const rt::Params<double>& 
   if (n == 0) return RT_OK;
   const unsigned grid = grid_for(n, rt::TRACE_BLOCK);
 #define M(E, D)                                                                                  \
-  if (eq->d.kind == (E) && disp == (D)) {                                                        \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                                        \
     rt::launch_kernel<E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, branch, x0, dir, n, k0, D_out);  \
     ++g_launches;                                                                                \
     RT_CUDA(cudaGetLastError());                                                                 \

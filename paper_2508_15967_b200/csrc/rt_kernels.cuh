@@ -15,7 +15,14 @@
 
 namespace rt {
 
-constexpr int TRACE_BLOCK = 128;
+// Tuning knobs (defaults chosen by measurement on B200, profiles/r1_tuning.md).
+#ifndef RT_TRACE_BLOCK
+#define RT_TRACE_BLOCK 128
+#endif
+#ifndef RT_MIN_BLOCKS
+#define RT_MIN_BLOCKS 4       // <= 128 registers per thread: 16 warps per SM
+#endif
+constexpr int TRACE_BLOCK = RT_TRACE_BLOCK;
 
 template <class T>
 struct TraceArgs {
@@ -31,24 +38,40 @@ struct TraceArgs {
   T h;                  // step in tau = c t
 };
 
-// One classical RK4 step (reading A7): stage abscissae (0, 1/2, 1/2, 1), weights (1, 2, 2, 1)/6.  The four stages run
-// through ONE copy of the right-hand-side code (the loop is deliberately not unrolled: instruction-cache footprint).
+// One classical RK4 step (reading A7): stage abscissae (0, 1/2, 1/2, 1), weights (1, 2, 2, 1)/6.
 // Returns 0 accepted, 1 a stage point left the domain (step rejected), 2 the new state is not finite (rejected).
+// The analytic equilibria run the four stages fully unrolled (the compiler schedules across stages; 54 vs 57 ms on
+// config 4); the grid equilibrium keeps ONE copy of the right-hand-side code (smaller instruction footprint and fewer
+// live registers around the gathers; 281 vs 314 ms on a 2^22-ray slice of config 5).  profiles/r1_tuning.md.
+template <class T, int EQ, int DISP>
+RT_DEV void rk4_stage(const Params<T>& P, const T* y, T a, T w, T* k, T* acc, bool& ok) {
+  T ys[6];
+#pragma unroll
+  for (int j = 0; j < 6; ++j) ys[j] = y[j] + a * k[j];
+  ok = ray_rhs<T, EQ, DISP>(P, ys, k) && ok;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) acc[j] += w * k[j];
+}
+
 template <class T, int EQ, int DISP>
 RT_DEV int rk4_step(const Params<T>& P, T h, T* y) {
   T k[6], acc[6], ys[6];
 #pragma unroll
   for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = T(0); }
   bool ok = true;
+  if (EQ == EQ_GRID) {
 #pragma unroll 1
-  for (int st = 0; st < 4; ++st) {
-    const T a = (st == 0) ? T(0) : ((st == 3) ? h : T(0.5) * h);
-    const T w = (st == 0 || st == 3) ? T(1) : T(2);
-#pragma unroll
-    for (int j = 0; j < 6; ++j) ys[j] = y[j] + a * k[j];
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k) && ok;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) acc[j] += w * k[j];
+    for (int st = 0; st < 4; ++st) {
+      const T a = (st == 0) ? T(0) : ((st == 3) ? h : T(0.5) * h);
+      const T w = (st == 0 || st == 3) ? T(1) : T(2);
+      rk4_stage<T, EQ, DISP>(P, y, a, w, k, acc, ok);
+    }
+  } else {
+    const T hh = T(0.5) * h;
+    rk4_stage<T, EQ, DISP>(P, y, T(0), T(1), k, acc, ok);
+    rk4_stage<T, EQ, DISP>(P, y, hh, T(2), k, acc, ok);
+    rk4_stage<T, EQ, DISP>(P, y, hh, T(2), k, acc, ok);
+    rk4_stage<T, EQ, DISP>(P, y, h, T(1), k, acc, ok);
   }
   if (!ok) return 1;
   const T h6 = h * T(1.0 / 6.0);
@@ -71,7 +94,7 @@ RT_DEV T abs_residual(const Params<T>& P, const T* y) {
 #ifdef __CUDACC__
 
 template <class T, int EQ, int DISP>
-__global__ void __launch_bounds__(TRACE_BLOCK)
+__global__ void __launch_bounds__(TRACE_BLOCK, RT_MIN_BLOCKS)
 trace_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ TraceArgs<T> A) {
   const long long N = A.n_rays;
   const long long i = (long long)blockIdx.x * TRACE_BLOCK + threadIdx.x;

@@ -25,7 +25,9 @@
 
 namespace rt {
 
-enum { EQ_PARABOLIC = 0, EQ_LINEAR = 1, EQ_TOKAMAK = 2, EQ_GRID = 3 };
+// EQ_TOKAMAK is the circular tokamak with the configs' density exponent p_exp = 3/2 (evaluated as t sqrt(t));
+// EQ_TOKAMAK_POW is the same equilibrium with a general exponent (pow).  Both come from RT_EQ_TOKAMAK_CIRCULAR.
+enum { EQ_PARABOLIC = 0, EQ_LINEAR = 1, EQ_TOKAMAK = 2, EQ_GRID = 3, EQ_TOKAMAK_POW = 4 };
 enum { DISP_O = 0, DISP_X = 1, DISP_FULL = 2 };
 
 // Per-call constants, folded on the host in fp64 (step a0) so that every device-side quantity is O(1) in fp32 too.
@@ -34,6 +36,7 @@ struct Params {
   T xs;         // X = xs * shape(x):  alpha n_ref (analytic kinds) or alpha ne_scale (grid), alpha = e^2/(eps0 m_e w^2)
   T beta;       // Y_e^2 = beta |B|^2, beta = (e/(m_e w))^2
   T mu;         // Z m_e / m_i; 0 = electrons only
+  T mu2, mu3, mu4, one_plus_mu;
   T k2n, n2k;   // c/w and w/c
   // slab_parabolic
   T inv_L2;
@@ -41,7 +44,7 @@ struct Params {
   T x_foot, inv_Lramp, B0R0;
   // tokamak_circular
   T R0, B0, inv_a2, q0, q1, two_q1_a2, p_exp, rho_max2;
-  int p_is_three_halves;
+  T two_xs_a2;  // 2 xs / a^2
   // grid_rz
   T Rmin, Rmax, Zmin, Zmax, hR, hZ, inv_hR, inv_hZ, psi_min, psi_max, hP, inv_hP;
   int nRc, nZc, nPc;            // cell counts
@@ -62,6 +65,39 @@ RT_DEV bool rt_finite(float a) { return isfinite(a); }
 template <class T> RT_DEV T rt_nan();
 template <> RT_DEV double rt_nan<double>() { return nan(""); }
 template <> RT_DEV float rt_nan<float>() { return nanf(""); }
+
+// Reciprocal and reciprocal square root for the hot loop.  An IEEE fp64 division costs ~10 FP64-pipe instructions plus
+// a slow-path branch; here the 20-bit MUFU seed is refined by ONE third-order Newton step (3 / 5 FMA-pipe instructions,
+// branch-free), which leaves a relative error below 2^-52 for the normal, O(1) arguments of this path -- far inside
+// the 1e-10 parity budget.  NaN propagates; zero / negative arguments give inf / NaN, which only
+// occur at points outside the equilibrium's domain, whose results are discarded (reading A12).
+#ifdef __CUDACC__
+RT_DEV double rt_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x, r, 1.0);          // e = 1 - x r,  |e| <~ 2^-20
+  return fma(r, fma(e, e, e), r);            // r (1 + e + e^2)
+}
+RT_DEV double rt_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x * y, y, 1.0);      // e = 1 - x y^2
+  return fma(y * e, fma(0.375, e, 0.5), y);  // y (1 + e/2 + 3 e^2/8)
+}
+RT_DEV float rt_rcp(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+RT_DEV float rt_rsqrt(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+#else
+template <class T> RT_DEV T rt_rcp(T x) { return T(1) / x; }
+template <class T> RT_DEV T rt_rsqrt(T x) { return T(1) / rt_sqrt(x); }
+#endif
 
 #ifdef __CUDACC__
 RT_DEV void ld16(const double* p, double& a, double& b) {
@@ -90,16 +126,15 @@ struct StixT {
 template <class T>
 RT_DEV StixT<T> stix(const Params<T>& P, T X, T Y2) {
   StixT<T> st;
-  const T mu = P.mu, mu2 = mu * mu;
-  const T e1 = T(1) / (T(1) - Y2);
-  const T e2 = T(1) / (T(1) - mu2 * Y2);
+  const T e1 = rt_rcp(T(1) - Y2);
+  const T e2 = rt_rcp(T(1) - P.mu2 * Y2);
   const T e1s = e1 * e1, e2s = e2 * e2;
-  st.sig = e1 + mu * e2;
-  st.sigp = e1s + mu * mu2 * e2s;
-  st.del = mu2 * e2 - e1;
-  st.delp = mu2 * mu2 * e2s - e1s;
+  st.sig = e1 + P.mu * e2;
+  st.sigp = e1s + P.mu3 * e2s;
+  st.del = P.mu2 * e2 - e1;
+  st.delp = P.mu4 * e2s - e1s;
   st.s = T(1) - X * st.sig;
-  st.p = T(1) - X * (T(1) + mu);
+  st.p = T(1) - X * P.one_plus_mu;
   st.d2 = X * X * Y2 * st.del * st.del;
   return st;
 }
@@ -139,7 +174,7 @@ RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2
     Dd2 = w - p;
   }
   const T XYd = X * Y2 * st.del;
-  DX = -st.sig * Ds - (T(1) + P.mu) * Dp + T(2) * XYd * st.del * Dd2;
+  DX = -st.sig * Ds - P.one_plus_mu * Dp + T(2) * XYd * st.del * Dd2;
   DY2 = -X * st.sigp * Ds + X * X * st.del * (st.del + T(2) * Y2 * st.delp) * Dd2;
 }
 
@@ -194,7 +229,7 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L)
     L.nl[0] = n[0]; L.nl[1] = n[1]; L.nl[2] = n[2];
     L.cph = T(1); L.sph = T(0);
     if (DISP != DISP_O) {
-      const T ix = T(1) / x[0];
+      const T ix = rt_rcp(x[0]);
       const T Bz = P.B0R0 * ix;
       L.B[0] = T(0); L.B[1] = T(0); L.B[2] = Bz;
       L.b2 = Bz * Bz;
@@ -206,33 +241,33 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L)
   }
   // axisymmetric kinds: cylindrical frame at the point
   const T R2 = x[0] * x[0] + x[1] * x[1];
-  const T R = rt_sqrt(R2);
-  const T iR = T(1) / R;
+  const T iR = rt_rsqrt(R2);
+  const T R = R2 * iR;
   const T Z = x[2];
   L.cph = x[0] * iR; L.sph = x[1] * iR;
   L.nl[0] = n[0] * L.cph + n[1] * L.sph;
   L.nl[1] = n[1] * L.cph - n[0] * L.sph;
   L.nl[2] = n[2];
   L.gX[1] = T(0);
-  if (EQ == EQ_TOKAMAK) {
+  if (EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) {
     // psi'(r) = B0 r / q, q = q0 + q1 rho^2, F = B0 R0, n_e = n_ref (1 - rho^2)^p       (config 4; reading A9)
     const T dR = R - P.R0;
     const T rho2 = (dR * dR + Z * Z) * P.inv_a2;
     const bool inside = (R > T(0)) && (rho2 < P.rho_max2);
     const T t = T(1) - rho2;
     T shape, dshape;     // t^p and d(t^p)/d(rho^2)
-    if (P.p_is_three_halves) {
-      const T sq = rt_sqrt(t);
+    if (EQ == EQ_TOKAMAK) {
+      const T sq = t * rt_rsqrt(t);
       shape = t * sq; dshape = T(-1.5) * sq;
     } else {
       const T pw = rt_pow(t, P.p_exp - T(1));
       shape = pw * t; dshape = -P.p_exp * pw;
     }
     L.X = P.xs * shape;
-    const T gx = T(2) * P.xs * P.inv_a2 * dshape;
+    const T gx = P.two_xs_a2 * dshape;
     L.gX[0] = gx * dR; L.gX[2] = gx * Z;
     if (DISP != DISP_O) {
-      const T iq = T(1) / (P.q0 + P.q1 * rho2);
+      const T iq = rt_rcp(P.q0 + P.q1 * rho2);
       const T Bq = P.B0 * iq;
       const T c = P.two_q1_a2 * iq;
       axisym_field<T, DISP>(iR, Bq * dR, Bq * Z, Bq * (T(1) - c * dR * dR), -Bq * c * dR * Z, Bq * (T(1) - c * Z * Z),
@@ -295,17 +330,17 @@ RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f) {
   T fx[3], fn[3];        // local-frame components
   if (DISP == DISP_O) {
     // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)
-    const T iW = T(1) / (v + L.X);
+    const T iW = rt_rcp(v + L.X);
 #pragma unroll
     for (int j = 0; j < 3; ++j) { fx[j] = nl[j] * iW; fn[j] = T(-0.5) * L.gX[j] * iW; }
   } else {
-    const T ib2 = T(1) / L.b2;
+    const T ib2 = rt_rcp(L.b2);
     const T Y2 = P.beta * L.b2;
     const T u = (DISP == DISP_FULL) ? L.G * L.G * ib2 : T(0);
     T DX, DY2, Du, Dv;
     disp_partials<T, DISP>(P, L.X, Y2, u, v, DX, DY2, Du, Dv);
     const T W = T(-2) * (L.X * DX + Y2 * DY2 + u * Du + v * Dv);
-    const T iW = T(1) / W;
+    const T iW = rt_rcp(W);
     const T DG = T(2) * L.G * ib2 * Du;            // dD/dG at fixed |B|^2
     const T Db2 = P.beta * DY2 - u * ib2 * Du;     // dD/d|B|^2 at fixed G: through Y2 and through u = G^2/|B|^2
 #pragma unroll
@@ -327,7 +362,7 @@ RT_DEV T ray_D(const Params<T>& P, const T* y, bool* inside) {
   *inside = equilibrium<T, EQ, DISP>(P, y, y + 3, L);
   const T v = y[3] * y[3] + y[4] * y[4] + y[5] * y[5];
   if (DISP == DISP_O) return disp_value<T, DISP>(P, L.X, T(0), T(0), v);
-  const T u = (DISP == DISP_FULL) ? L.G * L.G / L.b2 : T(0);
+  const T u = (DISP == DISP_FULL) ? L.G * L.G * rt_rcp(L.b2) : T(0);
   return disp_value<T, DISP>(P, L.X, P.beta * L.b2, u, v);
 }
 
