@@ -13,15 +13,10 @@
 
 #include "../../include/rt.h"
 #include "rt_kernels.cuh"
+#include "rt_params.h"
 #include "spline_fit.h"
 
 namespace {
-
-// CODATA-2022 numerals (reading A6)
-constexpr double kC = 299792458.0;          // m/s
-constexpr double kQe = 1.602176634e-19;     // C
-constexpr double kMe = 9.1093837139e-31;    // kg
-constexpr double kEps0 = 8.8541878188e-12;  // F/m
 
 thread_local std::string g_err;
 std::atomic<long long> g_launches{0};
@@ -65,49 +60,11 @@ namespace {
 
 template <class T>
 rt::Params<T> make_params(const rt_equilibrium* eq, double omega) {
-  rt::Params<T> P;
-  std::memset(&P, 0, sizeof(P));
-  const rt_equilibrium_desc& d = eq->d;
-  const double alpha = kQe * kQe / (kEps0 * kMe * omega * omega);       // X_e = alpha n_e
-  const double nscale = (d.kind == RT_EQ_GRID_RZ) ? eq->ne_scale : d.n_ref;
-  P.xs = (T)(alpha * nscale);
-  const double wce_per_T = kQe / (kMe * omega);
-  P.beta = (T)(wce_per_T * wce_per_T);
-  const double mu = (d.ion_mass > 0.0) ? d.ion_charge * kMe / d.ion_mass : 0.0;
-  P.mu = (T)mu; P.mu2 = (T)(mu * mu); P.mu3 = (T)(mu * mu * mu); P.mu4 = (T)(mu * mu * mu * mu);
-  P.one_plus_mu = (T)(1.0 + mu);
-  P.k2n = (T)(kC / omega);
-  P.n2k = (T)(omega / kC);
-  P.inv_L2 = (T)(d.L != 0.0 ? 1.0 / (d.L * d.L) : 0.0);
-  P.x_foot = (T)d.x_foot;
-  P.inv_Lramp = (T)(d.L_ramp != 0.0 ? 1.0 / d.L_ramp : 0.0);
-  P.B0R0 = (T)(d.B0 * d.R0);
-  P.R0 = (T)d.R0;
-  P.B0 = (T)d.B0;
-  const double inv_a2 = d.a != 0.0 ? 1.0 / (d.a * d.a) : 0.0;
-  P.inv_a2 = (T)inv_a2;
-  P.q0 = (T)d.q0;
-  P.q1 = (T)d.q1;
-  P.two_q1_a2 = (T)(2.0 * d.q1 * inv_a2);
-  P.p_exp = (T)d.p_exp;
-  P.two_xs_a2 = (T)(2.0 * alpha * nscale * inv_a2);
-  P.rho_max2 = (T)(eq->rho_max * eq->rho_max);
-  if (d.kind == RT_EQ_GRID_RZ) {
-    const double hR = (d.Rmax - d.Rmin) / (d.nR - 1), hZ = (d.Zmax - d.Zmin) / (d.nZ - 1);
-    const double hP = (d.psi_max - d.psi_min) / (d.nPsi - 1);
-    P.Rmin = (T)d.Rmin; P.Rmax = (T)d.Rmax; P.Zmin = (T)d.Zmin; P.Zmax = (T)d.Zmax;
-    P.hR = (T)hR; P.hZ = (T)hZ; P.inv_hR = (T)(1.0 / hR); P.inv_hZ = (T)(1.0 / hZ);
-    P.psi_min = (T)d.psi_min; P.psi_max = (T)d.psi_max; P.hP = (T)hP; P.inv_hP = (T)(1.0 / hP);
-    P.nRc = d.nR - 1; P.nZc = d.nZ - 1; P.nPc = d.nPsi - 1;
-    if (sizeof(T) == 8) {
-      P.psi_pp = reinterpret_cast<const T*>(eq->psi_pp64);
-      P.prof_pp = reinterpret_cast<const T*>(eq->prof_pp64);
-    } else {
-      P.psi_pp = reinterpret_cast<const T*>(eq->psi_pp32);
-      P.prof_pp = reinterpret_cast<const T*>(eq->prof_pp32);
-    }
-  }
-  return P;
+  if (sizeof(T) == 8)
+    return rt::fold_params<T>(eq->d, eq->rho_max, eq->ne_scale, omega, reinterpret_cast<const T*>(eq->psi_pp64),
+                              reinterpret_cast<const T*>(eq->prof_pp64));
+  return rt::fold_params<T>(eq->d, eq->rho_max, eq->ne_scale, omega, reinterpret_cast<const T*>(eq->psi_pp32),
+                            reinterpret_cast<const T*>(eq->prof_pp32));
 }
 
 int check_combo(const rt_equilibrium* eq, int disp) {

@@ -38,66 +38,137 @@ struct TraceArgs {
   T h;                  // step in tau = c t
 };
 
-// One classical RK4 step (reading A7): stage abscissae (0, 1/2, 1/2, 1), weights (1, 2, 2, 1)/6.
+// One classical RK4 step (reading A7): stage abscissae (0, 1/2, 1/2, 1), weights (1, 2, 2, 1)/6, written so that every
+// update is one fused multiply-add: acc = y + h/6 k1 + h/3 k2 + h/3 k3, y_new = acc + h/6 k4 (42 FMAs per step).
 // Returns 0 accepted, 1 a stage point left the domain (step rejected), 2 the new state is not finite (rejected).
-// The analytic equilibria run the four stages fully unrolled (the compiler schedules across stages; 54 vs 57 ms on
-// config 4); the grid equilibrium keeps ONE copy of the right-hand-side code (smaller instruction footprint and fewer
-// live registers around the gathers; 281 vs 314 ms on a 2^22-ray slice of config 5).  profiles/r1_tuning.md.
-template <class T, int EQ, int DISP>
-RT_DEV void rk4_stage(const Params<T>& P, const T* y, T a, T w, T* k, T* acc, bool& ok) {
-  T ys[6];
-#pragma unroll
-  for (int j = 0; j < 6; ++j) ys[j] = y[j] + a * k[j];
-  ok = ray_rhs<T, EQ, DISP>(P, ys, k) && ok;
-#pragma unroll
-  for (int j = 0; j < 6; ++j) acc[j] += w * k[j];
+// The analytic equilibria run the four stages fully unrolled (the compiler schedules across stages); the grid
+// equilibrium keeps ONE copy of the right-hand-side code (smaller instruction footprint and fewer live registers around
+// the gathers).  Components of the right-hand side that are structurally zero (slabs: dn_y/dtau = dn_z/dtau = 0,
+// parabolic: dn_z/dtau = 0) are skipped, which also keeps them bit-for-bit constant.
+template <int EQ>
+RT_DEV constexpr bool rhs_component_active(int j) {
+  return !((EQ == EQ_LINEAR && j >= 4) || (EQ == EQ_PARABOLIC && j == 5));
 }
 
-template <class T, int EQ, int DISP>
-RT_DEV int rk4_step(const Params<T>& P, T h, T* y) {
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
+  const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
   T k[6], acc[6], ys[6];
-#pragma unroll
-  for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = T(0); }
   bool ok = true;
   if (EQ == EQ_GRID) {
+#pragma unroll
+    for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; }
 #pragma unroll 1
     for (int st = 0; st < 4; ++st) {
-      const T a = (st == 0) ? T(0) : ((st == 3) ? h : T(0.5) * h);
-      const T w = (st == 0 || st == 3) ? T(1) : T(2);
-      rk4_stage<T, EQ, DISP>(P, y, a, w, k, acc, ok);
+      const T a = (st == 0) ? T(0) : ((st == 3) ? h : hh);
+      const T w = (st == 0 || st == 3) ? h6 : h3;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) ys[j] = rt_fma(a, k[j], y[j]);
+      ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) acc[j] = rt_fma(w, k[j], acc[j]);
     }
+#pragma unroll
+    for (int j = 0; j < 6; ++j) ys[j] = acc[j];
   } else {
-    const T hh = T(0.5) * h;
-    rk4_stage<T, EQ, DISP>(P, y, T(0), T(1), k, acc, ok);
-    rk4_stage<T, EQ, DISP>(P, y, hh, T(2), k, acc, ok);
-    rk4_stage<T, EQ, DISP>(P, y, hh, T(2), k, acc, ok);
-    rk4_stage<T, EQ, DISP>(P, y, h, T(1), k, acc, ok);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) { ys[j] = y[j]; acc[j] = y[j]; }
+    ok = ray_rhs<T, EQ, DISP>(P, y, k, gather);
+#pragma unroll
+    for (int j = 0; j < 6; ++j)
+      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(h6, k[j], y[j]); ys[j] = rt_fma(hh, k[j], y[j]); }
+    ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+#pragma unroll
+    for (int j = 0; j < 6; ++j)
+      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(h3, k[j], acc[j]); ys[j] = rt_fma(hh, k[j], y[j]); }
+    ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+#pragma unroll
+    for (int j = 0; j < 6; ++j)
+      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(h3, k[j], acc[j]); ys[j] = rt_fma(h, k[j], y[j]); }
+    ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) ys[j] = rhs_component_active<EQ>(j) ? rt_fma(h6, k[j], acc[j]) : y[j];
   }
   if (!ok) return 1;
-  const T h6 = h * T(1.0 / 6.0);
   bool fin = true;
 #pragma unroll
-  for (int j = 0; j < 6; ++j) { ys[j] = y[j] + h6 * acc[j]; fin = fin && rt_finite(ys[j]); }
+  for (int j = 0; j < 6; ++j) fin = fin && rt_finite(ys[j]);
   if (!fin) return 2;
 #pragma unroll
   for (int j = 0; j < 6; ++j) y[j] = ys[j];
   return 0;
 }
 
-template <class T, int EQ, int DISP>
-RT_DEV T abs_residual(const Params<T>& P, const T* y) {
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV T abs_residual(const Params<T>& P, const T* y, Gather& gather) {
   bool inside;
-  const T D = ray_D<T, EQ, DISP>(P, y, &inside);
+  const T D = ray_D<T, EQ, DISP>(P, y, &inside, gather);
   return inside ? rt_abs(D) : rt_nan<T>();
 }
 
 #ifdef __CUDACC__
+
+// Shared-memory cell cache of the grid equilibrium.  A ray moves ~1 mm per RK4 step through 5.9 mm cells, so the 16
+// psi pieces (one 128-B line in fp64) and the 8 profile pieces it needs are the same for many consecutive stages.  Read
+// straight from global memory, every 128-bit load of a warp touches 32 different lines and the L1 data pipe saturates
+// (99.8 % `l1tex__data_pipe_lsu_wavefronts`, FP64 pipe 43 %: profiles/r1_cfg5_ncu.md).  Here each thread keeps its
+// current cell's pieces in its own column of a [chunk][thread] shared array -- 16-byte chunks, consecutive threads in
+// consecutive chunks, so a warp's LDS.128 is 4 conflict-free wavefronts -- and refills the column from global memory
+// only when its cell index changes.  The column is private to the thread: no barrier is needed.
+template <class T> struct Vec16;
+template <> struct Vec16<double> { typedef double2 type; };
+template <> struct Vec16<float> { typedef float4 type; };
+RT_DEV void unpack4(const double2* s, int row, int pitch, double* c) {
+  const double2 a = s[(2 * row) * pitch], b = s[(2 * row + 1) * pitch];
+  c[0] = a.x; c[1] = a.y; c[2] = b.x; c[3] = b.y;
+}
+RT_DEV void unpack4(const float4* s, int row, int pitch, float* c) {
+  const float4 a = s[row * pitch];
+  c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w;
+}
+
+template <class T, int BLOCK>
+struct GatherCached {
+  typedef typename Vec16<T>::type V;
+  static constexpr int PSI_CHUNKS = 16 * sizeof(T) / 16, PROF_CHUNKS = 8 * sizeof(T) / 16;
+  static constexpr int CHUNKS = PSI_CHUNKS + PROF_CHUNKS;
+  V* col;                  // this thread's column: chunk j at col[j * BLOCK]
+  int cell, pcell;         // cached cell indices (-1: nothing cached)
+  RT_DEV void psi_select(const Params<T>& P, int c) {
+    if (c != cell) {
+      const V* g = reinterpret_cast<const V*>(P.psi_pp + (size_t)c * 16);
+#pragma unroll
+      for (int j = 0; j < PSI_CHUNKS; ++j) col[j * BLOCK] = __ldg(g + j);
+      cell = c;
+    }
+  }
+  RT_DEV void prof_select(const Params<T>& P, int c) {
+    if (c != pcell) {
+      const V* g = reinterpret_cast<const V*>(P.prof_pp + (size_t)c * 8);
+#pragma unroll
+      for (int j = 0; j < PROF_CHUNKS; ++j) col[(PSI_CHUNKS + j) * BLOCK] = __ldg(g + j);
+      pcell = c;
+    }
+  }
+  RT_DEV void psi_row(const Params<T>&, int, int p, T* c) const { unpack4(col, p, BLOCK, c); }
+  RT_DEV void prof_row(const Params<T>&, int, int which, T* c) const { unpack4(col + PSI_CHUNKS * BLOCK, which, BLOCK, c); }
+};
+
+template <class T, int EQ> struct TraceGather { typedef GatherDirect type; };
+template <class T> struct TraceGather<T, EQ_GRID> { typedef GatherCached<T, TRACE_BLOCK> type; };
 
 template <class T, int EQ, int DISP>
 __global__ void __launch_bounds__(TRACE_BLOCK, RT_MIN_BLOCKS)
 trace_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ TraceArgs<T> A) {
   const long long N = A.n_rays;
   const long long i = (long long)blockIdx.x * TRACE_BLOCK + threadIdx.x;
+  typename TraceGather<T, EQ>::type gather;
+  if constexpr (EQ == EQ_GRID) {
+    typedef GatherCached<T, TRACE_BLOCK> GC;
+    __shared__ typename GC::V cache[GC::CHUNKS * TRACE_BLOCK];
+    gather.col = cache + threadIdx.x;
+    gather.cell = -1; gather.pcell = -1;
+  }
   if (i >= N) return;
   T y[6];
 #pragma unroll
@@ -113,12 +184,12 @@ trace_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ TraceA
       A.traj[(m * 6 + c) * N + i] = y[c];
       A.traj[(m * 6 + 3 + c) * N + i] = y[3 + c] * P.n2k;
     }
-    if (A.res) A.res[m * N + i] = abs_residual<T, EQ, DISP>(P, y);
+    if (A.res) A.res[m * N + i] = abs_residual<T, EQ, DISP>(P, y, gather);
     ++m;
   }
   long long countdown = A.stride;
   for (long long s = 0; s < A.n_steps; ++s) {
-    if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, y);
+    if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, y, gather);
     if (A.traj && --countdown == 0) {
       countdown = A.stride;
 #pragma unroll
@@ -126,7 +197,7 @@ trace_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ TraceA
         A.traj[(m * 6 + c) * N + i] = y[c];
         A.traj[(m * 6 + 3 + c) * N + i] = y[3 + c] * P.n2k;
       }
-      if (A.res) A.res[m * N + i] = abs_residual<T, EQ, DISP>(P, y);
+      if (A.res) A.res[m * N + i] = abs_residual<T, EQ, DISP>(P, y, gather);
       ++m;
     }
   }
@@ -137,7 +208,7 @@ trace_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ TraceA
       A.fin[(3 + c) * N + i] = y[3 + c] * P.n2k;
     }
   }
-  if (!A.traj && A.res) A.res[i] = abs_residual<T, EQ, DISP>(P, y);
+  if (!A.traj && A.res) A.res[i] = abs_residual<T, EQ, DISP>(P, y, gather);
   if (A.status) A.status[i] = status;
 }
 
@@ -150,14 +221,15 @@ rhs_kernel(const __grid_constant__ Params<T> P, const T* __restrict__ x, const T
   T y[6], f[6];
 #pragma unroll
   for (int c = 0; c < 3; ++c) { y[c] = x[c * n + i]; y[3 + c] = k[c * n + i] * P.k2n; }
-  const bool inside = ray_rhs<T, EQ, DISP>(P, y, f);
+  GatherDirect gather;
+  const bool inside = ray_rhs<T, EQ, DISP>(P, y, f, gather);
   if (rhs_out) {
 #pragma unroll
     for (int c = 0; c < 6; ++c) rhs_out[c * n + i] = inside ? f[c] : T(0);
   }
   if (D_out) {
     bool in2;
-    const T D = ray_D<T, EQ, DISP>(P, y, &in2);
+    const T D = ray_D<T, EQ, DISP>(P, y, &in2, gather);
     D_out[i] = in2 ? D : rt_nan<T>();
   }
   if (inside_out) inside_out[i] = inside ? 1 : 0;
@@ -174,7 +246,8 @@ launch_kernel(const __grid_constant__ Params<double> P, int branch, const double
 #pragma unroll
   for (int c = 0; c < 3; ++c) { x[c] = x0[c * n + i]; d[c] = dir[c * n + i]; }
   Local<double> L;
-  const bool inside = equilibrium<double, EQ, DISP>(P, x, d, L);
+  GatherDirect gather;
+  const bool inside = equilibrium<double, EQ, DISP>(P, x, d, L, gather);
   const double X = L.X;
   double Y2 = 0.0, c2 = 0.0, n2;
   if (DISP == DISP_O) {

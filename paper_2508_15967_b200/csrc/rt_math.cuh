@@ -12,7 +12,15 @@
 //      Y2 = (Wce/w)^2 = beta |B|^2                        (ion: Y_i^2 = mu^2 Y2)
 //      u  = n_par^2   = (n.B)^2/|B|^2
 //      v  = n^2
-// and under w -> lambda w at fixed (x, k) all four scale as lambda^-2, hence W = -2 (X D_X + Y2 D_Y2 + u D_u + v D_v).
+// and under w -> lambda w at fixed (x, k) all four scale as lambda^-2, hence W = -2 s, s = X D_X + Y2 D_Y2 + u D_u + v D_v.
+//
+// The hot path never forms D's gradient vectors and divides them by W component by component.  With r = 1/s, G = n.B:
+//      dx/dtau = A n + C B ,                         A = D_v r,            C = (G/|B|^2) D_u r
+//      dn/dtau = Ax grad X + Ab (grad |B|^2)/2 - C grad_x(n.B)|_n ,
+//                                                    Ax = -D_X r/2,        Ab = -(beta D_Y2 - u D_u/|B|^2) r
+// so the reciprocal is folded into four scalars (disp_coefs) before anything multiplies a vector, and every structural
+// zero of an equilibrium (slab: only d/dx; axisymmetric: no d/dphi of X and |B|^2) is skipped at compile time -- the
+// FP64 pipe is the roofline of this path, so the instruction count per stage is what is optimised.
 #pragma once
 
 #include <math.h>
@@ -30,20 +38,22 @@ namespace rt {
 enum { EQ_PARABOLIC = 0, EQ_LINEAR = 1, EQ_TOKAMAK = 2, EQ_GRID = 3, EQ_TOKAMAK_POW = 4 };
 enum { DISP_O = 0, DISP_X = 1, DISP_FULL = 2 };
 
-// Per-call constants, folded on the host in fp64 (step a0) so that every device-side quantity is O(1) in fp32 too.
+// Per-call constants, folded on the host in fp64 (step a0, rt_params.h) so that every device-side quantity is O(1) in
+// fp32 too.
 template <class T>
 struct Params {
   T xs;         // X = xs * shape(x):  alpha n_ref (analytic kinds) or alpha ne_scale (grid), alpha = e^2/(eps0 m_e w^2)
   T beta;       // Y_e^2 = beta |B|^2, beta = (e/(m_e w))^2
+  T beta2;      // 2 beta
   T mu;         // Z m_e / m_i; 0 = electrons only
   T mu2, mu3, mu4, one_plus_mu;
   T k2n, n2k;   // c/w and w/c
-  // slab_parabolic
-  T inv_L2;
-  // slab_linear_br
-  T x_foot, inv_Lramp, B0R0;
+  // slab_parabolic:  X = xs + par_g (x^2 + y^2)
+  T par_g;      // xs / L^2
+  // slab_linear_br:  X = (x - x_foot) lin_gx
+  T x_foot, lin_gx, B0R0;   // lin_gx = -xs / L_ramp
   // tokamak_circular
-  T R0, B0, inv_a2, q0, q1, two_q1_a2, p_exp, rho_max2;
+  T R0, B0, inv_a2, q0, q1_a2, two_q1_a2, p_exp, rmax2;   // q = q0 + q1_a2 r^2;  domain r^2 < rmax2 = (rho_max a)^2
   T two_xs_a2;  // 2 xs / a^2
   // grid_rz
   T Rmin, Rmax, Zmin, Zmax, hR, hZ, inv_hR, inv_hZ, psi_min, psi_max, hP, inv_hP;
@@ -60,6 +70,8 @@ RT_DEV double rt_floor(double a) { return floor(a); }
 RT_DEV float rt_floor(float a) { return floorf(a); }
 RT_DEV double rt_abs(double a) { return fabs(a); }
 RT_DEV float rt_abs(float a) { return fabsf(a); }
+RT_DEV double rt_fma(double a, double b, double c) { return fma(a, b, c); }
+RT_DEV float rt_fma(float a, float b, float c) { return fmaf(a, b, c); }
 RT_DEV bool rt_finite(double a) { return isfinite(a); }
 RT_DEV bool rt_finite(float a) { return isfinite(a); }
 template <class T> RT_DEV T rt_nan();
@@ -113,6 +125,34 @@ RT_DEV void ld4(const float* p, float* c) {
 template <class T> RT_DEV void ld4(const T* p, T* c) { for (int i = 0; i < 4; ++i) c[i] = p[i]; }
 #endif
 
+// How the grid equilibrium fetches a cell's spline pieces.  GatherDirect reads the global tables (diagnostic kernels,
+// launch solver, host builds); the trace kernel passes a shared-memory cell cache instead (rt_kernels.cuh: GatherCached).
+struct GatherDirect {
+  template <class T> RT_DEV void psi_select(const Params<T>&, int) {}
+  template <class T> RT_DEV void prof_select(const Params<T>&, int) {}
+  template <class T> RT_DEV void psi_row(const Params<T>& P, int cell, int p, T* c) const { ld4(P.psi_pp + (size_t)cell * 16 + 4 * p, c); }
+  template <class T> RT_DEV void prof_row(const Params<T>& P, int cell, int which, T* c) const { ld4(P.prof_pp + (size_t)cell * 8 + 4 * which, c); }
+};
+
+// Cubic c0 + c1 s + c2 s^2 + c3 s^3 with its first derivative and HALF its second derivative in 6 fused multiply-adds
+// (Horner's scheme, the derivative chains reusing the partial sums).
+template <class T>
+RT_DEV void cubic012(const T* c, T s, T& f, T& f1, T& f2h) {
+  const T b1 = rt_fma(c[3], s, c[2]);
+  const T b0 = rt_fma(b1, s, c[1]);
+  f = rt_fma(b0, s, c[0]);
+  const T d1 = rt_fma(c[3], s, b1);        // 2 c3 s + c2
+  f1 = rt_fma(d1, s, b0);                  // 3 c3 s^2 + 2 c2 s + c1
+  f2h = rt_fma(c[3], s, d1);               // 3 c3 s + c2
+}
+template <class T>
+RT_DEV void cubic01(const T* c, T s, T& f, T& f1) {
+  const T b1 = rt_fma(c[3], s, c[2]);
+  const T b0 = rt_fma(b1, s, c[1]);
+  f = rt_fma(b0, s, c[0]);
+  f1 = rt_fma(rt_fma(c[3], s, b1), s, b0);
+}
+
 // ---- Stix elements (Eq. 8-10) as functions of X, Y2 ------------------------------------------
 //   S = 1 - X sig,  sig = 1/(1-Y2) + mu/(1-mu^2 Y2)
 //   Dx^2 = X^2 Y2 del^2,  del = mu^2/(1-mu^2 Y2) - 1/(1-Y2)      (eps12 = -i Dx; only Dx^2 enters D)
@@ -154,7 +194,8 @@ RT_DEV T disp_value(const Params<T>& P, T X, T Y2, T u, T v) {
   return (st.p - w) * RL + st.s * (w * v - st.p * (v + u)) + st.p * u * v;
 }
 
-// Partials of D with respect to (X, Y2, u, v); also returns D's scale-free pieces for W.
+// Partials of D with respect to (X, Y2, u, v) in their plain form (launch solver and diagnostics; the hot loop uses
+// disp_coefs below).
 template <class T, int DISP>
 RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2, T& Du, T& Dv) {
   if (DISP == DISP_O) { DX = T(1); DY2 = T(0); Du = T(0); Dv = T(1); return; }
@@ -178,100 +219,186 @@ RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2
   DY2 = -X * st.sigp * Ds + X * X * st.del * (st.del + T(2) * Y2 * st.delp) * Dd2;
 }
 
+// ---- the four scalars of the ray RHS (header comment) for the magnetised dispersion functions --------------------
+// Reverse-mode differentiation of  D = pw ab - t b,  w = v - u, pw = P - w, a = S - u, b = S - v, ab = a b - Dx^2,
+// t = w u  (the full determinant above), or of D = S v - S^2 + Dx^2 (X-mode):
+//   D_S = pw b + (pw a - t),  D_P = ab,  D_{Dx^2} = -pw,  D_w = -(ab + b u),  D_v = D_w - (pw a - t),
+//   D_u = -b w - pw b - D_w.
+// With S_X = -sig, P_X = -(1+mu), (Dx^2)_X = q1 = 2 X Y2 del^2, S_Y2 = -X sig', (Dx^2)_Y2 = q2 = X^2 del (del + 2 Y2 del'):
+//   -D_X = DXn = sig D_S + (1+mu) D_P + q1 pw ,     -D_Y2 = DYn = X sig' D_S + q2 pw.
+template <class T>
+struct Coef { T A, C, Ax, Ab; };
+
+template <class T, int DISP>
+RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
+  const T Y2 = P.beta * b2, Y22 = P.beta2 * b2;
+  const T e1 = rt_rcp(T(1) - Y2);
+  const T e2 = rt_rcp(rt_fma(-P.mu2, Y2, T(1)));
+  const T e1s = e1 * e1, e2s = e2 * e2;
+  const T sig = rt_fma(P.mu, e2, e1);
+  const T sigp = rt_fma(P.mu3, e2s, e1s);
+  const T del = rt_fma(P.mu2, e2, -e1);
+  const T delp = rt_fma(P.mu4, e2s, -e1s);
+  const T S = rt_fma(-X, sig, T(1));
+  const T Xd = X * del;
+  const T XdY22 = Xd * Y22;                          // 2 X Y2 del
+  const T q1 = XdY22 * del;
+  const T q2 = (Xd * X) * rt_fma(Y22, delp, del);
+  const T Xsp = X * sigp;
+  Coef<T> c;
+  if (DISP == DISP_X) {
+    const T DS = rt_fma(T(-2), S, v);
+    const T DXn = rt_fma(sig, DS, -q1);
+    const T DYn = rt_fma(Xsp, DS, -q2);
+    const T s = rt_fma(v, S, -rt_fma(Y2, DYn, X * DXn));
+    const T r = rt_rcp(s);
+    c.A = S * r;
+    c.C = T(0);
+    c.Ax = DXn * (T(0.5) * r);
+    c.Ab = (P.beta * r) * DYn;
+  } else {
+    const T d2 = (T(0.5) * Xd) * XdY22;
+    const T Pp = rt_fma(-X, P.one_plus_mu, T(1));
+    const T Bc = G * rt_rcp(b2);
+    const T u = G * Bc;
+    const T w = v - u, pw = Pp - w, a = S - u, b = S - v;
+    const T ab = rt_fma(a, b, -d2);
+    const T pb = pw * b;
+    const T pat = rt_fma(pw, a, -(w * u));
+    const T DS = pb + pat;
+    const T Dw = -rt_fma(b, u, ab);
+    const T Du = rt_fma(-b, w, -pb) - Dw;
+    const T Dv = Dw - pat;
+    const T DXn = rt_fma(q1, pw, rt_fma(P.one_plus_mu, ab, sig * DS));
+    const T DYn = rt_fma(q2, pw, Xsp * DS);
+    const T s = rt_fma(v, Dv, rt_fma(u, Du, -rt_fma(Y2, DYn, X * DXn)));
+    const T r = rt_rcp(s);
+    c.A = Dv * r;
+    c.C = Bc * (Du * r);
+    c.Ax = DXn * (T(0.5) * r);
+    c.Ab = rt_fma(Bc, c.C, (P.beta * r) * DYn);
+  }
+  return c;
+}
+
 // ---- equilibrium at one stage point, in a local orthonormal frame ------------------------------------------------
-// Frame: (e1, e2, e3) = (R^, phi^, Z^) for the axisymmetric kinds, Cartesian for the slabs (cph = 1, sph = 0).
-// Gradients are the frame components of the Cartesian gradient; gG = grad_x (n.B) at fixed Cartesian n.
+// Frame: (e1, e2, e3) = (R^, phi^, Z^) for the axisymmetric kinds, Cartesian for the slabs.  Only the entries an
+// equilibrium can make non-zero are written (and read): slabs vary along e1 = x only; axisymmetric X and |B|^2 have no
+// e2 = phi derivative.  gG = grad_x (n.B) at fixed Cartesian n, hgb2 = (1/2) grad |B|^2.
 template <class T>
 struct Local {
   T X, gX[3];
-  T B[3], b2, gb2[3], gG[3], G;
+  T B[3], b2, hgb2[3], G, gG[3];
   T nl[3];       // n in the local frame
-  T cph, sph;    // e1 = (cph, sph, 0), e2 = (-sph, cph, 0)
+  T cph, sph;    // axisymmetric kinds: e1 = (cph, sph, 0), e2 = (-sph, cph, 0)
 };
 
-// shared tail of the two axisymmetric kinds: psi derivatives, F, its (R,Z) derivatives -> B and its gradients
+template <int EQ> struct is_axisym { static constexpr bool value = (EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW || EQ == EQ_GRID); };
+
+// Tail of the grid equilibrium: B = (-psi_Z, F, psi_R)/R and its derivatives from psi's and F's.  With
+// Q = psi_R^2 + psi_Z^2 + F^2 = R^2 |B|^2 and g = -n_R psi_Z + n_phi F + n_Z psi_R = R (n.B):
+//   (1/2) grad|B|^2 = (Q_R/2, Q_Z/2)/R^2 - (|B|^2/R) R^ ,   grad_x(n.B) = ((g_R - n.B)/R, (n_phi B_R - n_R B_phi)/R, g_Z/R).
+// psiRRh / psiZZh are HALF the second derivatives.
 template <class T, int DISP>
-RT_DEV void axisym_field(T iR, T psiR, T psiZ, T psiRR, T psiRZ, T psiZZ, T F, T FR, T FZ, Local<T>& L) {
+RT_DEV void axisym_field(T iR, T psiR, T psiZ, T psiRRh, T psiRZ, T psiZZh, T F, T Fp, Local<T>& L) {
   if (DISP == DISP_O) return;
-  const T BR = -psiZ * iR, BZ = psiR * iR, Bp = F * iR;
-  const T BR_R = -iR * (psiRZ + BR), BR_Z = -psiZZ * iR;
-  const T BZ_R = iR * (psiRR - BZ), BZ_Z = psiRZ * iR;
-  const T Bp_R = iR * (FR - Bp), Bp_Z = FZ * iR;
-  L.B[0] = BR; L.B[1] = Bp; L.B[2] = BZ;
-  L.b2 = BR * BR + BZ * BZ + Bp * Bp;
-  L.gb2[0] = T(2) * (BR * BR_R + BZ * BZ_R + Bp * Bp_R);
-  L.gb2[1] = T(0);
-  L.gb2[2] = T(2) * (BR * BR_Z + BZ * BZ_Z + Bp * Bp_Z);
-  const T nR = L.nl[0], nP = L.nl[1], nZ = L.nl[2];
-  L.G = nR * BR + nP * Bp + nZ * BZ;
-  L.gG[0] = nR * BR_R + nP * Bp_R + nZ * BZ_R;
-  L.gG[1] = (nP * BR - nR * Bp) * iR;      // (1/R) d/dphi of n.B at fixed Cartesian n
-  L.gG[2] = nR * BR_Z + nP * Bp_Z + nZ * BZ_Z;
+  const T iR2 = iR * iR;
+  const T Q = rt_fma(F, F, rt_fma(psiR, psiR, psiZ * psiZ));
+  L.b2 = Q * iR2;
+  const T psiRR = psiRRh + psiRRh, psiZZ = psiZZh + psiZZh;
+  const T FFp = F * Fp;
+  const T hQR = rt_fma(FFp, psiR, rt_fma(psiR, psiRR, psiZ * psiRZ));
+  const T hQZ = rt_fma(FFp, psiZ, rt_fma(psiR, psiRZ, psiZ * psiZZ));
+  L.hgb2[0] = rt_fma(hQR, iR2, -L.b2 * iR);
+  L.hgb2[2] = hQZ * iR2;
+  if (DISP == DISP_FULL) {
+    const T nR = L.nl[0], nP = L.nl[1], nZ = L.nl[2];
+    L.B[0] = -psiZ * iR; L.B[1] = F * iR; L.B[2] = psiR * iR;
+    const T g = rt_fma(nZ, psiR, rt_fma(nP, F, -nR * psiZ));
+    L.G = g * iR;
+    const T nPFp = nP * Fp;
+    const T gR = rt_fma(nZ, psiRR, rt_fma(nPFp, psiR, -nR * psiRZ));
+    const T gZ = rt_fma(nZ, psiRZ, rt_fma(nPFp, psiZ, -nR * psiZZ));
+    L.gG[0] = (gR - L.G) * iR;
+    L.gG[1] = -rt_fma(nP, psiZ, nR * F) * iR2;
+    L.gG[2] = gZ * iR;
+  }
 }
 
-template <class T, int EQ, int DISP>
-RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L) {
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L, Gather& gather) {
   if (EQ == EQ_PARABOLIC) {
     // X = xs (1 + (x^2+y^2)/L^2)                                          (BASELINE.json config 1)
-    const T g = P.xs * P.inv_L2;
-    L.X = P.xs + g * (x[0] * x[0] + x[1] * x[1]);
-    L.gX[0] = T(2) * g * x[0]; L.gX[1] = T(2) * g * x[1]; L.gX[2] = T(0);
-    L.nl[0] = n[0]; L.nl[1] = n[1]; L.nl[2] = n[2];
-    L.cph = T(1); L.sph = T(0);
-    return true;
+    L.X = rt_fma(P.par_g, rt_fma(x[0], x[0], x[1] * x[1]), P.xs);
+    return true;                                                           // grad X = 2 par_g (x, y, 0): see ray_rhs
   }
   if (EQ == EQ_LINEAR) {
     // n_e = n_ref (x_foot - x)/L_ramp ;  B = (B0 R0 / x) z^                (config 3; Eq. 4 profile)
     const bool inside = x[0] > T(0);
-    const T gx = -P.xs * P.inv_Lramp;
-    L.X = (x[0] - P.x_foot) * gx;
-    L.gX[0] = gx; L.gX[1] = T(0); L.gX[2] = T(0);
-    L.nl[0] = n[0]; L.nl[1] = n[1]; L.nl[2] = n[2];
-    L.cph = T(1); L.sph = T(0);
+    L.X = (x[0] - P.x_foot) * P.lin_gx;                                    // grad X = (lin_gx, 0, 0)
     if (DISP != DISP_O) {
       const T ix = rt_rcp(x[0]);
       const T Bz = P.B0R0 * ix;
-      L.B[0] = T(0); L.B[1] = T(0); L.B[2] = Bz;
+      L.B[2] = Bz;
       L.b2 = Bz * Bz;
-      L.gb2[0] = T(-2) * L.b2 * ix; L.gb2[1] = T(0); L.gb2[2] = T(0);
-      L.G = n[2] * Bz;
-      L.gG[0] = -L.G * ix; L.gG[1] = T(0); L.gG[2] = T(0);
+      L.hgb2[0] = -L.b2 * ix;
+      if (DISP == DISP_FULL) {
+        L.G = n[2] * Bz;
+        L.gG[0] = -L.G * ix;
+      }
     }
     return inside;
   }
   // axisymmetric kinds: cylindrical frame at the point
-  const T R2 = x[0] * x[0] + x[1] * x[1];
+  const T R2 = rt_fma(x[0], x[0], x[1] * x[1]);
   const T iR = rt_rsqrt(R2);
   const T R = R2 * iR;
   const T Z = x[2];
   L.cph = x[0] * iR; L.sph = x[1] * iR;
-  L.nl[0] = n[0] * L.cph + n[1] * L.sph;
-  L.nl[1] = n[1] * L.cph - n[0] * L.sph;
-  L.nl[2] = n[2];
-  L.gX[1] = T(0);
+  if (DISP == DISP_FULL) {
+    L.nl[0] = rt_fma(n[0], L.cph, n[1] * L.sph);
+    L.nl[1] = rt_fma(n[1], L.cph, -n[0] * L.sph);
+    L.nl[2] = n[2];
+  }
   if (EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) {
     // psi'(r) = B0 r / q, q = q0 + q1 rho^2, F = B0 R0, n_e = n_ref (1 - rho^2)^p       (config 4; reading A9)
     const T dR = R - P.R0;
-    const T rho2 = (dR * dR + Z * Z) * P.inv_a2;
-    const bool inside = (R > T(0)) && (rho2 < P.rho_max2);
-    const T t = T(1) - rho2;
-    T shape, dshape;     // t^p and d(t^p)/d(rho^2)
+    const T r2 = rt_fma(dR, dR, Z * Z);
+    const bool inside = (R > T(0)) && (r2 < P.rmax2);
+    const T t = rt_fma(-P.inv_a2, r2, T(1));                               // 1 - rho^2
+    T gx;                                                                  // grad X = gx (dR, 0, Z)
     if (EQ == EQ_TOKAMAK) {
       const T sq = t * rt_rsqrt(t);
-      shape = t * sq; dshape = T(-1.5) * sq;
+      L.X = (P.xs * sq) * t;
+      gx = (T(-1.5) * P.two_xs_a2) * sq;
     } else {
       const T pw = rt_pow(t, P.p_exp - T(1));
-      shape = pw * t; dshape = -P.p_exp * pw;
+      L.X = (P.xs * pw) * t;
+      gx = (-P.p_exp * P.two_xs_a2) * pw;
     }
-    L.X = P.xs * shape;
-    const T gx = P.two_xs_a2 * dshape;
     L.gX[0] = gx * dR; L.gX[2] = gx * Z;
     if (DISP != DISP_O) {
-      const T iq = rt_rcp(P.q0 + P.q1 * rho2);
-      const T Bq = P.B0 * iq;
+      // B = (-h Z, g, h dR), h = B0/(q R), g = B0 R0/R; with e = 1/R + c dR, c = q'/q = 2 q1/(a^2 q):
+      //   h_R = -h e, h_Z = -h c Z, g_R = -g/R.
+      const T iq = rt_rcp(rt_fma(P.q1_a2, r2, P.q0));
+      const T h = (P.B0 * iq) * iR;
+      const T g = P.B0R0 * iR;
       const T c = P.two_q1_a2 * iq;
-      axisym_field<T, DISP>(iR, Bq * dR, Bq * Z, Bq * (T(1) - c * dR * dR), -Bq * c * dR * Z, Bq * (T(1) - c * Z * Z),
-                            P.B0R0, T(0), T(0), L);
+      const T e = rt_fma(c, dR, iR);
+      const T h2 = h * h, g2 = g * g;
+      const T giR = g * iR;
+      L.b2 = rt_fma(h2, r2, g2);                                           // |B|^2 = h^2 r^2 + g^2
+      L.hgb2[0] = rt_fma(h2, rt_fma(-r2, e, dR), -g * giR);                // h^2 (dR - r^2 e) - g^2/R
+      L.hgb2[2] = (h2 * Z) * rt_fma(-c, r2, T(1));                         // h^2 Z (1 - c r^2)
+      if (DISP == DISP_FULL) {
+        const T nR = L.nl[0], nP = L.nl[1], nZ = L.nl[2];
+        L.B[0] = -h * Z; L.B[1] = g; L.B[2] = h * dR;
+        const T m = rt_fma(nZ, dR, -nR * Z);
+        L.G = rt_fma(h, m, g * nP);
+        L.gG[0] = rt_fma(-nP, giR, h * rt_fma(-e, m, nZ));                 // h (n_Z - e m) - n_phi g/R
+        L.gG[1] = rt_fma(nP, L.B[0], -nR * g) * iR;                        // (n_phi B_R - n_R B_phi)/R
+        L.gG[2] = -h * rt_fma(c * Z, m, nR);                               // -h (n_R + c Z m)
+      }
     }
     return inside;
   }
@@ -281,85 +408,107 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L)
   iRc = iRc < 0 ? 0 : (iRc > P.nRc - 1 ? P.nRc - 1 : iRc);
   iZc = iZc < 0 ? 0 : (iZc > P.nZc - 1 ? P.nZc - 1 : iZc);
   if (!inside) { iRc = 0; iZc = 0; }      // NaN positions convert to unspecified ints: keep the gather in bounds
-  const T dR = R - (P.Rmin + T(iRc) * P.hR), dZ = Z - (P.Zmin + T(iZc) * P.hZ);
-  const T* cc = P.psi_pp + ((size_t)iRc * P.nZc + iZc) * 16;
-  T a[4], a1[4], a2[4];   // a_p(dZ) = sum_q c[p][q] dZ^q and its first / second dZ-derivatives
+  const T dR = R - rt_fma(T(iRc), P.hR, P.Rmin), dZ = Z - rt_fma(T(iZc), P.hZ, P.Zmin);
+  const int cell = iRc * P.nZc + iZc;
+  gather.psi_select(P, cell);
+  T a[4], a1[4], a2h[4];   // a_p(dZ) = sum_q c[p][q] dZ^q, its first dZ-derivative and half its second
 #pragma unroll
   for (int p = 0; p < 4; ++p) {
     T c[4];
-    ld4(cc + 4 * p, c);
-    a[p] = ((c[3] * dZ + c[2]) * dZ + c[1]) * dZ + c[0];
-    a1[p] = (T(3) * c[3] * dZ + T(2) * c[2]) * dZ + c[1];
-    a2[p] = T(6) * c[3] * dZ + T(2) * c[2];
+    gather.psi_row(P, cell, p, c);
+    if (DISP == DISP_O) cubic01(c, dZ, a[p], a1[p]);
+    else cubic012(c, dZ, a[p], a1[p], a2h[p]);
   }
-  const T psi = ((a[3] * dR + a[2]) * dR + a[1]) * dR + a[0];
-  const T psiR = (T(3) * a[3] * dR + T(2) * a[2]) * dR + a[1];
-  const T psiZ = ((a1[3] * dR + a1[2]) * dR + a1[1]) * dR + a1[0];
+  T psi, psiR, psiRRh = T(0), psiZ, psiRZ = T(0), psiZZh = T(0);
+  if (DISP == DISP_O) {
+    cubic01(a, dR, psi, psiR);
+    psiZ = rt_fma(rt_fma(rt_fma(a1[3], dR, a1[2]), dR, a1[1]), dR, a1[0]);
+  } else {
+    cubic012(a, dR, psi, psiR, psiRRh);
+    cubic01(a1, dR, psiZ, psiRZ);
+    psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
+  }
   inside = inside && (psi >= P.psi_min) && (psi <= P.psi_max);
   int iP = (int)rt_floor((psi - P.psi_min) * P.inv_hP);
   iP = iP < 0 ? 0 : (iP > P.nPc - 1 ? P.nPc - 1 : iP);
   if (!inside) iP = 0;
-  const T ds = psi - (P.psi_min + T(iP) * P.hP);
-  T f[4], g[4];
-  ld4(P.prof_pp + (size_t)iP * 8, f);
-  ld4(P.prof_pp + (size_t)iP * 8 + 4, g);
-  const T Ne = ((g[3] * ds + g[2]) * ds + g[1]) * ds + g[0];
-  const T Nep = (T(3) * g[3] * ds + T(2) * g[2]) * ds + g[1];
+  const T ds = psi - rt_fma(T(iP), P.hP, P.psi_min);
+  T g[4], Ne, Nep;
+  gather.prof_select(P, iP);
+  gather.prof_row(P, iP, 1, g);
+  cubic01(g, ds, Ne, Nep);
   L.X = P.xs * Ne;
   const T gx = P.xs * Nep;
   L.gX[0] = gx * psiR; L.gX[2] = gx * psiZ;
   if (DISP != DISP_O) {
-    const T F = ((f[3] * ds + f[2]) * ds + f[1]) * ds + f[0];
-    const T Fp = (T(3) * f[3] * ds + T(2) * f[2]) * ds + f[1];
-    const T psiRR = T(6) * a[3] * dR + T(2) * a[2];
-    const T psiRZ = (T(3) * a1[3] * dR + T(2) * a1[2]) * dR + a1[1];
-    const T psiZZ = ((a2[3] * dR + a2[2]) * dR + a2[1]) * dR + a2[0];
-    axisym_field<T, DISP>(iR, psiR, psiZ, psiRR, psiRZ, psiZZ, F, Fp * psiR, Fp * psiZ, L);
+    T f[4], F, Fp;
+    gather.prof_row(P, iP, 0, f);
+    cubic01(f, ds, F, Fp);
+    axisym_field<T, DISP>(iR, psiR, psiZ, psiRRh, psiRZ, psiZZh, F, Fp, L);
   }
   return inside;
 }
 
 // ---- one evaluation of the ray right-hand side f(y), y = (x, n) --------------------------------------------------
 // Returns false (and f unspecified) if x is outside the equilibrium's domain.
-template <class T, int EQ, int DISP>
-RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f) {
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, Gather& gather) {
   Local<T> L;
-  const bool inside = equilibrium<T, EQ, DISP>(P, y, y + 3, L);
-  const T* nl = L.nl;
-  const T v = nl[0] * nl[0] + nl[1] * nl[1] + nl[2] * nl[2];
-  T fx[3], fn[3];        // local-frame components
+  const T* n = y + 3;
+  const bool inside = equilibrium<T, EQ, DISP>(P, y, n, L, gather);
+  const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
   if (DISP == DISP_O) {
-    // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)
-    const T iW = rt_rcp(v + L.X);
-#pragma unroll
-    for (int j = 0; j < 3; ++j) { fx[j] = nl[j] * iW; fn[j] = T(-0.5) * L.gX[j] * iW; }
-  } else {
-    const T ib2 = rt_rcp(L.b2);
-    const T Y2 = P.beta * L.b2;
-    const T u = (DISP == DISP_FULL) ? L.G * L.G * ib2 : T(0);
-    T DX, DY2, Du, Dv;
-    disp_partials<T, DISP>(P, L.X, Y2, u, v, DX, DY2, Du, Dv);
-    const T W = T(-2) * (L.X * DX + Y2 * DY2 + u * Du + v * Dv);
-    const T iW = rt_rcp(W);
-    const T DG = T(2) * L.G * ib2 * Du;            // dD/dG at fixed |B|^2
-    const T Db2 = P.beta * DY2 - u * ib2 * Du;     // dD/d|B|^2 at fixed G: through Y2 and through u = G^2/|B|^2
-#pragma unroll
-    for (int j = 0; j < 3; ++j) {
-      T dn = T(2) * Dv * nl[j], dx = DX * L.gX[j] + Db2 * L.gb2[j];
-      if (DISP == DISP_FULL) { dn += DG * L.B[j]; dx += DG * L.gG[j]; }
-      fx[j] = -dn * iW; fn[j] = dx * iW;
+    // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)   =>   dx/dtau = n r, dn/dtau = -grad X r/2, r = 1/(v+X)
+    const T r = rt_rcp(v + L.X);
+    f[0] = n[0] * r; f[1] = n[1] * r; f[2] = n[2] * r;
+    if (EQ == EQ_PARABOLIC) {
+      const T c = -P.par_g * r;
+      f[3] = c * y[0]; f[4] = c * y[1]; f[5] = T(0);
+    } else if (EQ == EQ_LINEAR) {
+      f[3] = (T(-0.5) * P.lin_gx) * r; f[4] = T(0); f[5] = T(0);
+    } else {
+      const T hr = T(-0.5) * r;
+      const T fR = hr * L.gX[0];
+      f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = hr * L.gX[2];
     }
+    return inside;
   }
-  f[0] = fx[0] * L.cph - fx[1] * L.sph; f[1] = fx[0] * L.sph + fx[1] * L.cph; f[2] = fx[2];
-  f[3] = fn[0] * L.cph - fn[1] * L.sph; f[4] = fn[0] * L.sph + fn[1] * L.cph; f[5] = fn[2];
+  const Coef<T> c = disp_coefs<T, DISP>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
+  f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
+  if (EQ == EQ_LINEAR) {
+    T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gx);
+    if (DISP == DISP_FULL) {
+      f[2] = rt_fma(c.C, L.B[2], f[2]);
+      fn = rt_fma(-c.C, L.gG[0], fn);
+    }
+    f[3] = fn; f[4] = T(0); f[5] = T(0);
+    return inside;
+  }
+  // axisymmetric kinds: assemble in (R^, phi^, Z^), rotate to Cartesian
+  T fR = rt_fma(c.Ab, L.hgb2[0], c.Ax * L.gX[0]);
+  T fZ = rt_fma(c.Ab, L.hgb2[2], c.Ax * L.gX[2]);
+  if (DISP == DISP_FULL) {
+    const T xR = c.C * L.B[0], xP = c.C * L.B[1];
+    f[0] = rt_fma(xR, L.cph, rt_fma(-xP, L.sph, f[0]));
+    f[1] = rt_fma(xR, L.sph, rt_fma(xP, L.cph, f[1]));
+    f[2] = rt_fma(c.C, L.B[2], f[2]);
+    fR = rt_fma(-c.C, L.gG[0], fR);
+    fZ = rt_fma(-c.C, L.gG[2], fZ);
+    const T fP = -c.C * L.gG[1];
+    f[3] = rt_fma(fR, L.cph, -fP * L.sph);
+    f[4] = rt_fma(fR, L.sph, fP * L.cph);
+  } else {
+    f[3] = fR * L.cph; f[4] = fR * L.sph;
+  }
+  f[5] = fZ;
   return inside;
 }
 
 // signed D at y = (x, n); *inside reports the domain test
-template <class T, int EQ, int DISP>
-RT_DEV T ray_D(const Params<T>& P, const T* y, bool* inside) {
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV T ray_D(const Params<T>& P, const T* y, bool* inside, Gather& gather) {
   Local<T> L;
-  *inside = equilibrium<T, EQ, DISP>(P, y, y + 3, L);
+  *inside = equilibrium<T, EQ, DISP>(P, y, y + 3, L, gather);
   const T v = y[3] * y[3] + y[4] * y[4] + y[5] * y[5];
   if (DISP == DISP_O) return disp_value<T, DISP>(P, L.X, T(0), T(0), v);
   const T u = (DISP == DISP_FULL) ? L.G * L.G * rt_rcp(L.b2) : T(0);

@@ -1,0 +1,65 @@
+// rt_params.h -- step a0 of the hot path: fold the wave frequency w into O(1) constants, once per call, in fp64 on the
+// host (Eq. 6: n = c k / w; L189: w_p, W_c per species), so that every device-side quantity stays O(1)
+// in fp32 as well.  Host code only; no CUDA dependency.
+#pragma once
+
+#include <cstring>
+
+#include "../../include/rt.h"
+#include "rt_math.cuh"
+
+namespace rt {
+
+// CODATA-2022 numerals (reading A6)
+constexpr double kC = 299792458.0;          // m/s
+constexpr double kQe = 1.602176634e-19;     // C
+constexpr double kMe = 9.1093837139e-31;    // kg
+constexpr double kEps0 = 8.8541878188e-12;  // F/m
+
+// d: the equilibrium's scalars; rho_max: resolved domain radius (tokamak); ne_scale: what the grid's n_e table was
+// divided by; psi_pp / prof_pp: device tables of element type T (grid kind), else NULL.
+template <class T>
+Params<T> fold_params(const rt_equilibrium_desc& d, double rho_max, double ne_scale, double omega, const T* psi_pp,
+                      const T* prof_pp) {
+  Params<T> P;
+  std::memset(&P, 0, sizeof(P));
+  const double alpha = kQe * kQe / (kEps0 * kMe * omega * omega);       // X_e = alpha n_e
+  const double nscale = (d.kind == RT_EQ_GRID_RZ) ? ne_scale : d.n_ref;
+  const double xs = alpha * nscale;
+  P.xs = (T)xs;
+  const double wce_per_T = kQe / (kMe * omega);
+  P.beta = (T)(wce_per_T * wce_per_T);
+  P.beta2 = (T)(2.0 * wce_per_T * wce_per_T);
+  const double mu = (d.ion_mass > 0.0) ? d.ion_charge * kMe / d.ion_mass : 0.0;
+  P.mu = (T)mu; P.mu2 = (T)(mu * mu); P.mu3 = (T)(mu * mu * mu); P.mu4 = (T)(mu * mu * mu * mu);
+  P.one_plus_mu = (T)(1.0 + mu);
+  P.k2n = (T)(kC / omega);
+  P.n2k = (T)(omega / kC);
+  P.par_g = (T)(d.L != 0.0 ? xs / (d.L * d.L) : 0.0);
+  P.x_foot = (T)d.x_foot;
+  P.lin_gx = (T)(d.L_ramp != 0.0 ? -xs / d.L_ramp : 0.0);
+  P.B0R0 = (T)(d.B0 * d.R0);
+  P.R0 = (T)d.R0;
+  P.B0 = (T)d.B0;
+  const double inv_a2 = d.a != 0.0 ? 1.0 / (d.a * d.a) : 0.0;
+  P.inv_a2 = (T)inv_a2;
+  P.q0 = (T)d.q0;
+  P.q1_a2 = (T)(d.q1 * inv_a2);
+  P.two_q1_a2 = (T)(2.0 * d.q1 * inv_a2);
+  P.p_exp = (T)d.p_exp;
+  P.two_xs_a2 = (T)(2.0 * xs * inv_a2);
+  P.rmax2 = (T)(rho_max * rho_max * d.a * d.a);
+  if (d.kind == RT_EQ_GRID_RZ) {
+    const double hR = (d.Rmax - d.Rmin) / (d.nR - 1), hZ = (d.Zmax - d.Zmin) / (d.nZ - 1);
+    const double hP = (d.psi_max - d.psi_min) / (d.nPsi - 1);
+    P.Rmin = (T)d.Rmin; P.Rmax = (T)d.Rmax; P.Zmin = (T)d.Zmin; P.Zmax = (T)d.Zmax;
+    P.hR = (T)hR; P.hZ = (T)hZ; P.inv_hR = (T)(1.0 / hR); P.inv_hZ = (T)(1.0 / hZ);
+    P.psi_min = (T)d.psi_min; P.psi_max = (T)d.psi_max; P.hP = (T)hP; P.inv_hP = (T)(1.0 / hP);
+    P.nRc = d.nR - 1; P.nZc = d.nZ - 1; P.nPc = d.nPsi - 1;
+    P.psi_pp = psi_pp;
+    P.prof_pp = prof_pp;
+  }
+  return P;
+}
+
+}  // namespace rt
