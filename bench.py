@@ -40,9 +40,17 @@ from paper_2508_15967_b200 import inputs  # noqa: E402
 METRIC = "ray_steps_per_s"
 UNIT = "ray-steps/s"
 
-# Algorithmic flops per ray-step: adds + multiplies + divisions + square roots of the
-# hand-derived formulation, one RK4 step = 4 right-hand sides + the tableau; a fused multiply-add counts 2.
-FLOPS_PER_RAY_STEP = {1: 263, 2: 263, 3: 571, 4: 1067, 5: 1507}
+# Algorithmic flops per ray-step: adds + multiplies + divisions + square roots of the hand-derived
+# formulation, one RK4 step = 4 right-hand sides + the tableau; a fused multiply-add counts 2, a division or square root 1
+# (its Newton refinement is NOT counted).  FP_INSTR_PER_RAY_STEP is what the FP64 / FP32 pipe actually issues per
+# ray-step (FMA, MUL, ADD, SETP instructions, refinements included).  Both tables are counted from the compiled kernels by
+# paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
+FLOPS_PER_RAY_STEP = {(1, "f64"): 132, (2, "f64"): 132, (3, "f64"): 276, (4, "f64"): 824, (5, "f64"): 1272,
+                      (1, "f32"): 132, (2, "f32"): 132, (3, "f32"): 276, (4, "f32"): 816, (5, "f32"): 1268}
+FP_INSTR_PER_RAY_STEP = {(1, "f64"): 92, (2, "f64"): 92, (3, "f64"): 234, (4, "f64"): 666, (5, "f64"): 900,
+                         (1, "f32"): 86, (2, "f32"): 86, (3, "f32"): 192, (4, "f32"): 564, (5, "f32"): 834}
+# (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
+KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None
 NCU_DRAM_BYTES = {}
 
@@ -314,13 +322,15 @@ def run_ours(args) -> int:
                "d2h_bytes_per_step": d2h, "steps": k_e2e, "api": "rt_trace_host (pinned host buffers, 2-stream chunk pipeline)"}
         del x0h, k0h, hout
 
-    flops = FLOPS_PER_RAY_STEP[cfg] * job.ray_steps
+    flops = FLOPS_PER_RAY_STEP[(cfg, prec)] * job.ray_steps
     launch_residual = job.launch_residual
     peak = 2.0 * peak_after
     achieved = flops / (kernel_ms * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": NCU_DRAM_BYTES.get((cfg, prec)), "kernel": f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
-                "kernel_ms": kernel_ms, "flops_per_ray_step": FLOPS_PER_RAY_STEP[cfg],
+                "kernel_ms": kernel_ms, "flops_per_ray_step": FLOPS_PER_RAY_STEP[(cfg, prec)],
+                "fp_instr_per_ray_step": FP_INSTR_PER_RAY_STEP[(cfg, prec)],
+                "pipe_frac": FP_INSTR_PER_RAY_STEP[(cfg, prec)] * job.ray_steps / (kernel_ms * 1e-3) / peak_after,
                 "peak_source": f"rt_fma_peak({prec}) measured in this process after the timed region: "
                                f"{peak_after / 1e12:.3f} T{'D' if prec == 'f64' else 'F'}FMA/s at {peak_mhz:.0f} MHz "
                                f"(before: {peak_before / 1e12:.3f})"}
@@ -337,7 +347,8 @@ def run_ours(args) -> int:
             _, kms = time_steps(torch, j, 3, 1, flush)
             pk, _ = rt.fma_peak(p, 100.0)
             extra.append({"workload": f"cfg{c}", "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
-                          "roofline_frac": FLOPS_PER_RAY_STEP[c] * j.ray_steps / (kms * 1e-3) / (2.0 * pk)})
+                          "roofline_frac": FLOPS_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / (2.0 * pk),
+                          "pipe_frac": FP_INSTR_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / pk})
             j.close()
             del j
             torch.cuda.empty_cache()

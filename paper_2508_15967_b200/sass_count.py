@@ -1,0 +1,109 @@
+"""Count the floating-point work of one ray-step in the compiled ``trace_kernel`` instantiations (``cuobjdump -sass``).
+
+    python -m paper_2508_15967_b200.sass_count            # table for every trace kernel in librt_b200.so
+
+A ray-step is one pass through the RK4 step region of the kernel (the ``if (status == 0) status = rk4_step(...)`` body:
+the largest reconvergence region of the SASS); for the grid equilibrium the stage loop inside it is rolled and runs 4 times.
+Reported per kernel:
+
+* ``instr``     FP-pipe instructions per ray-step (DFMA + DMUL + DADD + DSETP, or the FP32 analogues) -- what the FP64
+                (FP32) pipe has to issue, the quantity the kernels are optimised for;
+* ``executed``  flops as executed, a fused multiply-add counted as 2;
+* ``mufu``      MUFU seeds (reciprocals and reciprocal square roots), ``rsqrt`` of them square roots;
+* ``flops``     the ALGORITHMIC flops bench.py uses for ``roofline.achieved``: every division and square root counted as
+                ONE flop.  In fp64 a reciprocal executes 3 FMAs (6 flops) and a reciprocal square root 2 MUL + 3 FMA
+                (8 flops) of Newton refinement after the seed, so flops = executed - 5 rcp - 7 rsqrt; in fp32 the seed
+                is used as is, so flops = executed + mufu.  The two precisions agree on this figure to within 1 %.
+
+This is a measuring tool; nothing in the product path imports it.  ``tests/test_abi.py`` checks
+bench.py's ``FLOPS_PER_RAY_STEP`` table against it, so the table cannot go stale when the kernels change.
+"""
+from __future__ import annotations
+
+import re
+import shutil
+import subprocess
+from collections import Counter
+from pathlib import Path
+
+LIB = Path(__file__).resolve().parent / "librt_b200.so"
+_INS = re.compile(r"\s+/\*([0-9a-f]+)\*/\s+(?:@!?U?P\w+\s+)?([A-Z0-9_.]+)(.*?);")
+_FP = {"d": ("DFMA", "DMUL", "DADD", "DSETP"), "f": ("FFMA", "FMUL", "FADD", "FSETP")}
+
+
+def cuobjdump() -> str | None:
+    for cand in (shutil.which("cuobjdump"), "/usr/local/cuda/bin/cuobjdump"):
+        if cand and Path(cand).exists():
+            return cand
+    return None
+
+
+def _parse(body: str):
+    out = []
+    for line in body.splitlines():
+        m = _INS.match(line)
+        if m:
+            out.append((int(m.group(1), 16), m.group(2), m.group(3)))
+    return out
+
+
+def _target(rest: str):
+    m = re.search(r"0x([0-9a-f]+)", rest)
+    return int(m.group(1), 16) if m else None
+
+
+def _count(ins, lo, hi):
+    return Counter(op.split(".")[0] for a, op, _ in ins if lo <= a < hi), \
+        sum(1 for a, op, _ in ins if lo <= a < hi and op.startswith("MUFU.RSQ"))
+
+
+def count_kernels(lib: Path = LIB) -> dict:
+    """{(precision 'f64'|'f32', eq_kind, disp_kind): {'instr', 'executed', 'mufu', 'rsqrt', 'flops'}} per ray-step."""
+    exe = cuobjdump()
+    if exe is None:
+        raise RuntimeError("cuobjdump not found")
+    sass = subprocess.run([exe, "-sass", str(lib)], capture_output=True, text=True, check=True).stdout
+    res = {}
+    for fn in re.split(r"\n\s*Function : ", sass):
+        m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)E", fn)
+        if not m:
+            continue
+        prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
+        ins = _parse(fn)
+        region = None                                       # the RK4 step: largest BSSY ... BSYNC region
+        for a, op, rest in ins:
+            if op.startswith("BSSY"):
+                t = _target(rest)
+                if t is not None and (region is None or t - a > region[1] - region[0]):
+                    region = (a, t)
+        if region is None:
+            continue
+        c, rsq = _count(ins, *region)
+        tot = Counter(c)
+        inner = None                                        # rolled stage loop (grid): largest backward branch inside
+        for a, op, rest in ins:
+            if op.startswith("BRA") and region[0] <= a < region[1]:
+                t = _target(rest)
+                if t is not None and region[0] <= t < a and (inner is None or a - t > inner[1] - inner[0]):
+                    inner = (t, a)
+        if inner is not None and inner[1] - inner[0] > (region[1] - region[0]) // 2:
+            ci, rsqi = _count(ins, *inner)
+            for k, v in ci.items():
+                tot[k] += 3 * v
+            rsq += 3 * rsqi
+        fma, mul, add, setp = _FP[prec]
+        executed = 2 * tot[fma] + tot[mul] + tot[add]
+        mufu = tot["MUFU"]
+        flops = executed - 5 * (mufu - rsq) - 7 * rsq if prec == "d" else executed + mufu
+        res[("f64" if prec == "d" else "f32", eq, disp)] = dict(instr=tot[fma] + tot[mul] + tot[add] + tot[setp],
+                                                                executed=executed, mufu=mufu, rsqrt=rsq, flops=flops)
+    return res
+
+
+if __name__ == "__main__":
+    names = {0: "parabolic", 1: "linear", 2: "tokamak", 3: "grid", 4: "tokamak_pow"}
+    disps = {0: "O", 1: "X", 2: "full"}
+    print(f"{'kernel':34s} {'instr':>6s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s}")
+    for (prec, eq, disp), r in sorted(count_kernels().items()):
+        print(f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}> {r['instr']:6d} {r['executed']:9d} {r['mufu']:5d} "
+              f"{r['rsqrt']:6d} {r['flops']:6d}")

@@ -124,3 +124,27 @@ def test_product_never_imports_the_oracle():
         if path.suffix in (".py", ".cpp", ".h"):
             assert "paper_2508_15967_b200.binding" not in path.read_text() and "csrc" not in path.read_text().replace(
                 "paper_2508_15967_b200/csrc", ""), path
+
+
+def test_flop_tables_match_the_compiled_kernels(lib):
+    """bench.py's algorithmic-flop and FP-instruction tables are counted from the SASS of the trace kernels
+    (sass_count.py); a kernel change that alters the counts must update the tables."""
+    import bench
+    from paper_2508_15967_b200 import sass_count
+    if sass_count.cuobjdump() is None:
+        pytest.skip("cuobjdump not available")
+    counted = sass_count.count_kernels()
+    for (cfg, prec), flops in bench.FLOPS_PER_RAY_STEP.items():
+        eq, disp = bench.KERNEL_OF_CONFIG[cfg]
+        got = counted[(prec, eq, disp)]
+        assert got["flops"] == flops, (cfg, prec, got)
+        assert got["instr"] == bench.FP_INSTR_PER_RAY_STEP[(cfg, prec)], (cfg, prec, got)
+    # spills would show up as local-memory traffic: the build's ptxas report must be clean for every trace kernel
+    report_path = ROOT / "paper_2508_15967_b200" / "librt_b200.ptxas.txt"
+    if not report_path.exists():
+        rt_build.build(force=True)
+    report = report_path.read_text()
+    blocks = report.split("Compiling entry function")
+    traces = [b for b in blocks if "trace_kernel" in b.split("\n")[0]]
+    assert len(traces) == 26
+    assert all("0 bytes spill stores, 0 bytes spill loads" in b for b in traces)
