@@ -197,6 +197,59 @@ def test_cold_full_on_the_slab_inside_the_ramp(rt, oracle):
         eq.close()
 
 
+# --------------------------------------------------------------------------------- full sizes, sampled rays
+@pytest.mark.parametrize("cfg,prec", [(2, "f64"), (2, "f32"), (3, "f64"), (4, "f64"), (5, "f64"), (5, "f32")])
+def test_full_size_sampled_parity(rt, oracle, cfg, prec):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (one rt_trace call over the whole ensemble,
+    launch states from rt_launch, the config's output mode); 192 sampled rays are checked one by one against the oracle.
+    The sampled rays' launch wave vectors are the ORACLE's (oracle.launch on the same seeded positions / directions);
+    they are scattered into the device array so both sides start from identical bytes, after checking that rt_launch
+    agrees with them.  Every other ray must at least finish with status 0 and an on-shell residual."""
+    import torch
+    w = inputs.config(cfg)
+    n = w.n_rays
+    assert (n, w.n_steps) == inputs.FULL_SIZES[cfg]
+    rng = np.random.default_rng(4242 + cfg)
+    idx = np.unique(np.concatenate([np.arange(8), np.arange(n - 8, n), [127, 128, 129], rng.integers(0, n, 176)]))
+    oeq = oracle.Equilibrium(w.eq)
+    k0s, D0s = oracle.launch(oeq, w.disp, w.x0[:, idx], w.dirs[:, idx], w.omega, w.branch)
+    assert np.isfinite(k0s).all() and np.abs(D0s).max() < 2e-15
+    stride = w.save_stride if w.save_stride > 0 else 1
+    ref = oracle.trace(oeq, w.disp, w.x0[:, idx], k0s, w.omega, w.n_steps, w.dt, stride, traj=w.save_stride > 0)
+    assert (ref["status"] == 0).all()
+
+    eq = rt.create_equilibrium(w.eq)
+    x0d = _dev(w.x0)
+    k0d, _ = rt.launch(eq, w.disp, x0d, _dev(w.dirs), w.omega, w.branch)
+    idx_d = torch.from_numpy(idx).cuda()
+    got = _host(k0d[:, idx_d])
+    assert (np.linalg.norm(got - k0s, axis=0) / np.linalg.norm(k0s, axis=0)).max() < 1e-12
+    k0d[:, idx_d] = torch.from_numpy(k0s).cuda()
+    if prec == "f32":
+        x0d, k0d = x0d.float().contiguous(), k0d.float().contiguous()
+    out = rt.trace(eq, w.disp, x0d, k0d, w.omega, w.n_steps, w.dt, stride, traj=w.save_stride > 0)
+    torch.cuda.synchronize()
+    fin = _host(out["final"][:, idx_d])
+    ex, ek = rel_err_xk(fin, ref["final"])
+    assert ex < TOL[prec] and ek < TOL[prec], (cfg, prec, ex, ek)
+    assert int((out["status"] != 0).sum()) == 0
+    if w.save_stride > 0:
+        tr = _host(out["traj"][:, :, idx_d])
+        assert tr.shape == ref["traj"].shape
+        for m in range(0, tr.shape[0], 10):
+            ex, ek = rel_err_xk(tr[m], ref["traj"][m])
+            assert ex < TOL[prec] and ek < TOL[prec], (m, ex, ek)
+        _check_residual(oracle, oeq, w, tr, _host(out["residual"][:, idx_d]), ref["residual"], prec)
+    else:
+        _check_residual(oracle, oeq, w, fin, _host(out["residual"][idx_d]), ref["residual"], prec)
+    # the whole ensemble stays on-shell to integrator order (pin P3's magnitudes at the configs' dt in fp64; on the grid
+    # the piecewise-cubic equilibrium is only C^2, so crossing a cell boundary costs RK4 some order: ~1e-10 there)
+    red = _host(rt.reduce(out["residual"].reshape(-1)))
+    bound = {2: 1e-12, 3: 1e-11, 4: 1e-11, 5: 1e-9}[cfg] if prec == "f64" else 1e-3
+    assert red[2] == out["residual"].numel() and red[0] < bound, red
+    eq.close()
+
+
 # --------------------------------------------------------------------------------- status / freezing (reading A12)
 @pytest.mark.parametrize("cfg", [4, 5])
 def test_rays_leaving_the_domain_freeze_identically(rt, oracle, cfg):
