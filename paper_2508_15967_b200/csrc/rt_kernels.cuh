@@ -22,6 +22,9 @@ namespace rt {
 #ifndef RT_MIN_BLOCKS
 #define RT_MIN_BLOCKS 4       // <= 128 registers per thread: 16 warps per SM
 #endif
+#ifndef RT_GRID_ROLLED
+#define RT_GRID_ROLLED 1      // grid equilibrium: one copy of the stage code (stage loop not unrolled)
+#endif
 constexpr int TRACE_BLOCK = RT_TRACE_BLOCK;
 
 template <class T>
@@ -55,7 +58,7 @@ RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
   T k[6], acc[6], ys[6];
   bool ok = true;
-  if (EQ == EQ_GRID) {
+  if (EQ == EQ_GRID && RT_GRID_ROLLED) {
 #pragma unroll
     for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; }
 #pragma unroll 1
