@@ -63,6 +63,9 @@ def _load():
         lib = ctypes.CDLL(str(build()))
         P, D, I64, I32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_int
         lib.oracle_trace.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, I64, I64, D, I64, P, P, P, P, I32]
+        lib.oracle_trace_w.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, I64, D, I64, P, P, P, P, I32]
+        lib.oracle_launch_w.argtypes = [ctypes.POINTER(_CEq), I32, I32, P, P, P, I64, P, P]
+        lib.oracle_diagnostics.argtypes = [ctypes.POINTER(_CEq), P, P, P, I64, P]
         lib.oracle_dispersion.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, I64, P, P, P]
         lib.oracle_dispersion_value.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, P]
         lib.oracle_plasma.argtypes = [ctypes.POINTER(_CEq), P, D, I64, P, P, P, P]
@@ -146,10 +149,15 @@ def max_threads() -> int:
 def trace(eq, disp, x0, k0, omega, n_steps, dt, save_stride=1, *, traj=False, final=True, residual=True,
           status=True, n_threads=0) -> dict:
     """Integrate the ray equations; returns a dict with 'traj' [n_saved,6,n], 'final' [6,n],
-    'residual' ([n_saved,n] with traj else [n]) and 'status' [n] for the outputs requested."""
+    'residual' ([n_saved,n] with traj else [n]) and 'status' [n] for the outputs requested.
+    ``omega`` is one frequency for all rays or an array [n] with one frequency per ray (L147)."""
     lib, e = _load(), _eq(eq)
     x0, k0 = _soa(x0), _soa(k0)
     n = x0.shape[1]
+    per_ray = np.ndim(omega) > 0
+    if per_ray:
+        omega = np.ascontiguousarray(omega, dtype=np.float64)
+        assert omega.shape == (n,), omega.shape
     n_saved = n_steps // save_stride + 1
     out = {}
     if traj:
@@ -161,9 +169,10 @@ def trace(eq, disp, x0, k0, omega, n_steps, dt, save_stride=1, *, traj=False, fi
     if status:
         out["status"] = np.empty((n,), dtype=np.int32)
     ptr = lambda key: out[key].ctypes.data if key in out else None
-    rc = lib.oracle_trace(ctypes.byref(e.c), _disp(disp), x0.ctypes.data, k0.ctypes.data, float(omega), n,
-                          int(n_steps), float(dt), int(save_stride), ptr("traj"), ptr("final"), ptr("residual"),
-                          ptr("status"), int(n_threads))
+    fn, w = (lib.oracle_trace_w, omega.ctypes.data) if per_ray else (lib.oracle_trace, float(omega))
+    rc = fn(ctypes.byref(e.c), _disp(disp), x0.ctypes.data, k0.ctypes.data, w, n,
+            int(n_steps), float(dt), int(save_stride), ptr("traj"), ptr("final"), ptr("residual"),
+            ptr("status"), int(n_threads))
     if rc != 0:
         raise ValueError(f"oracle_trace rejected its arguments (rc={rc})")
     return out
@@ -210,13 +219,37 @@ def plasma(eq, x, omega):
 
 
 def launch(eq, disp, x0, dirs, omega, branch=0):
-    """On-shell launch wave vectors k0 [3,n] along unit directions dirs [3,n] (L159); also returns D there."""
+    """On-shell launch wave vectors k0 [3,n] along unit directions dirs [3,n] (L159); also returns D there.
+    ``omega``: a scalar or one frequency per ray [n]."""
     lib, e = _load(), _eq(eq)
     x0, dirs = _soa(x0), _soa(dirs)
     n = x0.shape[1]
     k0, D = np.empty((3, n)), np.empty(n)
-    rc = lib.oracle_launch(ctypes.byref(e.c), _disp(disp), int(branch), x0.ctypes.data, dirs.ctypes.data,
-                           float(omega), n, k0.ctypes.data, D.ctypes.data)
+    if np.ndim(omega) > 0:
+        w = np.ascontiguousarray(omega, dtype=np.float64)
+        assert w.shape == (n,), w.shape
+        rc = lib.oracle_launch_w(ctypes.byref(e.c), _disp(disp), int(branch), x0.ctypes.data, dirs.ctypes.data,
+                                 w.ctypes.data, n, k0.ctypes.data, D.ctypes.data)
+    else:
+        rc = lib.oracle_launch(ctypes.byref(e.c), _disp(disp), int(branch), x0.ctypes.data, dirs.ctypes.data,
+                               float(omega), n, k0.ctypes.data, D.ctypes.data)
     if rc != 0:
         raise ValueError("oracle_launch rejected its arguments")
     return k0, D
+
+
+DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
+
+
+def diagnostics(eq, x, k, omega):
+    """Critical-surface diagnostics (L149, Fig. 3-4) at points x, k [3,n]: array [10,n] with rows ``DIAG_ROWS``;
+    ``omega`` a scalar or one frequency per point [n]."""
+    lib, e = _load(), _eq(eq)
+    x, k = _soa(x), _soa(k)
+    n = x.shape[1]
+    w = np.ascontiguousarray(np.broadcast_to(np.asarray(omega, dtype=np.float64), (n,)))
+    out = np.empty((10, n))
+    rc = lib.oracle_diagnostics(ctypes.byref(e.c), x.ctypes.data, k.ctypes.data, w.ctypes.data, n, out.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_diagnostics rejected its arguments")
+    return out

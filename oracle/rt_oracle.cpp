@@ -348,9 +348,10 @@ extern "C" {
 // Trace n_rays rays.  All pointers are HOST pointers.  Layouts equal the C-ABI's (include/rt.h):
 // x0,k0 [3][n_rays]; out_traj [n_steps/save_stride+1][6][n_rays]; out_final [6][n_rays];
 // out_residual [n_saved][n_rays] if out_traj else [n_rays]; out_status [n_rays].  Any output may be NULL.
-int oracle_trace(const orc_equilibrium* eq, int disp, const double* x0, const double* k0, double omega,
-                 int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, double* out_traj,
-                 double* out_final, double* out_residual, int32_t* out_status, int n_threads) {
+// omega_rays: one frequency per ray [n_rays] (L147: w is a per-ray kernel input), or NULL to use `omega_all` for every ray.
+static int trace_impl(const orc_equilibrium* eq, int disp, const double* x0, const double* k0, double omega_all,
+                      const double* omega_rays, int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride,
+                      double* out_traj, double* out_final, double* out_residual, int32_t* out_status, int n_threads) {
   if (!eq || !combo_supported(*eq, disp) || n_rays < 0 || n_steps < 0 || save_stride < 1) return -1;
   if (out_traj && (n_steps % save_stride) != 0) return -1;
   const double h = dt / C_LIGHT;   // seconds (reading A3: dt is in tau = c t)
@@ -359,6 +360,7 @@ int oracle_trace(const orc_equilibrium* eq, int disp, const double* x0, const do
 #endif
 #pragma omp parallel for schedule(dynamic, 16)
   for (int64_t i = 0; i < n_rays; ++i) {
+    const double omega = omega_rays ? omega_rays[i] : omega_all;
     double y[6];
     for (int c = 0; c < 3; ++c) { y[c] = x0[c * n_rays + i]; y[3 + c] = k0[c * n_rays + i]; }
     int status = 0;
@@ -377,6 +379,55 @@ int oracle_trace(const orc_equilibrium* eq, int disp, const double* x0, const do
     if (out_final) for (int c = 0; c < 6; ++c) out_final[c * n_rays + i] = y[c];
     if (!out_traj && out_residual) out_residual[i] = residual(*eq, disp, omega, y);
     if (out_status) out_status[i] = status;
+  }
+  return 0;
+}
+
+int oracle_trace(const orc_equilibrium* eq, int disp, const double* x0, const double* k0, double omega,
+                 int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, double* out_traj,
+                 double* out_final, double* out_residual, int32_t* out_status, int n_threads) {
+  return trace_impl(eq, disp, x0, k0, omega, nullptr, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual,
+                    out_status, n_threads);
+}
+
+// The same with one frequency per ray: omega [n_rays].
+int oracle_trace_w(const orc_equilibrium* eq, int disp, const double* x0, const double* k0, const double* omega,
+                   int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, double* out_traj,
+                   double* out_final, double* out_residual, int32_t* out_status, int n_threads) {
+  if (!omega) return -1;
+  return trace_impl(eq, disp, x0, k0, 0.0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual,
+                    out_status, n_threads);
+}
+
+// Critical-surface diagnostics (L149: cut-offs and resonances; Fig. 3-4 L157/L175) at n points with one frequency per
+// point: out [10][n] = n_e, |B|, X = wpe^2/w^2, Y = |Wce|/w (electrons), S, Dx, P (Eq. 8-10), R = S + Dx, L = S - Dx,
+// n_par^2 = (n.B/|B|)^2 with n = c k / w (Eq. 6); n_par^2 = 0 where B = 0.  NaN outside the domain.
+int oracle_diagnostics(const orc_equilibrium* eq, const double* x, const double* k, const double* omega, int64_t n,
+                       double* out) {
+  if (!eq || !omega) return -1;
+  for (int64_t i = 0; i < n; ++i) {
+    const double xi[3] = {x[i], x[n + i], x[2 * n + i]};
+    const double w = omega[i];
+    const Plasma<double> pl = equilibrium<double>(*eq, xi);
+    if (!pl.inside) {
+      for (int r = 0; r < 10; ++r) out[r * n + i] = std::numeric_limits<double>::quiet_NaN();
+      continue;
+    }
+    const Stix<double> st = stix<double>(*eq, pl, w);
+    const double Bm = std::sqrt(pl.B[0] * pl.B[0] + pl.B[1] * pl.B[1] + pl.B[2] * pl.B[2]);
+    double npar = 0.0;
+    if (Bm > 0.0)
+      for (int c = 0; c < 3; ++c) npar += (C_LIGHT * k[c * n + i] / w) * (pl.B[c] / Bm);
+    out[0 * n + i] = pl.ne;
+    out[1 * n + i] = Bm;
+    out[2 * n + i] = pl.ne * (CHARGE_E * CHARGE_E / (EPS0 * MASS_E)) / (w * w);
+    out[3 * n + i] = (CHARGE_E / MASS_E) * Bm / w;
+    out[4 * n + i] = st.S;
+    out[5 * n + i] = st.Dx;
+    out[6 * n + i] = st.P;
+    out[7 * n + i] = st.S + st.Dx;
+    out[8 * n + i] = st.S - st.Dx;
+    out[9 * n + i] = npar * npar;
   }
   return 0;
 }
@@ -432,10 +483,11 @@ int oracle_plasma(const orc_equilibrium* eq, const double* x, double omega, int6
 //   COLD_FULL: the biquadratic A n^4 - B n^2 + C = 0 (Stix), A = S sin^2 + P cos^2, B = R L sin^2 + P S (1 + cos^2),
 //   C = P R L, theta the angle between dir and B; branch 0 = the root nearer to P ("O"), 1 = the other ("X")
 //   (reading A11).
-int oracle_launch(const orc_equilibrium* eq, int disp, int branch, const double* x0, const double* dir,
-                  double omega, int64_t n, double* k0, double* D_out) {
+static int launch_impl(const orc_equilibrium* eq, int disp, int branch, const double* x0, const double* dir,
+                       double omega_all, const double* omega_rays, int64_t n, double* k0, double* D_out) {
   if (!eq || !combo_supported(*eq, disp)) return -1;
   for (int64_t i = 0; i < n; ++i) {
+    const double omega = omega_rays ? omega_rays[i] : omega_all;
     const double xi[3] = {x0[i], x0[n + i], x0[2 * n + i]}, di[3] = {dir[i], dir[n + i], dir[2 * n + i]};
     const Plasma<double> pl = equilibrium<double>(*eq, xi);
     double n2 = std::numeric_limits<double>::quiet_NaN();
@@ -480,6 +532,17 @@ int oracle_launch(const orc_equilibrium* eq, int disp, int branch, const double*
     }
   }
   return 0;
+}
+
+int oracle_launch(const orc_equilibrium* eq, int disp, int branch, const double* x0, const double* dir,
+                  double omega, int64_t n, double* k0, double* D_out) {
+  return launch_impl(eq, disp, branch, x0, dir, omega, nullptr, n, k0, D_out);
+}
+
+int oracle_launch_w(const orc_equilibrium* eq, int disp, int branch, const double* x0, const double* dir,
+                    const double* omega, int64_t n, double* k0, double* D_out) {
+  if (!omega) return -1;
+  return launch_impl(eq, disp, branch, x0, dir, 0.0, omega, n, k0, D_out);
 }
 
 int oracle_max_threads(void) {

@@ -158,6 +158,13 @@ def tokamak_grid(n_rays: int, n_steps: int, seed: int, eps: float = 1e-3, precis
                     tuple(precisions), seed, extra=dict(eps=eps))
 
 
+def frequency_scan(n_rays: int, omega0: float, seed: int, spread: float = 0.1) -> np.ndarray:
+    """One wave frequency per ray, w_i = omega0 (1 + spread u_i), u_i ~ U[-1, 1] (SURVEY 8(f)-3: frequency scans;
+    PAPER.md L147: w is a per-ray kernel input).  Drawn from its own stream ``default_rng(seed + 900000)``."""
+    rng = np.random.default_rng(seed + 900000)
+    return omega0 * (1.0 + spread * rng.uniform(-1.0, 1.0, n_rays))
+
+
 # (n_rays, n_steps) of BASELINE.json's configs 1..5
 FULL_SIZES = {1: (1024, 1000), 2: (2**20, 2000), 3: (2**18, 3000), 4: (2**20, 1000), 5: (2**24, 500)}
 
