@@ -101,6 +101,15 @@ int rt_trace(const rt_equilibrium* eq, int disp, int precision, const void* x0, 
              int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
              void* out_residual, int32_t* out_status, void* cuda_stream);
 
+/* rt_trace with one frequency PER RAY ("inputs for x, k, t and w" -- w is a per-ray kernel input; frequency
+ * scans).  Identical to rt_trace except
+ *   omega         DEVICE double [n_rays], rad/s, each positive and finite (a ray with a bad w ends with status 2);
+ *                 always double, whatever `precision` is
+ * k0 and the k rows of the outputs are in rad/m at each ray's own frequency: n = c k / w_i (Eq. 6). */
+int rt_trace_w(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, const double* omega,
+               int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
+               void* out_residual, int32_t* out_status, void* cuda_stream);
+
 /* The same call with HOST buffers (pageable or pinned): copies x0, k0 to the device, runs the rt_trace kernel and
  * copies the requested outputs back, pipelined over ray chunks on the handle's own streams; returns after the
  * results are in host memory.  Uses (and grows) the handle's workspace: not re-entrant per handle. */
@@ -118,6 +127,25 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
  *   D_out         DEVICE double [n] D at the returned state (signed); or NULL */
 int rt_launch(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, double omega,
               int64_t n, double* k0, double* D_out, void* cuda_stream);
+
+/* rt_launch with one frequency per ray: omega DEVICE double [n]. */
+int rt_launch_w(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, const double* omega,
+                int64_t n, double* k0, double* D_out, void* cuda_stream);
+
+/* Critical-surface diagnostics at n points, e.g. the samples of a trajectory (cut-offs and resonances
+ * "denote important changes in wave behavior, and the behavior of rays in their vicinity is an indication of the
+ * correctness of the solution"; Fig. 3-4).  fp64.
+ *   x, k          DEVICE double [3][n]
+ *   omega         rad/s, used when omega_rays == NULL
+ *   omega_rays    DEVICE double [n] per-point frequencies, or NULL
+ *   out           DEVICE double [RT_NDIAG][n], rows:
+ *                   0 n_e [m^-3]   1 |B| [T]   2 X = wpe^2/w^2   3 Y = |Wce|/w   4 S   5 D   6 P   (Eq. 8-10: eps11 = S,
+ *                   eps12 = -i D, eps33 = P)   7 R = S + D   8 L = S - D   9 n_par^2 = (n.B)^2/|B|^2 (0 where B = 0)
+ *                 Cut-offs: P = 0 (O-mode; X = 1 for electrons only), R = 0, L = 0.  Resonances: S = 0 (upper hybrid),
+ *                 Y = 1 (cyclotron).  All rows are NaN at points outside the equilibrium's domain. */
+#define RT_NDIAG 10
+int rt_diagnostics(const rt_equilibrium* eq, const double* x, const double* k, double omega, const double* omega_rays,
+                   int64_t n, double* out, void* cuda_stream);
 
 /* Diagnostic evaluation of the integrand at n points (the quantities one RK4 stage computes):
  *   x, k          DEVICE [3][n]

@@ -24,8 +24,10 @@ DISP_KINDS = {"omode": 0, "xmode": 1, "cold_full": 2}
 PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
-SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_host", "rt_launch", "rt_rhs", "rt_reduce",
-           "rt_fma_peak", "rt_launch_count", "rt_last_error", "rt_version")
+SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_launch", "rt_launch_w",
+           "rt_diagnostics", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_launch_count", "rt_last_error", "rt_version")
+NDIAG = 10
+DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
 
 
 class RtError(RuntimeError):
@@ -88,6 +90,9 @@ def load() -> ctypes.CDLL:
         lib.rt_create_equilibrium.argtypes = [ctypes.POINTER(EquilibriumDesc), ctypes.POINTER(P)]
         lib.rt_destroy.argtypes = [P]
         lib.rt_trace.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
+        lib.rt_trace_w.argtypes = [P, I32, I32, P, P, P, I64, I64, D, I64, P, P, P, P, P]
+        lib.rt_launch_w.argtypes = [P, I32, I32, P, P, P, I64, P, P, P]
+        lib.rt_diagnostics.argtypes = [P, P, P, D, P, I64, P, P]
         lib.rt_trace_host.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P]
         lib.rt_launch.argtypes = [P, I32, I32, P, P, D, I64, P, P, P]
         lib.rt_rhs.argtypes = [P, I32, I32, P, P, D, I64, P, P, P, P]
@@ -177,9 +182,20 @@ def _dev_soa(t, rows, n=None):
     return t
 
 
-def trace(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: float, save_stride: int = 1, *, traj=False,
+def _omega_rays(omega, n):
+    """None for a scalar frequency, else the validated per-ray tensor (float64 CUDA [n])."""
+    import torch
+    if not torch.is_tensor(omega):
+        return None
+    if not omega.is_cuda or omega.dtype != torch.float64 or not omega.is_contiguous() or tuple(omega.shape) != (n,):
+        raise ValueError(f"per-ray omega must be a contiguous float64 CUDA tensor of shape [{n}]")
+    return omega
+
+
+def trace(eq: Equilibrium, disp, x0, k0, omega, n_steps: int, dt: float, save_stride: int = 1, *, traj=False,
           final=True, residual=True, status=True, out: dict | None = None) -> dict:
-    """``rt_trace`` on the current CUDA stream.  x0, k0: CUDA tensors [3, n_rays] (float64 or float32).  Returns a dict
+    """``rt_trace`` (``rt_trace_w`` when ``omega`` is a float64 CUDA tensor [n_rays]) on the current CUDA stream.
+    x0, k0: CUDA tensors [3, n_rays] (float64 or float32).  Returns a dict
     of freshly allocated (or, via ``out``, caller-provided) device tensors: 'traj' [n_saved, 6, n], 'final' [6, n],
     'residual' ([n_saved, n] with traj else [n]), 'status' [n] int32.  Does not synchronise."""
     import torch
@@ -201,10 +217,15 @@ def trace(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: float, 
         o["residual"] = torch.empty((n_saved, n) if traj else (n,), **kw)
     if status and "status" not in o:
         o["status"] = torch.empty((n,), dtype=torch.int32, device=x0.device)
-    _check(lib.rt_trace(eq.handle, _disp(disp), prec, _ptr(x0), _ptr(k0), float(omega), n, int(n_steps), float(dt),
-                        int(save_stride), _ptr(o.get("traj") if traj else None), _ptr(o.get("final") if final else None),
-                        _ptr(o.get("residual") if residual else None), _ptr(o.get("status") if status else None),
-                        _stream()))
+    outs = (_ptr(o.get("traj") if traj else None), _ptr(o.get("final") if final else None),
+            _ptr(o.get("residual") if residual else None), _ptr(o.get("status") if status else None))
+    w = _omega_rays(omega, n)
+    if w is None:
+        _check(lib.rt_trace(eq.handle, _disp(disp), prec, _ptr(x0), _ptr(k0), float(omega), n, int(n_steps), float(dt),
+                            int(save_stride), *outs, _stream()))
+    else:
+        _check(lib.rt_trace_w(eq.handle, _disp(disp), prec, _ptr(x0), _ptr(k0), _ptr(w), n, int(n_steps), float(dt),
+                              int(save_stride), *outs, _stream()))
     return o
 
 
@@ -252,9 +273,9 @@ def trace_host(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: fl
     return o
 
 
-def launch(eq: Equilibrium, disp, x0, dirs, omega: float, branch: int = 0):
-    """``rt_launch``: on-shell k0 [3, n] along unit directions dirs [3, n] from positions x0 (float64 CUDA tensors);
-    also returns D at the launch state."""
+def launch(eq: Equilibrium, disp, x0, dirs, omega, branch: int = 0):
+    """``rt_launch`` (``rt_launch_w`` when ``omega`` is a float64 CUDA tensor [n]): on-shell k0 [3, n] along unit
+    directions dirs [3, n] from positions x0 (float64 CUDA tensors); also returns D at the launch state."""
     import torch
     lib = load()
     x0 = _dev_soa(x0, 3)
@@ -264,9 +285,31 @@ def launch(eq: Equilibrium, disp, x0, dirs, omega: float, branch: int = 0):
         raise TypeError("rt_launch is fp64 only")
     k0 = torch.empty((3, n), dtype=torch.float64, device=x0.device)
     D = torch.empty((n,), dtype=torch.float64, device=x0.device)
-    _check(lib.rt_launch(eq.handle, _disp(disp), int(branch), _ptr(x0), _ptr(dirs), float(omega), n, _ptr(k0), _ptr(D),
-                         _stream()))
+    w = _omega_rays(omega, n)
+    if w is None:
+        _check(lib.rt_launch(eq.handle, _disp(disp), int(branch), _ptr(x0), _ptr(dirs), float(omega), n, _ptr(k0), _ptr(D),
+                             _stream()))
+    else:
+        _check(lib.rt_launch_w(eq.handle, _disp(disp), int(branch), _ptr(x0), _ptr(dirs), _ptr(w), n, _ptr(k0), _ptr(D),
+                               _stream()))
     return k0, D
+
+
+def diagnostics(eq: Equilibrium, x, k, omega):
+    """``rt_diagnostics``: [NDIAG, n] float64 device tensor, rows ``DIAG_ROWS`` (n_e, |B|, X, Y, S, D, P, R, L, n_par^2)
+    at points x, k [3, n] (float64 CUDA tensors); ``omega`` a float or a float64 CUDA tensor [n]."""
+    import torch
+    lib = load()
+    x = _dev_soa(x, 3)
+    n = x.shape[1]
+    k = _dev_soa(k, 3, n)
+    if x.dtype != torch.float64 or k.dtype != torch.float64:
+        raise TypeError("rt_diagnostics is fp64 only")
+    out = torch.empty((NDIAG, n), dtype=torch.float64, device=x.device)
+    w = _omega_rays(omega, n)
+    _check(lib.rt_diagnostics(eq.handle, _ptr(x), _ptr(k), 0.0 if w is not None else float(omega), _ptr(w), n, _ptr(out),
+                              _stream()))
+    return out
 
 
 def rhs(eq: Equilibrium, disp, x, k, omega: float):

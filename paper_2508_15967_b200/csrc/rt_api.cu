@@ -99,13 +99,16 @@ unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / 
 template <class T>
 int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const rt::TraceArgs<T>& A, cudaStream_t st) {
   if (A.n_rays == 0) return RT_OK;
-  const unsigned grid = grid_for(A.n_rays, rt::TRACE_BLOCK);
-#define M(E, D)                                                                   \
-  if (kernel_kind(eq) == (E) && disp == (D)) {                                         \
-    rt::trace_kernel<T, E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, A);            \
-    ++g_launches;                                                                 \
-    RT_CUDA(cudaGetLastError());                                                  \
-    return RT_OK;                                                                 \
+#define M(E, D)                                                                            \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                             \
+    constexpr int block = rt::TraceShape<T, E>::BLOCK;                                     \
+    if (A.omega)                                                                           \
+      rt::trace_kernel<T, E, D, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A);  \
+    else                                                                                   \
+      rt::trace_kernel<T, E, D, false><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
+    ++g_launches;                                                                          \
+    RT_CUDA(cudaGetLastError());                                                           \
+    return RT_OK;                                                                          \
   }
   RT_FOR_COMBOS(M)
 #undef M
@@ -116,10 +119,10 @@ template <class T>
 int launch_rhs(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const T* x, const T* k, long long n, T* D_out,
                T* rhs_out, int32_t* inside_out, cudaStream_t st) {
   if (n == 0) return RT_OK;
-  const unsigned grid = grid_for(n, rt::TRACE_BLOCK);
+  const unsigned grid = grid_for(n, rt::AUX_BLOCK);
 #define M(E, D)                                                                                        \
   if (kernel_kind(eq) == (E) && disp == (D)) {                                                              \
-    rt::rhs_kernel<T, E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, x, k, n, D_out, rhs_out, inside_out);  \
+    rt::rhs_kernel<T, E, D><<<grid, rt::AUX_BLOCK, 0, st>>>(P, x, k, n, D_out, rhs_out, inside_out);  \
     ++g_launches;                                                                                      \
     RT_CUDA(cudaGetLastError());                                                                       \
     return RT_OK;                                                                                      \
@@ -130,27 +133,38 @@ int launch_rhs(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const
 }
 
 int launch_launch(const rt_equilibrium* eq, int disp, const rt::Params<double>& P, int branch, const double* x0,
-                  const double* dir, long long n, double* k0, double* D_out, cudaStream_t st) {
+                  const double* dir, const double* omega, double omega_ref, long long n, double* k0, double* D_out,
+                  cudaStream_t st) {
   if (n == 0) return RT_OK;
-  const unsigned grid = grid_for(n, rt::TRACE_BLOCK);
-#define M(E, D)                                                                                  \
-  if (kernel_kind(eq) == (E) && disp == (D)) {                                                        \
-    rt::launch_kernel<E, D><<<grid, rt::TRACE_BLOCK, 0, st>>>(P, branch, x0, dir, n, k0, D_out);  \
-    ++g_launches;                                                                                \
-    RT_CUDA(cudaGetLastError());                                                                 \
-    return RT_OK;                                                                                \
+  const unsigned grid = grid_for(n, rt::AUX_BLOCK);
+#define M(E, D)                                                                                                        \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                                                         \
+    if (omega)                                                                                                         \
+      rt::launch_kernel<E, D, true><<<grid, rt::AUX_BLOCK, 0, st>>>(P, branch, x0, dir, omega, omega_ref, n, k0, D_out);  \
+    else                                                                                                               \
+      rt::launch_kernel<E, D, false><<<grid, rt::AUX_BLOCK, 0, st>>>(P, branch, x0, dir, omega, omega_ref, n, k0, D_out); \
+    ++g_launches;                                                                                                      \
+    RT_CUDA(cudaGetLastError());                                                                                       \
+    return RT_OK;                                                                                                      \
   }
   RT_FOR_COMBOS(M)
 #undef M
   return fail(RT_ERR_UNSUPPORTED, "no kernel for this equilibrium / dispersion combination");
 }
 
+// Per-ray frequencies: the per-call constants are folded at this reference and rescaled per thread (rt_kernels.cuh:
+// params_at_frequency).  1 rad/s keeps every folded constant finite in fp32 and needs no knowledge of the device array.
+constexpr double kOmegaRefPerRay = 1.0;
+
+// omega_rays: DEVICE [n_rays] per-ray frequencies (then `omega` is ignored), or NULL for the one frequency `omega`
 template <class T>
-int trace_device(const rt_equilibrium* eq, int disp, const void* x0, const void* k0, double omega, long long n_rays,
-                 long long n_steps, double dt, long long save_stride, void* out_traj, void* out_final,
-                 void* out_residual, int32_t* out_status, cudaStream_t st) {
-  const rt::Params<T> P = make_params<T>(eq, omega);
+int trace_device(const rt_equilibrium* eq, int disp, const void* x0, const void* k0, double omega,
+                 const double* omega_rays, long long n_rays, long long n_steps, double dt, long long save_stride,
+                 void* out_traj, void* out_final, void* out_residual, int32_t* out_status, cudaStream_t st) {
+  const rt::Params<T> P = make_params<T>(eq, omega_rays ? kOmegaRefPerRay : omega);
   rt::TraceArgs<T> A;
+  A.omega = omega_rays;
+  A.omega_ref = kOmegaRefPerRay;
   A.x0 = static_cast<const T*>(x0);
   A.k0 = static_cast<const T*>(k0);
   A.traj = static_cast<T*>(out_traj);
@@ -318,8 +332,25 @@ int rt_trace(const rt_equilibrium* eq, int disp, int precision, const void* x0, 
     return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (precision == RT_F64)
-    return trace_device<double>(eq, disp, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
-  return trace_device<float>(eq, disp, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+    return trace_device<double>(eq, disp, x0, k0, omega, nullptr, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+  return trace_device<float>(eq, disp, x0, k0, omega, nullptr, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+}
+
+int rt_trace_w(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, const double* omega,
+               int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
+               void* out_residual, int32_t* out_status, void* cuda_stream) {
+  int rc = check_trace_args(eq, disp, precision, x0, k0, 1.0, n_rays, n_steps, dt, save_stride, out_traj);
+  if (rc) return rc;
+  if (n_rays == 0) return RT_OK;
+  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(k0, "k0", false)) ||
+      (rc = require_device_ptr(omega, "omega", false)) ||
+      (rc = require_device_ptr(out_traj, "out_traj", true)) || (rc = require_device_ptr(out_final, "out_final", true)) ||
+      (rc = require_device_ptr(out_residual, "out_residual", true)) || (rc = require_device_ptr(out_status, "out_status", true)))
+    return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (precision == RT_F64)
+    return trace_device<double>(eq, disp, x0, k0, 0.0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+  return trace_device<float>(eq, disp, x0, k0, 0.0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
 }
 
 int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
@@ -373,9 +404,9 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
     void* r = out_residual ? dres : nullptr;
     int32_t* s = out_status ? reinterpret_cast<int32_t*>(dstat) : nullptr;
     if (precision == RT_F64)
-      rc = trace_device<double>(eq, disp, dx, dk, omega, c, n_steps, dt, save_stride, t, f, r, s, st);
+      rc = trace_device<double>(eq, disp, dx, dk, omega, nullptr, c, n_steps, dt, save_stride, t, f, r, s, st);
     else
-      rc = trace_device<float>(eq, disp, dx, dk, omega, c, n_steps, dt, save_stride, t, f, r, s, st);
+      rc = trace_device<float>(eq, disp, dx, dk, omega, nullptr, c, n_steps, dt, save_stride, t, f, r, s, st);
     if (rc) { cudaDeviceSynchronize(); return rc; }
     if (out_traj)
       RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_traj) + (size_t)off * es, hp, dtraj, w, w, (size_t)n_saved * 6, cudaMemcpyDeviceToHost, st));
@@ -403,7 +434,52 @@ int rt_launch(const rt_equilibrium* eq, int disp, int branch, const double* x0, 
       (rc = require_device_ptr(k0, "k0", false)) || (rc = require_device_ptr(D_out, "D_out", true)))
     return rc;
   const rt::Params<double> P = make_params<double>(eq, omega);
-  return launch_launch(eq, disp, P, branch, x0, dir, n, k0, D_out, static_cast<cudaStream_t>(cuda_stream));
+  return launch_launch(eq, disp, P, branch, x0, dir, nullptr, omega, n, k0, D_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rt_launch_w(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, const double* omega,
+                int64_t n, double* k0, double* D_out, void* cuda_stream) {
+  int rc = check_combo(eq, disp);
+  if (rc) return rc;
+  if (branch != 0 && branch != 1) return fail(RT_ERR_INVALID, "branch must be 0 or 1");
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  if (n == 0) return RT_OK;
+  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(dir, "dir", false)) ||
+      (rc = require_device_ptr(omega, "omega", false)) || (rc = require_device_ptr(k0, "k0", false)) ||
+      (rc = require_device_ptr(D_out, "D_out", true)))
+    return rc;
+  const rt::Params<double> P = make_params<double>(eq, kOmegaRefPerRay);
+  return launch_launch(eq, disp, P, branch, x0, dir, omega, kOmegaRefPerRay, n, k0, D_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rt_diagnostics(const rt_equilibrium* eq, const double* x, const double* k, double omega, const double* omega_rays,
+                   int64_t n, double* out, void* cuda_stream) {
+  if (!eq) return fail(RT_ERR_INVALID, "equilibrium handle is NULL");
+  int rc;
+  if (!omega_rays && (rc = check_omega(omega))) return rc;
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  if (n == 0) return RT_OK;
+  if ((rc = require_device_ptr(x, "x", false)) || (rc = require_device_ptr(k, "k", false)) ||
+      (rc = require_device_ptr(omega_rays, "omega_rays", true)) || (rc = require_device_ptr(out, "out", false)))
+    return rc;
+  const double wref = omega_rays ? kOmegaRefPerRay : omega;
+  const rt::Params<double> P = make_params<double>(eq, wref);
+  const double inv_alpha = rt::kEps0 * rt::kMe * wref * wref / (rt::kQe * rt::kQe);   // n_e = X / alpha at w_ref
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const unsigned grid = grid_for(n, rt::AUX_BLOCK);
+#define M(E)                                                                                                    \
+  if (kernel_kind(eq) == (E)) {                                                                                 \
+    if (omega_rays)                                                                                             \
+      rt::diag_kernel<E, true><<<grid, rt::AUX_BLOCK, 0, st>>>(P, inv_alpha, x, k, omega_rays, wref, n, out);   \
+    else                                                                                                        \
+      rt::diag_kernel<E, false><<<grid, rt::AUX_BLOCK, 0, st>>>(P, inv_alpha, x, k, omega_rays, wref, n, out);  \
+    ++g_launches;                                                                                               \
+    RT_CUDA(cudaGetLastError());                                                                                \
+    return RT_OK;                                                                                               \
+  }
+  M(rt::EQ_PARABOLIC) M(rt::EQ_LINEAR) M(rt::EQ_TOKAMAK) M(rt::EQ_TOKAMAK_POW) M(rt::EQ_GRID)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no diagnostics kernel for this equilibrium kind");
 }
 
 int rt_rhs(const rt_equilibrium* eq, int disp, int precision, const void* x, const void* k, double omega, int64_t n,

@@ -15,17 +15,27 @@
 
 namespace rt {
 
-// Tuning knobs (defaults chosen by measurement on B200, profiles/r1_tuning.md).
-#ifndef RT_TRACE_BLOCK
-#define RT_TRACE_BLOCK 128
-#endif
-#ifndef RT_MIN_BLOCKS
-#define RT_MIN_BLOCKS 4       // <= 128 registers per thread: 16 warps per SM
-#endif
+// Launch shapes.  The trace kernels are bound by the FP64 (FP32) pipe and by registers, not by memory, so what is tuned is
+// how many warps fit beside each other: 64-thread blocks with a per-kernel register cap (`__maxnreg__`) chosen by
+// measurement on B200 (profiles/r1_tuning.md):
+//   fp64, analytic equilibria   112 registers -> 9 blocks = 18 warps per SM (128 registers / 16 warps: +1.7 % time;
+//                                96 registers / 20 warps spills 112 B and is 2.8 % slower)
+//   fp64, grid equilibrium       96 registers -> 10 blocks = 20 warps per SM (the LDS latency of the cell cache wants
+//                                more warps: 2.9 % faster than 128 registers; no spills)
+//   fp32                         72 registers -> 14 blocks = 28 warps per SM
+// The diagnostic kernels (rhs, launch) use plain 128-thread blocks.
 #ifndef RT_GRID_ROLLED
 #define RT_GRID_ROLLED 1      // grid equilibrium: one copy of the stage code (stage loop not unrolled)
 #endif
-constexpr int TRACE_BLOCK = RT_TRACE_BLOCK;
+constexpr int AUX_BLOCK = 128;
+template <class T, int EQ> struct TraceTune { static constexpr int BLOCK = 64, MAXNREG = 72; };
+template <int EQ> struct TraceTune<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
+template <> struct TraceTune<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 96; };
+#ifdef RT_TRACE_BLOCK       // experiments: one shape for every trace kernel
+template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = RT_TRACE_BLOCK, MAXNREG = RT_MAXNREG; };
+#else
+template <class T, int EQ> struct TraceShape : TraceTune<T, EQ> {};
+#endif
 
 template <class T>
 struct TraceArgs {
@@ -39,6 +49,8 @@ struct TraceArgs {
   long long n_steps;
   long long stride;
   T h;                  // step in tau = c t
+  const double* omega;  // per-ray frequencies [n_rays] (PW kernels only), rad/s
+  double omega_ref;     // the frequency the Params were folded at
 };
 
 // One classical RK4 step (reading A7): stage abscissae (0, 1/2, 1/2, 1), weights (1, 2, 2, 1)/6, written so that every
@@ -158,68 +170,121 @@ struct GatherCached {
 };
 
 template <class T, int EQ> struct TraceGather { typedef GatherDirect type; };
-template <class T> struct TraceGather<T, EQ_GRID> { typedef GatherCached<T, TRACE_BLOCK> type; };
+template <class T> struct TraceGather<T, EQ_GRID> { typedef GatherCached<T, TraceShape<T, EQ_GRID>::BLOCK> type; };
 
-template <class T, int EQ, int DISP>
-__global__ void __launch_bounds__(TRACE_BLOCK, RT_MIN_BLOCKS)
-trace_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ TraceArgs<T> A) {
+// Per-ray frequency (w is a per-ray kernel input).  The per-call constants are folded at
+// the reference frequency w_ref; a ray with its own w sees X and Y^2 scaled by lam^2 and n = c k/w by lam, lam = w_ref/w.
+// The thread-local copy below overrides exactly the w-dependent fields; everything else stays in the constant bank.
+template <class T>
+RT_DEV Params<T> params_at_frequency(const Params<T>& P, double lam) {
+  Params<T> Q = P;
+  const double l2 = lam * lam;
+  Q.xs = T(P.xs * l2); Q.beta = T(P.beta * l2); Q.beta2 = T(P.beta2 * l2);
+  Q.par_g = T(P.par_g * l2); Q.lin_gx = T(P.lin_gx * l2); Q.two_xs_a2 = T(P.two_xs_a2 * l2);
+  Q.k2n = T(P.k2n * lam); Q.n2k = T(P.n2k / lam);
+  return Q;
+}
+
+// Output staging: 128-bit coalesced stores (DESIGN.md section 6 "Trajectory stores").  A saved sample is 6 state rows
+// (+ 1 residual row) of consecutive rays.  Each thread drops its 7 values into its column of a [7][BLOCK] shared array;
+// after a warp barrier lane l reads 16-byte chunks along the rows (conflict-free) and writes them with one 128-bit
+// store each, so a warp emits 4 (fp64) / 2 (fp32) STG.128 wavefront groups of 512 contiguous bytes per row pair instead
+// of 7 STG.64 / STG.32.  Requires the row pitch N to be a multiple of 16 / sizeof(T) (rows stay 16-byte aligned); other
+// N fall back to scalar stores.  The staging slice is private to the warp: __syncwarp() is the only barrier.
+template <class T, int BLOCK>
+struct RowStore {
+  typedef typename Vec16<T>::type V;
+  static constexpr int VEC = 16 / sizeof(T), CPR = 32 / VEC;    // elements per chunk, chunks per row per warp
+  T* stage;              // this warp's slice: row r at stage[r * BLOCK + lane]
+  long long N, i0;       // row pitch; first ray of this warp
+  int lane;
+  bool vec;
+  // rows6: row 0 of a [6][N] block or NULL; res_row: a [N] row or NULL
+  RT_DEV void store(T* rows6, T* res_row, const T* v, T r, bool valid) const {
+    if (!vec) {
+      if (!valid) return;
+      if (rows6) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) rows6[c * N + i0 + lane] = v[c];
+      }
+      if (res_row) res_row[i0 + lane] = r;
+      return;
+    }
+#pragma unroll
+    for (int c = 0; c < 6; ++c) stage[c * BLOCK + lane] = v[c];
+    stage[6 * BLOCK + lane] = r;
+    __syncwarp();
+    const int first = rows6 ? 0 : 6 * CPR, last = res_row ? 7 * CPR : 6 * CPR;
+    for (int q = first + lane; q < last; q += 32) {
+      const int row = q / CPR, col = (q % CPR) * VEC;
+      if (i0 + col < N) {
+        const V val = *reinterpret_cast<const V*>(stage + row * BLOCK + col);
+        T* dst = (row < 6) ? rows6 + row * N : res_row;
+        *reinterpret_cast<V*>(dst + i0 + col) = val;
+      }
+    }
+    __syncwarp();
+  }
+};
+
+template <class T, int EQ, int DISP, bool PW>
+__global__ void __maxnreg__((TraceShape<T, EQ>::MAXNREG + (PW ? 16 : 0)))
+trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ TraceArgs<T> A) {
+  constexpr int BLOCK = TraceShape<T, EQ>::BLOCK;
   const long long N = A.n_rays;
-  const long long i = (long long)blockIdx.x * TRACE_BLOCK + threadIdx.x;
+  const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
+  const bool valid = i < N;
   typename TraceGather<T, EQ>::type gather;
   if constexpr (EQ == EQ_GRID) {
-    typedef GatherCached<T, TRACE_BLOCK> GC;
-    __shared__ typename GC::V cache[GC::CHUNKS * TRACE_BLOCK];
+    typedef GatherCached<T, BLOCK> GC;
+    __shared__ typename GC::V cache[GC::CHUNKS * BLOCK];
     gather.col = cache + threadIdx.x;
     gather.cell = -1; gather.pcell = -1;
   }
-  if (i >= N) return;
+  __shared__ __align__(16) T stage[7 * BLOCK];
+  Params<T> Pw;                                    // PW only: this ray's own copy of the w-dependent constants
+  if constexpr (PW) Pw = params_at_frequency(P0, valid ? A.omega_ref / A.omega[i] : 1.0);
+  const Params<T>& P = PW ? Pw : P0;
   T y[6];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    y[c] = A.x0[c * N + i];
-    y[3 + c] = A.k0[c * N + i] * P.k2n;          // n = c k / w  (Eq. 6)
+    y[c] = valid ? A.x0[c * N + i] : T(0);
+    y[3 + c] = valid ? A.k0[c * N + i] * P.k2n : T(0);          // n = c k / w  (Eq. 6)
   }
-  int status = 0;
-  long long m = 0;                                 // next trajectory sample
-  if (A.traj) {
+  int status = valid ? 0 : 3;                      // 3: padding lane of the last block, never stored
+  // Everything the store needs is recomputed here from threadIdx / the kernel arguments, so that nothing of it stays
+  // live across the step loop (the loop is register-bound).
+  auto save = [&](T* rows6, T* res_row) {
+    RowStore<T, BLOCK> out;
+    out.lane = threadIdx.x & 31;
+    out.stage = stage + (threadIdx.x & ~31);
+    out.N = A.n_rays;
+    out.i0 = (long long)blockIdx.x * BLOCK + (threadIdx.x & ~31);
+    out.vec = (A.n_rays % RowStore<T, BLOCK>::VEC) == 0;
+    T v[6];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      A.traj[(m * 6 + c) * N + i] = y[c];
-      A.traj[(m * 6 + 3 + c) * N + i] = y[3 + c] * P.n2k;
-    }
-    if (A.res) A.res[m * N + i] = abs_residual<T, EQ, DISP>(P, y, gather);
-    ++m;
+    for (int c = 0; c < 3; ++c) { v[c] = y[c]; v[3 + c] = y[3 + c] * P.n2k; }
+    const T r = res_row ? abs_residual<T, EQ, DISP>(P, y, gather) : T(0);
+    out.store(rows6, res_row, v, r, out.i0 + out.lane < A.n_rays);
+  };
+  // Sample m = state after m * stride steps (sample 0 = launch state).  The inner loop holds the step and nothing else.
+  const long long n_outer = A.traj ? A.n_steps / A.stride : 1, n_inner = A.traj ? A.stride : A.n_steps;
+  if (A.traj) save(A.traj, A.res);
+  for (long long m = 1; m <= n_outer; ++m) {
+#pragma unroll 1
+    for (long long s = 0; s < n_inner; ++s)
+      if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, y, gather);
+    if (A.traj) save(A.traj + m * 6 * A.n_rays, A.res ? A.res + m * A.n_rays : nullptr);
   }
-  long long countdown = A.stride;
-  for (long long s = 0; s < A.n_steps; ++s) {
-    if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, y, gather);
-    if (A.traj && --countdown == 0) {
-      countdown = A.stride;
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        A.traj[(m * 6 + c) * N + i] = y[c];
-        A.traj[(m * 6 + 3 + c) * N + i] = y[3 + c] * P.n2k;
-      }
-      if (A.res) A.res[m * N + i] = abs_residual<T, EQ, DISP>(P, y, gather);
-      ++m;
-    }
-  }
-  if (A.fin) {
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      A.fin[c * N + i] = y[c];
-      A.fin[(3 + c) * N + i] = y[3 + c] * P.n2k;
-    }
-  }
-  if (!A.traj && A.res) A.res[i] = abs_residual<T, EQ, DISP>(P, y, gather);
-  if (A.status) A.status[i] = status;
+  if (A.fin || (!A.traj && A.res)) save(A.fin, A.traj ? nullptr : A.res);
+  if (A.status && valid) A.status[i] = status;
 }
 
 template <class T, int EQ, int DISP>
-__global__ void __launch_bounds__(TRACE_BLOCK)
+__global__ void __launch_bounds__(AUX_BLOCK)
 rhs_kernel(const __grid_constant__ Params<T> P, const T* __restrict__ x, const T* __restrict__ k, long long n,
            T* __restrict__ D_out, T* __restrict__ rhs_out, int32_t* __restrict__ inside_out) {
-  const long long i = (long long)blockIdx.x * TRACE_BLOCK + threadIdx.x;
+  const long long i = (long long)blockIdx.x * AUX_BLOCK + threadIdx.x;
   if (i >= n) return;
   T y[6], f[6];
 #pragma unroll
@@ -239,12 +304,14 @@ rhs_kernel(const __grid_constant__ Params<T> P, const T* __restrict__ x, const T
 }
 
 // Launch conditions.  `dir` is passed to the equilibrium in the role of n, so L.G = dir.B.
-template <int EQ, int DISP>
-__global__ void __launch_bounds__(TRACE_BLOCK)
-launch_kernel(const __grid_constant__ Params<double> P, int branch, const double* __restrict__ x0,
-              const double* __restrict__ dir, long long n, double* __restrict__ k0, double* __restrict__ D_out) {
-  const long long i = (long long)blockIdx.x * TRACE_BLOCK + threadIdx.x;
+template <int EQ, int DISP, bool PW>
+__global__ void __launch_bounds__(AUX_BLOCK)
+launch_kernel(const __grid_constant__ Params<double> P0, int branch, const double* __restrict__ x0,
+              const double* __restrict__ dir, const double* __restrict__ omega, double omega_ref, long long n,
+              double* __restrict__ k0, double* __restrict__ D_out) {
+  const long long i = (long long)blockIdx.x * AUX_BLOCK + threadIdx.x;
   if (i >= n) return;
+  const Params<double> P = PW ? params_at_frequency(P0, omega_ref / omega[i]) : P0;
   double x[3], d[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) { x[c] = x0[c * n + i]; d[c] = dir[c * n + i]; }
@@ -293,6 +360,38 @@ launch_kernel(const __grid_constant__ Params<double> P, int branch, const double
     const double v = sn * sn;
     D_out[i] = disp_value<double, DISP>(P, X, Y2, v * c2, v);
   }
+}
+
+// Critical-surface diagnostics (cut-offs and resonances along the ray).
+// Rows of out [10][n]: n_e [m^-3], |B| [T], X = wpe^2/w^2, Y = |Wce|/w, S, Dx, P (Eq. 8-10), R = S + Dx,
+// L = S - Dx, n_par^2 = (n.B)^2/|B|^2.  Cut-offs: P = 0 (X = 1 for electrons only), R = 0, L = 0; resonance: S = 0 (upper
+// hybrid), Y = 1 (cyclotron).  Everything is NaN outside the equilibrium's domain.  inv_alpha_ref = n_e / X at w_ref.
+template <int EQ, bool PW>
+__global__ void __launch_bounds__(AUX_BLOCK)
+diag_kernel(const __grid_constant__ Params<double> P0, double inv_alpha_ref, const double* __restrict__ x,
+            const double* __restrict__ k, const double* __restrict__ omega, double omega_ref, long long n,
+            double* __restrict__ out) {
+  constexpr int DISP = (EQ == EQ_PARABOLIC) ? DISP_O : DISP_FULL;
+  const long long i = (long long)blockIdx.x * AUX_BLOCK + threadIdx.x;
+  if (i >= n) return;
+  const double lam = PW ? omega_ref / omega[i] : 1.0;
+  const Params<double> P = PW ? params_at_frequency(P0, lam) : P0;
+  double xx[3], nn[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { xx[c] = x[c * n + i]; nn[c] = k[c * n + i] * P.k2n; }
+  Local<double> L;
+  GatherDirect gather;
+  L.b2 = 0.0; L.G = 0.0;
+  const bool inside = equilibrium<double, EQ, DISP>(P, xx, nn, L, gather);
+  const double X = L.X, b2 = (EQ == EQ_PARABOLIC) ? 0.0 : L.b2;
+  const double Y2 = P.beta * b2;
+  const StixT<double> st = stix(P, X, Y2);
+  const double Y = sqrt(Y2);
+  const double Dx = X * Y * st.del;
+  const double v[10] = {X * inv_alpha_ref / (lam * lam), sqrt(b2), X, Y, st.s, Dx, st.p, st.s + Dx, st.s - Dx,
+                        (EQ == EQ_PARABOLIC) ? 0.0 : L.G * L.G / b2};
+#pragma unroll
+  for (int r = 0; r < 10; ++r) out[r * n + i] = inside ? v[r] : rt_nan<double>();
 }
 
 // out[0] = max |D|, out[1] = sum |D|, out[2] = #finite, out[3..5] = #status 0/1/2.  out must be zeroed beforehand.

@@ -3,13 +3,16 @@
     python -m paper_2508_15967_b200.sass_count            # table for every trace kernel in librt_b200.so
 
 A ray-step is one pass through the RK4 step region of the kernel (the ``if (status == 0) status = rk4_step(...)`` body:
-the largest reconvergence region of the SASS); for the grid equilibrium the stage loop inside it is rolled and runs 4 times.
+the reconvergence region inside the step loop that holds the most FP-pipe instructions -- the other one is the sample
+store); for the grid equilibrium the stage loop inside it is rolled and runs 4 times.
 Reported per kernel:
 
 * ``instr``     FP-pipe instructions per ray-step (DFMA + DMUL + DADD + DSETP, or the FP32 analogues) -- what the FP64
                 (FP32) pipe has to issue, the quantity the kernels are optimised for;
 * ``executed``  flops as executed, a fused multiply-add counted as 2;
 * ``mufu``      MUFU seeds (reciprocals and reciprocal square roots), ``rsqrt`` of them square roots;
+* ``local``     local-memory (spill) instructions executed per ray-step: must be 0.  ptxas may still report a few bytes
+                of spill for values parked once before the step loop and reloaded after it (the store staging);
 * ``flops``     the ALGORITHMIC flops bench.py uses for ``roofline.achieved``: every division and square root counted as
                 ONE flop.  In fp64 a reciprocal executes 3 FMAs (6 flops) and a reciprocal square root 2 MUL + 3 FMA
                 (8 flops) of Newton refinement after the seed, so flops = executed - 5 rcp - 7 rsqrt; in fp32 the seed
@@ -65,17 +68,29 @@ def count_kernels(lib: Path = LIB) -> dict:
     sass = subprocess.run([exe, "-sass", str(lib)], capture_output=True, text=True, check=True).stdout
     res = {}
     for fn in re.split(r"\n\s*Function : ", sass):
-        m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)E", fn)
+        m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)ELb0E", fn)      # the single-frequency kernels
         if not m:
             continue
         prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
         ins = _parse(fn)
-        region = None                                       # the RK4 step: largest BSSY ... BSYNC region
+        loop = None                                         # the step loop: largest backward branch
         for a, op, rest in ins:
-            if op.startswith("BSSY"):
+            if op.startswith("BRA"):
                 t = _target(rest)
-                if t is not None and (region is None or t - a > region[1] - region[0]):
-                    region = (a, t)
+                if t is not None and t < a and (loop is None or a - t > loop[1] - loop[0]):
+                    loop = (t, a)
+        if loop is None:
+            continue
+        fp_ops = _FP[prec]
+        region, best = None, -1                             # the RK4 step: the BSSY ... BSYNC region inside the loop
+        for a, op, rest in ins:                             # that holds the most FP-pipe instructions
+            if op.startswith("BSSY") and loop[0] <= a < loop[1]:
+                t = _target(rest)
+                if t is None or not (a < t <= loop[1] + 16):
+                    continue
+                nfp = sum(1 for b, o, _ in ins if a <= b < t and o.split(".")[0] in fp_ops)
+                if nfp > best:
+                    region, best = (a, t), nfp
         if region is None:
             continue
         c, rsq = _count(ins, *region)
@@ -95,15 +110,17 @@ def count_kernels(lib: Path = LIB) -> dict:
         executed = 2 * tot[fma] + tot[mul] + tot[add]
         mufu = tot["MUFU"]
         flops = executed - 5 * (mufu - rsq) - 7 * rsq if prec == "d" else executed + mufu
+        local = tot["STL"] + tot["LDL"]                     # spill traffic executed per ray-step (must be 0)
         res[("f64" if prec == "d" else "f32", eq, disp)] = dict(instr=tot[fma] + tot[mul] + tot[add] + tot[setp],
-                                                                executed=executed, mufu=mufu, rsqrt=rsq, flops=flops)
+                                                                executed=executed, mufu=mufu, rsqrt=rsq, flops=flops,
+                                                                local=local)
     return res
 
 
 if __name__ == "__main__":
     names = {0: "parabolic", 1: "linear", 2: "tokamak", 3: "grid", 4: "tokamak_pow"}
     disps = {0: "O", 1: "X", 2: "full"}
-    print(f"{'kernel':34s} {'instr':>6s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s}")
+    print(f"{'kernel':34s} {'instr':>6s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s} {'local':>6s}")
     for (prec, eq, disp), r in sorted(count_kernels().items()):
         print(f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}> {r['instr']:6d} {r['executed']:9d} {r['mufu']:5d} "
-              f"{r['rsqrt']:6d} {r['flops']:6d}")
+              f"{r['rsqrt']:6d} {r['flops']:6d} {r['local']:6d}")
