@@ -52,7 +52,7 @@ FP_INSTR_PER_RAY_STEP = {(1, "f64"): 92, (2, "f64"): 92, (3, "f64"): 234, (4, "f
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None
-NCU_DRAM_BYTES = {}
+NCU_DRAM_BYTES = {(4, "f64"): 5.99e9}     # profiles/r1_cfg4_f64_ncu_c.md: dram__bytes_read.sum + dram__bytes_write.sum
 
 WORKLOAD_NAMES = {
     1: "cfg1: O-mode, parabolic slab, 1024 rays x 1000 steps, full trajectory",
@@ -188,14 +188,16 @@ def run_reference(args) -> int:
 class Job:
     """One config resident on the current device: equilibrium handle, launch states, preallocated outputs."""
 
-    def __init__(self, rt, torch, cfg: int, prec: str, n_rays, rank: int):
+    def __init__(self, rt, torch, cfg: int, prec: str, n_rays, rank: int, scan: bool = False):
         self.rt, self.torch, self.cfg, self.prec = rt, torch, cfg, prec
         seed = 1000 + cfg + 7919 * rank                       # rank r traces its own batch (weak scaling, no exchange)
         self.w = w = inputs.config(cfg, n_rays=n_rays, seed=seed)
         self.eq = rt.create_equilibrium(w.eq)
         dt = torch.float64 if prec == "f64" else torch.float32
         x0 = torch.from_numpy(w.x0).cuda()
-        k0, D0 = rt.launch(self.eq, w.disp, x0, torch.from_numpy(w.dirs).cuda(), w.omega, w.branch)
+        # scan: a frequency scan, one w per ray (rt_launch_w / rt_trace_w); else the config's single frequency
+        self.omega = torch.from_numpy(inputs.frequency_scan(w.n_rays, w.omega, seed)).cuda() if scan else w.omega
+        k0, D0 = rt.launch(self.eq, w.disp, x0, torch.from_numpy(w.dirs).cuda(), self.omega, w.branch)
         if not bool(torch.isfinite(k0).all()):
             raise RuntimeError("rt_launch returned non-finite launch states for a bench workload")
         self.launch_residual = float(D0.abs().max())
@@ -211,7 +213,7 @@ class Job:
 
     def step(self):
         w = self.w
-        return self.rt.trace(self.eq, w.disp, self.x0, self.k0, w.omega, w.n_steps, w.dt, self.stride, traj=self.traj,
+        return self.rt.trace(self.eq, w.disp, self.x0, self.k0, self.omega, w.n_steps, w.dt, self.stride, traj=self.traj,
                              out=self.out)
 
     def host_buffers(self):
@@ -340,13 +342,15 @@ def run_ours(args) -> int:
         del job
         torch.cuda.empty_cache()
         extra = []
-        for c, p in ((2, "f64"), (2, "f32"), (3, "f64"), (4, "f32"), (5, "f64"), (5, "f32")):
-            if (c, p) == (cfg, prec):
+        for c, p, scan in ((2, "f64", False), (2, "f32", False), (3, "f64", False), (4, "f32", False), (5, "f64", False),
+                           (5, "f32", False), (4, "f64", True)):
+            if (c, p) == (cfg, prec) and not scan:
                 continue
-            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 0)
+            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 0, scan=scan)
             _, kms = time_steps(torch, j, 3, 1, flush)
             pk, _ = rt.fma_peak(p, 100.0)
-            extra.append({"workload": f"cfg{c}", "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
+            extra.append({"workload": f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else ""),
+                          "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
                           "roofline_frac": FLOPS_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / (2.0 * pk),
                           "pipe_frac": FP_INSTR_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / pk})
             j.close()

@@ -66,6 +66,7 @@ def _load():
         lib.oracle_trace_w.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, I64, D, I64, P, P, P, P, I32]
         lib.oracle_launch_w.argtypes = [ctypes.POINTER(_CEq), I32, I32, P, P, P, I64, P, P]
         lib.oracle_diagnostics.argtypes = [ctypes.POINTER(_CEq), P, P, P, I64, P]
+        lib.oracle_orbit.argtypes = [ctypes.POINTER(_CEq), P, P, D, I64, I64, D, I64, P, P, P, P, I32]
         lib.oracle_dispersion.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, I64, P, P, P]
         lib.oracle_dispersion_value.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, P]
         lib.oracle_plasma.argtypes = [ctypes.POINTER(_CEq), P, D, I64, P, P, P, P]
@@ -252,4 +253,30 @@ def diagnostics(eq, x, k, omega):
     rc = lib.oracle_diagnostics(ctypes.byref(e.c), x.ctypes.data, k.ctypes.data, w.ctypes.data, n, out.ctypes.data)
     if rc != 0:
         raise ValueError("oracle_diagnostics rejected its arguments")
+    return out
+
+
+def orbit(eq, x0, v0, charge_over_mass, n_steps, dt, save_stride=1, *, traj=False, final=True, drift=True, status=True,
+          n_threads=0) -> dict:
+    """Full-orbit particles (L121, L213): dx/dt = v, dv/dt = (q/m) v x B(x), classical RK4 with step dt [s].
+    x0, v0 [3,n]; returns 'traj' [n_saved,6,n], 'final' [6,n], 'drift' (|v|^2/|v0|^2 - 1; [n_saved,n] with traj else [n])
+    and 'status' [n] for the outputs requested."""
+    lib, e = _load(), _eq(eq)
+    x0, v0 = _soa(x0), _soa(v0)
+    n = x0.shape[1]
+    n_saved = n_steps // save_stride + 1
+    out = {}
+    if traj:
+        out["traj"] = np.empty((n_saved, 6, n))
+    if final:
+        out["final"] = np.empty((6, n))
+    if drift:
+        out["drift"] = np.empty((n_saved, n) if traj else (n,))
+    if status:
+        out["status"] = np.empty((n,), dtype=np.int32)
+    ptr = lambda key: out[key].ctypes.data if key in out else None
+    rc = lib.oracle_orbit(ctypes.byref(e.c), x0.ctypes.data, v0.ctypes.data, float(charge_over_mass), n, int(n_steps),
+                          float(dt), int(save_stride), ptr("traj"), ptr("final"), ptr("drift"), ptr("status"), int(n_threads))
+    if rc != 0:
+        raise ValueError(f"oracle_orbit rejected its arguments (rc={rc})")
     return out

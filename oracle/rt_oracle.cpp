@@ -27,7 +27,10 @@
 // if any of its 4 stage points lies outside the equilibrium's domain (status 1) or if the new state
 // is not finite (status 2).  |D| at a saved state outside the domain is NaN.
 //
-// Parity pins: tests/test_oracle_*.py (P1..P12 in DESIGN.md).  No function here is "parity unpinned".
+// Also here: per-ray frequencies and critical-surface diagnostics and the second ensemble workload,
+// full-orbit charged particles in the same equilibria (oracle_orbit).
+//
+// Parity pins: tests/test_oracle_*.py (P1..P19 in DESIGN.md).  No function here is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
@@ -543,6 +546,77 @@ int oracle_launch_w(const orc_equilibrium* eq, int disp, int branch, const doubl
                     const double* omega, int64_t n, double* k0, double* D_out) {
   if (!omega) return -1;
   return launch_impl(eq, disp, branch, x0, dir, 0.0, omega, n, k0, D_out);
+}
+
+// ---- second ensemble workload of the same shape: full-orbit charged particles in the same equilibrium -------------
+// (L121: "full orbit affects on particle losses in the edge"; L213: "waves or particles in a fusion plasmas ... any
+// physics problem involving a large ensemble of independent problems".)  Newton-Lorentz equations
+//      dx/dt = v ,    dv/dt = (q/m) v x B(x)
+// (no electric field: the equilibria define none), classical RK4 at fixed dt [s], same step-acceptance rule as the rays
+// (reading A12).  out_drift is the relative kinetic-energy drift |v|^2/|v0|^2 - 1 (the orbit's analogue of the rays'
+// |D|: exactly 0 for the differential equation, O(dt^4) for RK4); NaN never occurs (it needs no equilibrium).
+//   x0, v0 [3][n]; out_traj [n_steps/save_stride+1][6][n] rows (x,y,z,vx,vy,vz); out_final [6][n];
+//   out_drift [n_saved][n] if out_traj else [n]; out_status [n].
+int oracle_orbit(const orc_equilibrium* eq, const double* x0, const double* v0, double charge_over_mass, int64_t n,
+                 int64_t n_steps, double dt, int64_t save_stride, double* out_traj, double* out_final, double* out_drift,
+                 int32_t* out_status, int n_threads) {
+  if (!eq || eq->kind < 1 || eq->kind > 3 || n < 0 || n_steps < 0 || save_stride < 1) return -1;   // parabolic slab: no B
+  if (out_traj && (n_steps % save_stride) != 0) return -1;
+  const double qm = charge_over_mass;
+  auto rhs_orbit = [&](const double y[6], double f[6]) -> bool {
+    const Plasma<double> pl = equilibrium<double>(*eq, y);
+    if (!pl.inside) return false;
+    const double* v = y + 3;
+    f[0] = v[0]; f[1] = v[1]; f[2] = v[2];
+    f[3] = qm * (v[1] * pl.B[2] - v[2] * pl.B[1]);
+    f[4] = qm * (v[2] * pl.B[0] - v[0] * pl.B[2]);
+    f[5] = qm * (v[0] * pl.B[1] - v[1] * pl.B[0]);
+    return true;
+  };
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t i = 0; i < n; ++i) {
+    double y[6];
+    for (int c = 0; c < 3; ++c) { y[c] = x0[c * n + i]; y[3 + c] = v0[c * n + i]; }
+    const double e0 = y[3] * y[3] + y[4] * y[4] + y[5] * y[5];
+    auto drift = [&]() { return (y[3] * y[3] + y[4] * y[4] + y[5] * y[5]) / e0 - 1.0; };
+    int status = 0;
+    if (out_traj) {
+      for (int c = 0; c < 6; ++c) out_traj[(0 * 6 + c) * n + i] = y[c];
+      if (out_drift) out_drift[0 * n + i] = drift();
+    }
+    for (int64_t s = 1; s <= n_steps; ++s) {
+      if (status == 0) {
+        double k1[6], k2[6], k3[6], k4[6], ys[6];
+        bool ok = rhs_orbit(y, k1);
+        if (ok) { for (int j = 0; j < 6; ++j) ys[j] = y[j] + 0.5 * dt * k1[j]; ok = rhs_orbit(ys, k2); }
+        if (ok) { for (int j = 0; j < 6; ++j) ys[j] = y[j] + 0.5 * dt * k2[j]; ok = rhs_orbit(ys, k3); }
+        if (ok) { for (int j = 0; j < 6; ++j) ys[j] = y[j] + dt * k3[j]; ok = rhs_orbit(ys, k4); }
+        if (!ok) {
+          status = 1;
+        } else {
+          bool fin = true;
+          for (int j = 0; j < 6; ++j) {
+            ys[j] = y[j] + (dt / 6.0) * (k1[j] + 2.0 * k2[j] + 2.0 * k3[j] + k4[j]);
+            fin = fin && std::isfinite(ys[j]);
+          }
+          if (!fin) status = 2;
+          else for (int j = 0; j < 6; ++j) y[j] = ys[j];
+        }
+      }
+      if (out_traj && (s % save_stride) == 0) {
+        const int64_t m = s / save_stride;
+        for (int c = 0; c < 6; ++c) out_traj[(m * 6 + c) * n + i] = y[c];
+        if (out_drift) out_drift[m * n + i] = drift();
+      }
+    }
+    if (out_final) for (int c = 0; c < 6; ++c) out_final[c * n + i] = y[c];
+    if (!out_traj && out_drift) out_drift[i] = drift();
+    if (out_status) out_status[i] = status;
+  }
+  return 0;
 }
 
 int oracle_max_threads(void) {

@@ -165,6 +165,59 @@ def frequency_scan(n_rays: int, omega0: float, seed: int, spread: float = 0.1) -
     return omega0 * (1.0 + spread * rng.uniform(-1.0, 1.0, n_rays))
 
 
+@dataclass
+class OrbitWorkload:
+    name: str
+    eq: dict
+    charge_over_mass: float     # C/kg
+    x0: np.ndarray              # [3, n] launch positions, m
+    v0: np.ndarray              # [3, n] launch velocities, m/s
+    dt: float                   # s
+    n_steps: int
+    save_stride: int            # 0 = final state only
+    seed: int = 0
+
+    @property
+    def n(self) -> int:
+        return int(self.x0.shape[1])
+
+
+ORBIT_FULL_SIZE = (2**20, 1000)
+
+
+def orbit_config(eq_cfg: int = 4, n: int | None = None, n_steps: int | None = None, seed: int | None = None,
+                 energy_keV: float = 10.0) -> OrbitWorkload:
+    """The second ensemble workload (PAPER.md L121 / L213): deuterons of `energy_keV` on full orbits in
+    the equilibrium of config `eq_cfg` (3: the B0 R0/x slab, 4: analytic tokamak, 5: spline grid).  2^20 particles x
+    1000 steps of dt = 1 ns (about 66 steps per gyration at 2 T), trajectories every 10 steps like config 4.
+    Draw order (``default_rng(2000 + eq_cfg)``), whole arrays: rho, theta_p, phi (positions: rho ~ U[0.1, 0.8] a;
+    slab: x ~ U[1.9, 2.2], y ~ U[-0.2, 0.2], z ~ U[-0.2, 0.2] in the same three draws), then cos(pitch) ~ U[-1, 1] and
+    gyro-angle ~ U[0, 2 pi) (isotropic directions about z^)."""
+    nn, ns = ORBIT_FULL_SIZE
+    n = nn if n is None else int(n)
+    n_steps = ns if n_steps is None else int(n_steps)
+    seed = 2000 + eq_cfg if seed is None else int(seed)
+    rng = np.random.default_rng(seed)
+    a1, a2, a3 = rng.uniform(0.0, 1.0, n), rng.uniform(0.0, 1.0, n), rng.uniform(0.0, 1.0, n)
+    cp = rng.uniform(-1.0, 1.0, n)
+    ga = rng.uniform(0.0, 2.0 * np.pi, n)
+    if eq_cfg == 3:
+        eq = linear_slab(1, 1, 0).eq
+        x0 = np.stack([1.9 + 0.3 * a1, -0.2 + 0.4 * a2, -0.2 + 0.4 * a3])
+    elif eq_cfg in (4, 5):
+        t = TOKAMAK
+        eq = dict(kind="tokamak_circular", **t) if eq_cfg == 4 else synth_grid(1005)
+        rho, thp, phi = (0.1 + 0.7 * a1) * t["a"], 2.0 * np.pi * a2, 2.0 * np.pi * a3
+        R, Z = t["R0"] + rho * np.cos(thp), rho * np.sin(thp)
+        x0 = np.stack([R * np.cos(phi), R * np.sin(phi), Z])
+    else:
+        raise ValueError("orbit workloads exist on the equilibria of configs 3, 4 and 5")
+    speed = np.sqrt(2.0 * energy_keV * 1e3 * Q_E / M_D)
+    sp = np.sqrt(1.0 - cp * cp)
+    v0 = speed * np.stack([sp * np.cos(ga), sp * np.sin(ga), cp])
+    return OrbitWorkload(f"orbits_D_{energy_keV:g}keV_on_cfg{eq_cfg}", eq, Q_E / M_D, x0, v0, 1e-9, n_steps, 10, seed)
+
+
 # (n_rays, n_steps) of BASELINE.json's configs 1..5
 FULL_SIZES = {1: (1024, 1000), 2: (2**20, 2000), 3: (2**18, 3000), 4: (2**20, 1000), 5: (2**24, 500)}
 
