@@ -147,6 +147,25 @@ int rt_launch_w(const rt_equilibrium* eq, int disp, int branch, const double* x0
 int rt_diagnostics(const rt_equilibrium* eq, const double* x, const double* k, double omega, const double* omega_rays,
                    int64_t n, double* out, void* cuda_stream);
 
+/* The second ensemble workload of the same shape ("full orbit affects on particle losses", L213 "waves or
+ * particles in a fusion plasmas ... a large ensemble of independent problems"): full orbits of charged particles in the
+ * equilibrium's magnetic field,
+ *      dx/dt = v ,    dv/dt = (q/m) v x B(x)          (Newton-Lorentz; the equilibria define no electric field)
+ * integrated like the rays: classical RK4 at fixed step, all steps fused in one launch, one thread per particle, same
+ * status rule (a stage point outside the domain freezes the particle: 1; non-finite state: 2) and output layouts.
+ *   x0, v0        DEVICE [3][n]   positions [m], velocities [m/s]; element type per `precision`
+ *   charge_over_mass   q/m [C/kg], signed (relativistic particles: pass q/(gamma m); |v| is constant in a pure B field)
+ *   dt            time step [s]
+ *   out_traj      DEVICE [n_steps/save_stride + 1][6][n], rows (x, y, z, vx, vy, vz); or NULL
+ *   out_final     DEVICE [6][n]; or NULL
+ *   out_drift     DEVICE relative kinetic-energy drift |v|^2/|v0|^2 - 1 (exactly 0 for the differential equation,
+ *                 O(dt^4) for RK4 -- the orbits' analogue of the rays' |D|): [n_saved][n] if out_traj else [n]; or NULL
+ *   out_status    DEVICE int32 [n]; or NULL
+ * RT_ERR_UNSUPPORTED on the parabolic slab (no field). */
+int rt_orbit(const rt_equilibrium* eq, int precision, const void* x0, const void* v0, double charge_over_mass, int64_t n,
+             int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final, void* out_drift,
+             int32_t* out_status, void* cuda_stream);
+
 /* Diagnostic evaluation of the integrand at n points (the quantities one RK4 stage computes):
  *   x, k          DEVICE [3][n]
  *   D_out         DEVICE [n]     signed D(x,k,w); NaN outside the domain; or NULL

@@ -25,7 +25,7 @@ PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
 SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_launch", "rt_launch_w",
-           "rt_diagnostics", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_launch_count", "rt_last_error", "rt_version")
+           "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_launch_count", "rt_last_error", "rt_version")
 NDIAG = 10
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
 
@@ -93,6 +93,7 @@ def load() -> ctypes.CDLL:
         lib.rt_trace_w.argtypes = [P, I32, I32, P, P, P, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_launch_w.argtypes = [P, I32, I32, P, P, P, I64, P, P, P]
         lib.rt_diagnostics.argtypes = [P, P, P, D, P, I64, P, P]
+        lib.rt_orbit.argtypes = [P, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_trace_host.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P]
         lib.rt_launch.argtypes = [P, I32, I32, P, P, D, I64, P, P, P]
         lib.rt_rhs.argtypes = [P, I32, I32, P, P, D, I64, P, P, P, P]
@@ -310,6 +311,36 @@ def diagnostics(eq: Equilibrium, x, k, omega):
     _check(lib.rt_diagnostics(eq.handle, _ptr(x), _ptr(k), 0.0 if w is not None else float(omega), _ptr(w), n, _ptr(out),
                               _stream()))
     return out
+
+
+def orbit(eq: Equilibrium, x0, v0, charge_over_mass: float, n_steps: int, dt: float, save_stride: int = 1, *, traj=False,
+          final=True, drift=True, status=True, out: dict | None = None) -> dict:
+    """``rt_orbit`` on the current CUDA stream: full-orbit particles, x0, v0 CUDA tensors [3, n] (float64 or float32).
+    Returns device tensors 'traj' [n_saved, 6, n], 'final' [6, n], 'drift' ([n_saved, n] with traj else [n]) and
+    'status' [n] int32 for the outputs requested.  Does not synchronise."""
+    import torch
+    lib = load()
+    x0 = _dev_soa(x0, 3)
+    n = x0.shape[1]
+    v0 = _dev_soa(v0, 3, n)
+    if v0.dtype != x0.dtype:
+        raise TypeError("x0 and v0 must have the same dtype")
+    prec = _prec_of(x0)
+    n_saved = n_steps // save_stride + 1 if traj else 0
+    o = {} if out is None else out
+    kw = dict(dtype=x0.dtype, device=x0.device)
+    if traj and "traj" not in o:
+        o["traj"] = torch.empty((n_saved, 6, n), **kw)
+    if final and "final" not in o:
+        o["final"] = torch.empty((6, n), **kw)
+    if drift and "drift" not in o:
+        o["drift"] = torch.empty((n_saved, n) if traj else (n,), **kw)
+    if status and "status" not in o:
+        o["status"] = torch.empty((n,), dtype=torch.int32, device=x0.device)
+    _check(lib.rt_orbit(eq.handle, prec, _ptr(x0), _ptr(v0), float(charge_over_mass), n, int(n_steps), float(dt),
+                        int(save_stride), _ptr(o.get("traj") if traj else None), _ptr(o.get("final") if final else None),
+                        _ptr(o.get("drift") if drift else None), _ptr(o.get("status") if status else None), _stream()))
+    return o
 
 
 def rhs(eq: Equilibrium, disp, x, k, omega: float):

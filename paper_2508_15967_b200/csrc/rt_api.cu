@@ -224,6 +224,37 @@ void free_handle(rt_equilibrium* eq) {
 
 }  // namespace
 
+namespace {
+template <class T>
+int orbit_device(const rt_equilibrium* eq, const void* x0, const void* v0, double qm, long long n, long long n_steps, double dt,
+                 long long save_stride, void* out_traj, void* out_final, void* out_drift, int32_t* out_status, cudaStream_t st) {
+  const rt::Params<T> P = make_params<T>(eq, 1.0);          // B(x) does not depend on a wave frequency
+  rt::OrbitArgs<T> A;
+  A.x0 = static_cast<const T*>(x0);
+  A.v0 = static_cast<const T*>(v0);
+  A.traj = static_cast<T*>(out_traj);
+  A.fin = static_cast<T*>(out_final);
+  A.drift = static_cast<T*>(out_drift);
+  A.status = out_status;
+  A.n = n;
+  A.n_steps = n_steps;
+  A.stride = save_stride;
+  A.h = (T)dt;
+  A.qm = (T)qm;
+#define M(E)                                                                       \
+  if (kernel_kind(eq) == (E) || ((E) == rt::EQ_TOKAMAK && kernel_kind(eq) == rt::EQ_TOKAMAK_POW)) {  \
+    constexpr int block = rt::TraceShape<T, E>::BLOCK;                             \
+    rt::orbit_kernel<T, E><<<grid_for(n, block), block, 0, st>>>(P, A);            \
+    ++g_launches;                                                                  \
+    RT_CUDA(cudaGetLastError());                                                   \
+    return RT_OK;                                                                  \
+  }
+  M(rt::EQ_LINEAR) M(rt::EQ_TOKAMAK) M(rt::EQ_GRID)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no orbit kernel for this equilibrium kind");
+}
+}  // namespace
+
 // ==== C ABI ===========================================================================================================
 extern "C" {
 
@@ -351,6 +382,31 @@ int rt_trace_w(const rt_equilibrium* eq, int disp, int precision, const void* x0
   if (precision == RT_F64)
     return trace_device<double>(eq, disp, x0, k0, 0.0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
   return trace_device<float>(eq, disp, x0, k0, 0.0, omega, n_rays, n_steps, dt, save_stride, out_traj, out_final, out_residual, out_status, st);
+}
+
+int rt_orbit(const rt_equilibrium* eq, int precision, const void* x0, const void* v0, double charge_over_mass, int64_t n,
+             int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final, void* out_drift,
+             int32_t* out_status, void* cuda_stream) {
+  if (!eq) return fail(RT_ERR_INVALID, "equilibrium handle is NULL");
+  if (eq->d.kind == RT_EQ_SLAB_PARABOLIC)
+    return fail(RT_ERR_UNSUPPORTED, "the parabolic slab has no magnetic field: orbits are not defined on it");
+  if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if (!std::isfinite(charge_over_mass)) return fail(RT_ERR_INVALID, "charge_over_mass must be finite");
+  if (n < 0 || n_steps < 0) return fail(RT_ERR_INVALID, "n and n_steps must be >= 0");
+  if (!std::isfinite(dt)) return fail(RT_ERR_INVALID, "dt must be finite");
+  if (save_stride < 1) return fail(RT_ERR_INVALID, "save_stride must be >= 1");
+  if (out_traj && (n_steps % save_stride) != 0)
+    return fail(RT_ERR_INVALID, "n_steps must be a multiple of save_stride when out_traj is given");
+  if (n == 0) return RT_OK;
+  int rc;
+  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(v0, "v0", false)) ||
+      (rc = require_device_ptr(out_traj, "out_traj", true)) || (rc = require_device_ptr(out_final, "out_final", true)) ||
+      (rc = require_device_ptr(out_drift, "out_drift", true)) || (rc = require_device_ptr(out_status, "out_status", true)))
+    return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (precision == RT_F64)
+    return orbit_device<double>(eq, x0, v0, charge_over_mass, n, n_steps, dt, save_stride, out_traj, out_final, out_drift, out_status, st);
+  return orbit_device<float>(eq, x0, v0, charge_over_mass, n, n_steps, dt, save_stride, out_traj, out_final, out_drift, out_status, st);
 }
 
 int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,

@@ -3,6 +3,7 @@
 //   trace_kernel   one thread per ray; loads (x0, k0) once, runs all n_steps classical RK4 steps
 //                  with the state, the stage slopes and every intermediate of D's gradient in registers, and writes
 //                  decimated SoA trajectory samples / the final state / |D| / status (steps a1-a6 of DESIGN.md).
+//   orbit_kernel   the second ensemble workload: full-orbit particles, same structure as trace_kernel.
 //   rhs_kernel     one stage evaluation per point (diagnostics and gradient parity tests).
 //   launch_kernel  launch conditions: closed-form |n| on D = 0 plus Newton polish.
 //   reduce_kernel  max / sum of |D| and status counts (PAPER.md L76 reduction kernels).
@@ -277,6 +278,120 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
     if (A.traj) save(A.traj + m * 6 * A.n_rays, A.res ? A.res + m * A.n_rays : nullptr);
   }
   if (A.fin || (!A.traj && A.res)) save(A.fin, A.traj ? nullptr : A.res);
+  if (A.status && valid) A.status[i] = status;
+}
+
+// ---- second ensemble workload: full-orbit charged particles in the same equilibria -----------------
+// PAPER.md L121 ("full orbit affects on particle losses"), L213 ("waves or particles ... a large ensemble of independent
+// problems").  Newton-Lorentz equations dx/dt = v, dv/dt = (q/m) v x B(x), no electric field; state y = (x, v) in SI.
+// B comes from the same `equilibrium` code as the rays' (its density / gradient parts are dead code here and are
+// eliminated by the compiler); the slab's field is along z, so dv_z/dt = 0 is skipped and v_z stays bit-for-bit constant.
+template <class T, int EQ, class Gather>
+RT_DEV bool orbit_rhs(const Params<T>& P, T qm, const T* y, T* f, Gather& gather) {
+  Local<T> L;
+  const T* v = y + 3;
+  const bool inside = equilibrium<T, EQ, DISP_FULL>(P, y, v, L, gather);
+  f[0] = v[0]; f[1] = v[1]; f[2] = v[2];
+  if (EQ == EQ_LINEAR) {
+    const T w = qm * L.B[2];
+    f[3] = w * v[1]; f[4] = -w * v[0]; f[5] = T(0);
+    return inside;
+  }
+  const T Bx = rt_fma(L.B[0], L.cph, -L.B[1] * L.sph) * qm;
+  const T By = rt_fma(L.B[0], L.sph, L.B[1] * L.cph) * qm;
+  const T Bz = L.B[2] * qm;
+  f[3] = rt_fma(v[1], Bz, -v[2] * By);
+  f[4] = rt_fma(v[2], Bx, -v[0] * Bz);
+  f[5] = rt_fma(v[0], By, -v[1] * Bx);
+  return inside;
+}
+
+// One classical RK4 step of the orbit equations; same acceptance rule and return codes as rk4_step.
+template <class T, int EQ, class Gather>
+RT_DEV int orbit_step(const Params<T>& P, T qm, T h, T* y, Gather& gather) {
+  const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
+  constexpr int NA = (EQ == EQ_LINEAR) ? 5 : 6;          // active components (slab: v_z is constant)
+  T k[6], acc[6], ys[6];
+#pragma unroll
+  for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; ys[j] = y[j]; }
+  bool ok = true;
+#pragma unroll 1
+  for (int st = 0; st < 4; ++st) {
+    const T a = (st == 0) ? T(0) : ((st == 3) ? h : hh);
+    const T w = (st == 0 || st == 3) ? h6 : h3;
+#pragma unroll
+    for (int j = 0; j < NA; ++j) ys[j] = rt_fma(a, k[j], y[j]);
+    ok = orbit_rhs<T, EQ>(P, qm, ys, k, gather) && ok;
+#pragma unroll
+    for (int j = 0; j < NA; ++j) acc[j] = rt_fma(w, k[j], acc[j]);
+  }
+  if (!ok) return 1;
+  bool fin = true;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) fin = fin && rt_finite(acc[j]);
+  if (!fin) return 2;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) y[j] = acc[j];
+  return 0;
+}
+
+template <class T>
+struct OrbitArgs {
+  const T* x0;
+  const T* v0;
+  T* traj;
+  T* fin;
+  T* drift;             // relative kinetic-energy drift |v|^2/|v0|^2 - 1
+  int32_t* status;
+  long long n;
+  long long n_steps;
+  long long stride;
+  T h;                  // time step [s]
+  T qm;                 // charge over mass [C/kg]
+};
+
+template <class T, int EQ>
+__global__ void __maxnreg__((TraceShape<T, EQ>::MAXNREG))
+orbit_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ OrbitArgs<T> A) {
+  constexpr int BLOCK = TraceShape<T, EQ>::BLOCK;
+  const long long N = A.n;
+  const long long i = (long long)blockIdx.x * BLOCK + threadIdx.x;
+  const bool valid = i < N;
+  typename TraceGather<T, EQ>::type gather;
+  if constexpr (EQ == EQ_GRID) {
+    typedef GatherCached<T, BLOCK> GC;
+    __shared__ typename GC::V cache[GC::CHUNKS * BLOCK];
+    gather.col = cache + threadIdx.x;
+    gather.cell = -1; gather.pcell = -1;
+  }
+  __shared__ __align__(16) T stage[7 * BLOCK];
+  T y[6];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    y[c] = valid ? A.x0[c * N + i] : T(0);
+    y[3 + c] = valid ? A.v0[c * N + i] : T(1);
+  }
+  const T inv_e0 = T(1) / rt_fma(y[3], y[3], rt_fma(y[4], y[4], y[5] * y[5]));
+  int status = valid ? 0 : 3;
+  auto save = [&](T* rows6, T* drift_row) {
+    RowStore<T, BLOCK> out;
+    out.lane = threadIdx.x & 31;
+    out.stage = stage + (threadIdx.x & ~31);
+    out.N = A.n;
+    out.i0 = (long long)blockIdx.x * BLOCK + (threadIdx.x & ~31);
+    out.vec = (A.n % RowStore<T, BLOCK>::VEC) == 0;
+    const T e = rt_fma(y[3], y[3], rt_fma(y[4], y[4], y[5] * y[5]));
+    out.store(rows6, drift_row, y, rt_fma(e, inv_e0, T(-1)), out.i0 + out.lane < A.n);
+  };
+  const long long n_outer = A.traj ? A.n_steps / A.stride : 1, n_inner = A.traj ? A.stride : A.n_steps;
+  if (A.traj) save(A.traj, A.drift);
+  for (long long m = 1; m <= n_outer; ++m) {
+#pragma unroll 1
+    for (long long s = 0; s < n_inner; ++s)
+      if (status == 0) status = orbit_step<T, EQ>(P, A.qm, A.h, y, gather);
+    if (A.traj) save(A.traj + m * 6 * A.n, A.drift ? A.drift + m * A.n : nullptr);
+  }
+  if (A.fin || (!A.traj && A.drift)) save(A.fin, A.traj ? nullptr : A.drift);
   if (A.status && valid) A.status[i] = status;
 }
 

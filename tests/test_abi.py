@@ -96,6 +96,33 @@ def test_trace_argument_checks_come_before_cuda(lib):
     eq.close()
 
 
+def test_orbit_and_diagnostics_argument_checks_come_before_cuda(lib):
+    P = ctypes.c_void_p
+    buf = np.zeros((3, 8))
+    slab = binding.create_equilibrium(inputs.config(3, n_rays=4).eq)
+    par = binding.create_equilibrium(inputs.config(1, n_rays=4).eq)
+    call = lambda eq=slab, **kw: lib.rt_orbit(eq.handle if eq else None, kw.get("prec", 0), P(buf.ctypes.data),
+                                              P(buf.ctypes.data), kw.get("qm", 4.8e7), kw.get("n", 8), kw.get("steps", 4),
+                                              1e-9, kw.get("stride", 1), kw.get("traj", None), None, None, None, None)
+    assert call(eq=par) == binding.RT_ERR_UNSUPPORTED and b"parabolic" in lib.rt_last_error()
+    assert call(eq=None) == binding.RT_ERR_INVALID
+    assert call(prec=3) == binding.RT_ERR_INVALID
+    assert call(qm=float("inf")) == binding.RT_ERR_INVALID
+    assert call(n=-2) == binding.RT_ERR_INVALID
+    assert call(stride=0) == binding.RT_ERR_INVALID
+    assert call(steps=5, stride=2, traj=P(buf.ctypes.data)) == binding.RT_ERR_INVALID
+    assert call(n=0) == binding.RT_OK
+    assert call() in (binding.RT_ERR_INVALID, binding.RT_ERR_CUDA)          # host pointers: no CPU fallback
+    assert lib.rt_diagnostics(None, None, None, 1e11, None, 8, None, None) == binding.RT_ERR_INVALID
+    assert lib.rt_diagnostics(slab.handle, None, None, -1.0, None, 8, None, None) == binding.RT_ERR_INVALID
+    assert lib.rt_diagnostics(slab.handle, None, None, 1e11, None, 0, None, None) == binding.RT_OK
+    assert lib.rt_trace_w(slab.handle, 1, 0, None, None, None, 0, 4, 1e-3, 1, None, None, None, None, None) == binding.RT_OK
+    assert lib.rt_trace_w(slab.handle, 7, 0, None, None, None, 8, 4, 1e-3, 1, None, None, None, None, None) == binding.RT_ERR_INVALID
+    assert lib.rt_launch_w(slab.handle, 1, 2, None, None, None, 8, None, None, None) == binding.RT_ERR_INVALID
+    slab.close()
+    par.close()
+
+
 def test_no_cpu_fallback_without_a_device(lib):
     import torch
     if torch.cuda.is_available():

@@ -1,0 +1,159 @@
+"""GPU parity tests (-m gpu) for the second ensemble workload: rt_orbit -- full-orbit
+particles in the equilibria of configs 3, 4, 5 -- against oracle.orbit on the same seeded inputs, through the C ABI.
+
+Tolerances: per-particle 2-norms of x and of v.  Both sides apply the same discrete map (same ODE,
+tableau, dt), so they differ by rounding only: 1e-10 in fp64 like the rays.  In fp32 the velocity rotates through
+Phi = W t ~ 80-100 rad in 1000 steps, and a relative rounding delta of B, dt or q/m (6e-8 each in fp32, about ten of them
+per stage, not all independent from step to step) turns it by Phi * delta: a few 1e-5 each, 1e-4 observed; the bar is 5e-4.
+The energy drift is a difference of O(1) numbers: absolute 64 ulp against the drift formula evaluated at the kernel's own
+states.
+"""
+import numpy as np
+import pytest
+
+from paper_2508_15967_b200 import inputs
+from helpers import rel_err_xk
+from test_gpu_parity import _dev, _host, rt  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+TOL = {"f64": 1e-10, "f32": 5e-4}
+DRIFT_ATOL = {"f64": 64 * 2.2e-16, "f32": 64 * 1.2e-7}
+
+
+def _drift_of(states, v0):
+    return (np.asarray(states, dtype=np.float64)[..., 3:, :] ** 2).sum(-2) / (v0**2).sum(0) - 1.0
+
+
+@pytest.mark.parametrize("eq_cfg,precs", [(3, ("f64", "f32")), (4, ("f64", "f32")), (5, ("f64", "f32"))])
+def test_orbit_trajectory_parity(rt, oracle, eq_cfg, precs):
+    n = 64 * 5 + 37
+    w = inputs.orbit_config(eq_cfg, n=n, n_steps=1000)
+    ref = oracle.orbit(w.eq, w.x0, w.v0, w.charge_over_mass, 1000, w.dt, 100, traj=True)
+    assert (ref["status"] == 0).all()
+    eq = rt.create_equilibrium(w.eq)
+    for prec in precs:
+        out = rt.orbit(eq, _dev(w.x0, prec), _dev(w.v0, prec), w.charge_over_mass, 1000, w.dt, 100, traj=True)
+        tr = _host(out["traj"])
+        assert tr.shape == ref["traj"].shape == (11, 6, n)
+        for m in range(11):
+            ex, ev = rel_err_xk(tr[m], ref["traj"][m])
+            assert ex < TOL[prec] and ev < TOL[prec], (eq_cfg, prec, m, ex, ev)
+        np.testing.assert_array_equal(_host(out["final"]), tr[-1])
+        np.testing.assert_array_equal(tr[0, :3], w.x0 if prec == "f64" else w.x0.astype(np.float32))
+        assert np.array_equal(_host(out["status"]), ref["status"])
+        v0 = w.v0 if prec == "f64" else w.v0.astype(np.float32).astype(np.float64)
+        assert np.abs(_host(out["drift"]) - _drift_of(tr, v0)).max() <= DRIFT_ATOL[prec]
+        assert np.abs(_host(out["drift"]) - ref["drift"]).max() < (1e-11 if prec == "f64" else 1e-3)
+        # final-only mode: drift is [n]
+        fin = rt.orbit(eq, _dev(w.x0, prec), _dev(w.v0, prec), w.charge_over_mass, 1000, w.dt)
+        np.testing.assert_array_equal(_host(fin["final"]), tr[-1])
+        np.testing.assert_array_equal(_host(fin["drift"]), _host(out["drift"])[-1])
+    eq.close()
+
+
+def test_orbit_invariants_on_the_gpu_result(rt, oracle):
+    """Pins P17 / P18 applied to the CUDA path directly: v_z bit-for-bit constant in the slab; the toroidal canonical
+    momentum R v_phi + (q/m) psi (psi in closed form) conserved to integrator order in the tokamak."""
+    w = inputs.orbit_config(3, n=256, n_steps=400)
+    eq = rt.create_equilibrium(w.eq)
+    tr = _host(rt.orbit(eq, _dev(w.x0), _dev(w.v0), w.charge_over_mass, 400, w.dt, 100, traj=True)["traj"])
+    np.testing.assert_array_equal(tr[:, 5], np.broadcast_to(w.v0[2], tr[:, 5].shape))
+    B0R0 = w.eq["B0"] * w.eq["R0"]
+    py = tr[:, 4] + w.charge_over_mass * B0R0 * np.log(tr[:, 0])
+    assert np.abs(py - py[0]).max() / np.abs(w.v0).max() < 1e-7
+    eq.close()
+    w = inputs.orbit_config(4, n=256, n_steps=1000)
+    t = inputs.TOKAMAK
+    eq = rt.create_equilibrium(w.eq)
+    tr = _host(rt.orbit(eq, _dev(w.x0), _dev(w.v0), w.charge_over_mass, 1000, w.dt, 100, traj=True)["traj"])
+    R = np.hypot(tr[:, 0], tr[:, 1])
+    psi = 0.25 * t["B0"] * t["a"] ** 2 * np.log1p(2.0 * ((R - t["R0"]) ** 2 + tr[:, 2] ** 2) / t["a"] ** 2)
+    P = (-tr[:, 1] * tr[:, 3] + tr[:, 0] * tr[:, 4]) + w.charge_over_mass * psi
+    assert np.abs(P - P[0]).max() / (np.abs(w.v0).max() * t["R0"]) < 1e-7
+    eq.close()
+
+
+@pytest.mark.parametrize("eq_cfg", [4, 5])
+def test_particles_leaving_the_domain_freeze_identically(rt, oracle, eq_cfg):
+    w = inputs.orbit_config(eq_cfg, n=128, n_steps=600)
+    t = inputs.TOKAMAK
+    # half of the particles start just inside the domain edge on the outboard midplane (tokamak: rho_max = 0.98, grid:
+    # psi_max at rho = 1) flying outward: a Larmor radius (1.4 cm = 0.023 a) takes them across it and they freeze
+    k = np.arange(0, 128, 2)
+    ph = np.linspace(0.0, 2 * np.pi, len(k), endpoint=False)
+    R = t["R0"] + (0.965 if eq_cfg == 4 else 0.985) * t["a"]
+    speed = np.linalg.norm(w.v0[:, 0])
+    w.x0[:, k] = np.stack([R * np.cos(ph), R * np.sin(ph), np.zeros_like(ph)])
+    w.v0[:, k] = speed * np.stack([np.cos(ph), np.sin(ph), np.zeros_like(ph)])
+    ref = oracle.orbit(w.eq, w.x0, w.v0, w.charge_over_mass, 600, w.dt, 200, traj=True)
+    assert (ref["status"][k] == 1).all() and (ref["status"][1::2] == 0).all()
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.orbit(eq, _dev(w.x0), _dev(w.v0), w.charge_over_mass, 600, w.dt, 200, traj=True)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    ex, ev = rel_err_xk(_host(out["final"]), ref["final"])          # frozen particles stopped on the same step
+    assert ex < 1e-10 and ev < 1e-10, (ex, ev)
+    eq.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [1, 3, 33, 66, 130, 1001])
+def test_orbit_ragged_sizes_and_edges(rt, oracle, n, prec):
+    import torch
+    w = inputs.orbit_config(4, n=n, n_steps=60)
+    ref = oracle.orbit(w.eq, w.x0, w.v0, w.charge_over_mass, 60, w.dt, 30, traj=True)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.orbit(eq, _dev(w.x0, prec), _dev(w.v0, prec), w.charge_over_mass, 60, w.dt, 30, traj=True)
+    for m in range(3):
+        ex, ev = rel_err_xk(_host(out["traj"])[m], ref["traj"][m])
+        assert ex < TOL[prec] and ev < TOL[prec], (m, ex, ev)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    # n_steps = 0 returns the launch state; zero particles is a no-op; a NaN velocity makes the second stage point NaN,
+    # which is "outside the domain" on both sides (reading A12: domain tests are positive conditions): status 1
+    z = rt.orbit(eq, _dev(w.x0, prec), _dev(w.v0, prec), w.charge_over_mass, 0, w.dt, 1, traj=True)
+    np.testing.assert_array_equal(_host(z["final"]), _host(z["traj"])[0])
+    assert (np.abs(_host(z["drift"])) <= 2.4e-7).all()
+    e = torch.empty((3, 0), dtype=torch.float64, device="cuda")
+    assert rt.orbit(eq, e, e.clone(), w.charge_over_mass, 5, w.dt)["final"].shape == (6, 0)
+    v = w.v0.copy()
+    v[1, 0] = np.nan
+    bad = rt.orbit(eq, _dev(w.x0, prec), _dev(v, prec), w.charge_over_mass, 5, w.dt)
+    refb = oracle.orbit(w.eq, w.x0, v, w.charge_over_mass, 5, w.dt)
+    assert refb["status"][0] == 1 and np.array_equal(_host(bad["status"]), refb["status"])
+    with pytest.raises(rt.RtError):
+        rt.orbit(eq, _dev(w.x0, prec), _dev(w.v0, prec), w.charge_over_mass, 7, w.dt, 2, traj=True)
+    eq.close()
+
+
+def test_electron_orbits_turn_the_other_way(rt, oracle):
+    """q/m < 0 and 3670 times larger: electrons at dt = 0.25 ps."""
+    w = inputs.orbit_config(4, n=200, n_steps=400)
+    qm = -inputs.Q_E / inputs.M_E
+    ref = oracle.orbit(w.eq, w.x0, w.v0 * 30.0, qm, 400, 2.5e-13)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.orbit(eq, _dev(w.x0), _dev(w.v0 * 30.0), qm, 400, 2.5e-13)
+    ex, ev = rel_err_xk(_host(out["final"]), ref["final"])
+    assert ex < 1e-10 and ev < 1e-10 and (ref["status"] == 0).all()
+    eq.close()
+
+
+def test_full_size_sampled_orbit_parity(rt, oracle):
+    """The bench's orbit workload at full size (2^20 deuterons x 1000 steps, trajectory every 10 steps): 128 sampled
+    particles one by one against the oracle, the whole ensemble by status and energy drift."""
+    import torch
+    w = inputs.orbit_config(4)
+    assert (w.n, w.n_steps) == inputs.ORBIT_FULL_SIZE
+    idx = np.unique(np.concatenate([np.arange(4), np.arange(w.n - 4, w.n), [63, 64, 65],
+                                    np.random.default_rng(77).integers(0, w.n, 117)]))
+    ref = oracle.orbit(w.eq, w.x0[:, idx], w.v0[:, idx], w.charge_over_mass, w.n_steps, w.dt, w.save_stride, traj=True)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.orbit(eq, _dev(w.x0), _dev(w.v0), w.charge_over_mass, w.n_steps, w.dt, w.save_stride, traj=True)
+    torch.cuda.synchronize()
+    idx_d = torch.from_numpy(idx).cuda()
+    tr = _host(out["traj"][:, :, idx_d])
+    for m in range(0, tr.shape[0], 10):
+        ex, ev = rel_err_xk(tr[m], ref["traj"][m])
+        assert ex < 1e-10 and ev < 1e-10, (m, ex, ev)
+    assert np.array_equal(_host(out["status"][idx_d]), ref["status"])
+    assert int((out["status"] != 0).sum()) == 0
+    assert float(out["drift"].abs().max()) < 5e-4          # steps (W dt)^6/72, W dt up to 0.15 on the inboard side
+    eq.close()
