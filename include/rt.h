@@ -186,6 +186,15 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
  *   sm_clock_mhz  HOST out: average SM clock over the run derived from clock64()/globaltimer; or NULL */
 int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz);
 
+/* The same microbenchmark with its instruction shape and occupancy exposed (evidence for DESIGN.md section 6's
+ * "practical ceiling of the pipe"; rt_fma_peak is shape 0 with 4 blocks per SM).
+ *   shape          0: acc = acc * a + acc (two distinct source registers);  1: acc = acc * a + b (three distinct)
+ *   blocks_per_sm  1..8 blocks of 256 threads per SM, i.e. 2..16 warps per scheduler
+ * Errors: RT_ERR_INVALID for an unknown precision / shape / blocks_per_sm outside [1, 8] / min_ms outside (0, 10000]
+ * / fma_per_s NULL (all checked before the first CUDA call); RT_ERR_CUDA when no device is usable. */
+int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
+                      double* sm_clock_mhz);
+
 /* Number of kernel launches this library has enqueued on the calling process so far (for bench.py's gpu_launches). */
 int64_t rt_launch_count(void);
 

@@ -25,7 +25,7 @@ PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
 SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_launch", "rt_launch_w",
-           "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_launch_count", "rt_last_error", "rt_version")
+           "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_launch_count", "rt_last_error", "rt_version")
 NDIAG = 10
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
 
@@ -99,6 +99,7 @@ def load() -> ctypes.CDLL:
         lib.rt_rhs.argtypes = [P, I32, I32, P, P, D, I64, P, P, P, P]
         lib.rt_reduce.argtypes = [I32, P, P, I64, P, P]
         lib.rt_fma_peak.argtypes = [I32, D, ctypes.POINTER(D), ctypes.POINTER(D)]
+        lib.rt_fma_peak_shape.argtypes = [I32, I32, I32, D, ctypes.POINTER(D), ctypes.POINTER(D)]
         lib.rt_launch_count.restype = I64
         lib.rt_last_error.restype = ctypes.c_char_p
         lib.rt_version.restype = ctypes.c_char_p
@@ -381,3 +382,25 @@ def fma_peak(precision="f64", min_ms: float = 100.0):
     p = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
     _check(lib.rt_fma_peak(p, float(min_ms), ctypes.byref(rate), ctypes.byref(mhz)))
     return rate.value, mhz.value
+
+
+def fma_peak_shape(precision="f64", shape: int = 0, blocks_per_sm: int = 4, min_ms: float = 100.0):
+    """``rt_fma_peak_shape``: the same microbenchmark with its instruction shape (0: acc*a+acc, 1: acc*a+b) and
+    occupancy (256-thread blocks per SM) exposed.  Returns (fused multiply-adds per second, SM clock in MHz)."""
+    lib = load()
+    rate, mhz = ctypes.c_double(), ctypes.c_double()
+    p = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
+    _check(lib.rt_fma_peak_shape(p, int(shape), int(blocks_per_sm), float(min_ms), ctypes.byref(rate), ctypes.byref(mhz)))
+    return rate.value, mhz.value
+
+
+if __name__ == "__main__":      # python -m paper_2508_15967_b200.binding : print the microbenchmark's shape table
+    print("| precision | shape | warps / scheduler | FMA per clock per SM | TFMA/s | SM MHz |\n|---|---|---|---|---|---|")
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    for prec in ("f64", "f32"):
+        for shape in (0, 1):
+            for bps in (1, 2, 4, 8):
+                r, mhz = fma_peak_shape(prec, shape, bps, 100.0)
+                print(f"| {prec} | {'acc*a+acc' if shape == 0 else 'acc*a+b'} | {2 * bps} | {r / (mhz * 1e6) / sms:.1f} | "
+                      f"{r / 1e12:.2f} | {mhz:.0f} |")

@@ -580,13 +580,20 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
 }
 
 int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz) {
+  return rt_fma_peak_shape(precision, 0, 4, min_ms, fma_per_s, sm_clock_mhz);
+}
+
+int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
+                      double* sm_clock_mhz) {
   if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if (shape != 0 && shape != 1) return fail(RT_ERR_INVALID, "shape must be 0 (acc*a+acc) or 1 (acc*a+b)");
+  if (blocks_per_sm < 1 || blocks_per_sm > 8) return fail(RT_ERR_INVALID, "blocks_per_sm must be in [1, 8]");
   if (!fma_per_s) return fail(RT_ERR_INVALID, "fma_per_s is NULL");
   if (!(min_ms > 0.0) || min_ms > 10000.0) return fail(RT_ERR_INVALID, "min_ms must be in (0, 10000]");
   int dev = 0, sms = 0;
   RT_CUDA(cudaGetDevice(&dev));
   RT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const int grid = sms * 4;                                  // 4 x 256 threads per SM: 8 warps per scheduler
+  const int grid = sms * blocks_per_sm;                      // 256-thread blocks: 2 warps per scheduler each
   void* sink = nullptr;
   unsigned long long* clk = nullptr;
   RT_CUDA(cudaMalloc(&sink, (size_t)grid * rt::FMA_BLOCK * 8));
@@ -596,10 +603,14 @@ int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_cloc
   RT_CUDA(cudaEventCreate(&e1));
   auto run = [&](long long iters, float* ms) -> int {
     RT_CUDA(cudaEventRecord(e0, 0));
-    if (precision == RT_F64)
-      rt::fma_peak_kernel<double><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 1e-9, clk);
+    if (precision == RT_F64 && shape == 0)
+      rt::fma_peak_kernel<double, 0><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 1e-9, 1e-3, clk);
+    else if (precision == RT_F64)
+      rt::fma_peak_kernel<double, 1><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 0.999, 1e-3, clk);
+    else if (shape == 0)
+      rt::fma_peak_kernel<float, 0><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1e-7f, 1e-3f, clk);
     else
-      rt::fma_peak_kernel<float><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1e-7f, clk);
+      rt::fma_peak_kernel<float, 1><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 0.999f, 1e-3f, clk);
     ++g_launches;
     RT_CUDA(cudaGetLastError());
     RT_CUDA(cudaEventRecord(e1, 0));

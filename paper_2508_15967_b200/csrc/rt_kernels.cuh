@@ -545,13 +545,14 @@ reduce_kernel(const T* __restrict__ res, const int32_t* __restrict__ status, lon
 }
 
 // Roofline denominator: FMA_CHAINS independent accumulators per thread, each a dependent chain of fused multiply-adds.
-// The chain is acc = acc * a + acc (two distinct source registers): with three distinct 64-bit sources the DFMA rate
-// drops from 63.7 to 58.8 per clock per SM on B200 (register-bank conflicts; measured, profiles/r1_fma_peak_shapes.md).
+// SHAPE 0 (the denominator rt_fma_peak reports): acc = acc * a + acc, two distinct source registers.  SHAPE 1:
+// acc = acc * a + b, three distinct 64-bit sources -- what real code mostly issues; on B200 the DFMA rate then drops
+// from 63.7 to 58.8 per clock per SM (operand-bank conflicts; rt_fma_peak_shape, profiles/r1_fma_peak_shapes.md).
 constexpr int FMA_CHAINS = 16;
 constexpr int FMA_BLOCK = 256;
-template <class T>
+template <class T, int SHAPE>
 __global__ void __launch_bounds__(FMA_BLOCK)
-fma_peak_kernel(T* __restrict__ sink, long long iters, T a, unsigned long long* __restrict__ clk) {
+fma_peak_kernel(T* __restrict__ sink, long long iters, T a, T b, unsigned long long* __restrict__ clk) {
   T acc[FMA_CHAINS];
 #pragma unroll
   for (int j = 0; j < FMA_CHAINS; ++j) acc[j] = T(threadIdx.x + j) * T(1e-3);
@@ -562,7 +563,7 @@ fma_peak_kernel(T* __restrict__ sink, long long iters, T a, unsigned long long* 
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
 #pragma unroll
-      for (int j = 0; j < FMA_CHAINS; ++j) acc[j] = acc[j] * a + acc[j];
+      for (int j = 0; j < FMA_CHAINS; ++j) acc[j] = (SHAPE == 0) ? rt_fma(acc[j], a, acc[j]) : rt_fma(acc[j], a, b);
     }
   }
   const long long c1 = clock64();

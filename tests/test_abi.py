@@ -136,6 +136,9 @@ def test_no_cpu_fallback_without_a_device(lib):
     assert rc == binding.RT_ERR_CUDA
     rate = ctypes.c_double()
     assert lib.rt_fma_peak(0, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
+    assert lib.rt_fma_peak_shape(0, 1, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
+    assert lib.rt_fma_peak_shape(0, 2, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
+    assert lib.rt_fma_peak_shape(0, 0, 9, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
     with pytest.raises(binding.RtError):
         binding.create_equilibrium(inputs.synth_grid(seed=3, nR=9, nZ=9, nPsi=9))   # grid tables live on the device
     eq.close()
