@@ -45,10 +45,10 @@ UNIT = "ray-steps/s"
 # (its Newton refinement is NOT counted).  FP_INSTR_PER_RAY_STEP is what the FP64 / FP32 pipe actually issues per
 # ray-step (FMA, MUL, ADD, SETP instructions, refinements included).  Both tables are counted from the compiled kernels by
 # paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
-FLOPS_PER_RAY_STEP = {(1, "f64"): 132, (2, "f64"): 132, (3, "f64"): 276, (4, "f64"): 822, (5, "f64"): 1276,
-                      (1, "f32"): 132, (2, "f32"): 132, (3, "f32"): 279, (4, "f32"): 820, (5, "f32"): 1272}
-FP_INSTR_PER_RAY_STEP = {(1, "f64"): 92, (2, "f64"): 92, (3, "f64"): 234, (4, "f64"): 664, (5, "f64"): 904,
-                         (1, "f32"): 86, (2, "f32"): 86, (3, "f32"): 195, (4, "f32"): 568, (5, "f32"): 838}
+FLOPS_PER_RAY_STEP = {(1, "f64"): 132, (2, "f64"): 132, (3, "f64"): 264, (4, "f64"): 803, (5, "f64"): 1268,
+                      (1, "f32"): 132, (2, "f32"): 132, (3, "f32"): 267, (4, "f32"): 807, (5, "f32"): 1268}
+FP_INSTR_PER_RAY_STEP = {(1, "f64"): 92, (2, "f64"): 92, (3, "f64"): 218, (4, "f64"): 633, (5, "f64"): 896,
+                         (1, "f32"): 86, (2, "f32"): 86, (3, "f32"): 183, (4, "f32"): 547, (5, "f32"): 834}
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None

@@ -69,7 +69,7 @@ typedef struct rt_equilibrium_desc {
   int32_t nR, nZ, nPsi;               /* GRID_RZ: node counts (each >= 4) */
   double n_ref, L;                    /* n_ref [m^-3]: reference density of the three analytic kinds; L [m] */
   double x_foot, L_ramp, B0, R0;      /* [m], [m], [T], [m] */
-  double a, q0, q1, p_exp, rho_max;   /* minor radius [m]; q = q0 + q1 rho^2; rho_max <= 0 means 0.98 */
+  double a, q0, q1, p_exp, rho_max;   /* minor radius [m], 0 < a < R0; q = q0 + q1 rho^2; rho_max <= 0 means 0.98 */
   double Rmin, Rmax, Zmin, Zmax;      /* GRID_RZ: uniform node coordinates R_i = Rmin + i (Rmax-Rmin)/(nR-1) */
   double psi_min, psi_max;            /* GRID_RZ: uniform psi nodes of the two 1-D profiles */
   const double* psi_RZ;               /* HOST [nR][nZ] nodal psi, row-major (Z fastest) [T m^2] */

@@ -286,6 +286,7 @@ int rt_create_equilibrium(const rt_equilibrium_desc* desc, rt_equilibrium** out)
       if (bad(d.q0) || bad(d.q1) || !(d.q0 > 0.0) || d.q1 < 0.0) return fail(RT_ERR_INVALID, "tokamak: need q0 > 0, q1 >= 0");
       if (bad(d.p_exp) || d.p_exp < 1.0) return fail(RT_ERR_INVALID, "tokamak: p_exp must be >= 1");
       if (bad(d.rho_max) || d.rho_max >= 1.0) return fail(RT_ERR_INVALID, "tokamak: rho_max must be < 1");
+      if (!(d.a < d.R0)) return fail(RT_ERR_INVALID, "tokamak: need a < R0 (the domain rho < rho_max must exclude R = 0)");
       break;
     default:
       if (d.nR < 4 || d.nZ < 4 || d.nPsi < 4) return fail(RT_ERR_INVALID, "grid: nR, nZ, nPsi must each be >= 4");

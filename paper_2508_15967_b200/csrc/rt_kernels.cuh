@@ -31,7 +31,7 @@ namespace rt {
 constexpr int AUX_BLOCK = 128;
 template <class T, int EQ> struct TraceTune { static constexpr int BLOCK = 64, MAXNREG = 72; };
 template <int EQ> struct TraceTune<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
-template <> struct TraceTune<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 96; };
+template <> struct TraceTune<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 104; };
 #ifdef RT_TRACE_BLOCK       // experiments: one shape for every trace kernel
 template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = RT_TRACE_BLOCK, MAXNREG = RT_MAXNREG; };
 #else
@@ -182,6 +182,8 @@ RT_DEV Params<T> params_at_frequency(const Params<T>& P, double lam) {
   const double l2 = lam * lam;
   Q.xs = T(P.xs * l2); Q.beta = T(P.beta * l2); Q.beta2 = T(P.beta2 * l2);
   Q.par_g = T(P.par_g * l2); Q.lin_gx = T(P.lin_gx * l2); Q.two_xs_a2 = T(P.two_xs_a2 * l2);
+  Q.xsh = T(P.xsh * l2); Q.lin_gxh = T(P.lin_gxh * l2); Q.tok_gxh = T(P.tok_gxh * l2);
+  Q.sB0 = T(P.sB0 * lam); Q.sB0R0 = T(P.sB0R0 * lam);
   Q.k2n = T(P.k2n * lam); Q.n2k = T(P.n2k / lam);
   return Q;
 }

@@ -16,8 +16,8 @@
 //
 // The hot path never forms D's gradient vectors and divides them by W component by component.  With r = 1/s, G = n.B:
 //      dx/dtau = A n + C B ,                         A = D_v r,            C = (G/|B|^2) D_u r
-//      dn/dtau = Ax grad X + Ab (grad |B|^2)/2 - C grad_x(n.B)|_n ,
-//                                                    Ax = -D_X r/2,        Ab = -(beta D_Y2 - u D_u/|B|^2) r
+//      dn/dtau = Ax (grad X)/2 + Ab (grad |B|^2)/2 - C grad_x(n.B)|_n ,
+//                                                    Ax = -D_X r,          Ab = -(beta D_Y2 - u D_u/|B|^2) r
 // so the reciprocal is folded into four scalars (disp_coefs) before anything multiplies a vector, and every structural
 // zero of an equilibrium (slab: only d/dx; axisymmetric: no d/dphi of X and |B|^2) is skipped at compile time -- the
 // FP64 pipe is the roofline of this path, so the instruction count per stage is what is optimised.
@@ -43,6 +43,7 @@ enum { DISP_O = 0, DISP_X = 1, DISP_FULL = 2 };
 template <class T>
 struct Params {
   T xs;         // X = xs * shape(x):  alpha n_ref (analytic kinds) or alpha ne_scale (grid), alpha = e^2/(eps0 m_e w^2)
+  T xsh;        // xs / 2 (the hot loop carries HALF the gradient of X, see Local::hgX)
   T beta;       // Y_e^2 = beta |B|^2, beta = (e/(m_e w))^2
   T beta2;      // 2 beta
   T mu;         // Z m_e / m_i; 0 = electrons only
@@ -52,9 +53,14 @@ struct Params {
   T par_g;      // xs / L^2
   // slab_linear_br:  X = (x - x_foot) lin_gx
   T x_foot, lin_gx, B0R0;   // lin_gx = -xs / L_ramp
+  T lin_gxh;                // lin_gx / 2
+  // analytic fields in units of the electron cyclotron ratio: sB0 = sqrt(beta) B0, sB0R0 = sqrt(beta) B0 R0, so that
+  // |B'|^2 IS Y2 = (Wce/w)^2 and no beta multiplies anything in the hot loop (ray_rhs, SCALED)
+  T sB0, sB0R0;
   // tokamak_circular
   T R0, B0, inv_a2, q0, q1_a2, two_q1_a2, p_exp, rmax2;   // q = q0 + q1_a2 r^2;  domain r^2 < rmax2 = (rho_max a)^2
   T two_xs_a2;  // 2 xs / a^2
+  T tok_gxh;    // -p_exp xs / a^2:  (1/2) grad X = tok_gxh (1 - rho^2)^(p_exp - 1) (dR, 0, Z)
   // grid_rz
   T Rmin, Rmax, Zmin, Zmax, hR, hZ, inv_hR, inv_hZ, psi_min, psi_max, hP, inv_hP;
   int nRc, nZc, nPc;            // cell counts
@@ -106,9 +112,35 @@ RT_DEV float rt_rsqrt(float x) {
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
+// sqrt(x) from the same seed without forming 1/sqrt(x) first: g = x y, e = 1 - g y, sqrt = g (1 + e/2 + 3 e^2/8)
+// (2 MUL + 3 FMA; one instruction fewer than x * rt_rsqrt(x)).
+RT_DEV double rt_sqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double g = x * y;
+  const double e = fma(-g, y, 1.0);
+  return fma(g * e, fma(0.375, e, 0.5), g);
+}
+RT_DEV float rt_sqrt_fast(float x) { return x * rt_rsqrt(x); }
+// Domain tests of the fp64 hot loop as INTEGER comparisons of the bit patterns (a DSETP occupies the FP64 pipe, which is
+// the roofline of this path; the ALU pipe is idle).  Exactly equivalent to the floating-point comparisons they replace:
+//   rt_less_nonneg(a, b), a >= +0 or NaN, b > 0 finite:  a < b  <=>  bits(a) < bits(b) as unsigned (a NaN of either sign
+//   has a larger pattern than any finite positive number);
+//   rt_positive(a):  a > 0  <=>  0 < bits(a) <= bits(+inf)  <=>  (unsigned)(bits(a) - 1) < bits(+inf).
+RT_DEV bool rt_less_nonneg(double a, double b) {
+  return (unsigned long long)__double_as_longlong(a) < (unsigned long long)__double_as_longlong(b);
+}
+RT_DEV bool rt_less_nonneg(float a, float b) { return a < b; }
+RT_DEV bool rt_positive(double a) {
+  return (unsigned long long)(__double_as_longlong(a) - 1LL) < 0x7ff0000000000000ULL;
+}
+RT_DEV bool rt_positive(float a) { return a > 0.0f; }
 #else
 template <class T> RT_DEV T rt_rcp(T x) { return T(1) / x; }
 template <class T> RT_DEV T rt_rsqrt(T x) { return T(1) / rt_sqrt(x); }
+template <class T> RT_DEV T rt_sqrt_fast(T x) { return rt_sqrt(x); }
+template <class T> RT_DEV bool rt_less_nonneg(T a, T b) { return a < b; }
+template <class T> RT_DEV bool rt_positive(T a) { return a > T(0); }
 #endif
 
 #ifdef __CUDACC__
@@ -229,9 +261,11 @@ RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2
 template <class T>
 struct Coef { T A, C, Ax, Ab; };
 
-template <class T, int DISP>
+// SC: the caller's field is already in units of sqrt(beta) (Params::sB0), i.e. b2 IS Y2 and Ab multiplies (1/2) grad Y2.
+// Ax multiplies HALF the gradient of X (Local::hgX), which is where the 1/2 of the header comment has gone.
+template <class T, int DISP, bool SC>
 RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
-  const T Y2 = P.beta * b2, Y22 = P.beta2 * b2;
+  const T Y2 = SC ? b2 : P.beta * b2, Y22 = SC ? b2 + b2 : P.beta2 * b2;
   const T e1 = rt_rcp(T(1) - Y2);
   const T e2 = rt_rcp(rt_fma(-P.mu2, Y2, T(1)));
   const T e1s = e1 * e1, e2s = e2 * e2;
@@ -254,8 +288,8 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
     const T r = rt_rcp(s);
     c.A = S * r;
     c.C = T(0);
-    c.Ax = DXn * (T(0.5) * r);
-    c.Ab = (P.beta * r) * DYn;
+    c.Ax = DXn * r;
+    c.Ab = SC ? r * DYn : (P.beta * r) * DYn;
   } else {
     const T d2 = (T(0.5) * Xd) * XdY22;
     const T Pp = rt_fma(-X, P.one_plus_mu, T(1));
@@ -275,8 +309,8 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
     const T r = rt_rcp(s);
     c.A = Dv * r;
     c.C = Bc * (Du * r);
-    c.Ax = DXn * (T(0.5) * r);
-    c.Ab = rt_fma(Bc, c.C, (P.beta * r) * DYn);
+    c.Ax = DXn * r;
+    c.Ab = SC ? rt_fma(Bc, c.C, r * DYn) : rt_fma(Bc, c.C, (P.beta * r) * DYn);
   }
   return c;
 }
@@ -284,10 +318,13 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
 // ---- equilibrium at one stage point, in a local orthonormal frame ------------------------------------------------
 // Frame: (e1, e2, e3) = (R^, phi^, Z^) for the axisymmetric kinds, Cartesian for the slabs.  Only the entries an
 // equilibrium can make non-zero are written (and read): slabs vary along e1 = x only; axisymmetric X and |B|^2 have no
-// e2 = phi derivative.  gG = grad_x (n.B) at fixed Cartesian n, hgb2 = (1/2) grad |B|^2.
+// e2 = phi derivative.  gG = grad_x (n.B) at fixed Cartesian n, hgb2 = (1/2) grad |B|^2, hgX = (1/2) grad X.
+// SC (analytic kinds only): B is returned in units of 1/sqrt(beta), i.e. B' = sqrt(beta) B with |B'|^2 = Y2; the ray
+// right-hand side is invariant under this scaling once beta is dropped from disp_coefs (C' B' = C B, C' grad(n.B') =
+// C grad(n.B), Ab' grad Y2 = Ab grad |B|^2), and it removes three multiplications per stage.
 template <class T>
 struct Local {
-  T X, gX[3];
+  T X, hgX[3];   // X and HALF its gradient
   T B[3], b2, hgb2[3], G, gG[3];
   T nl[3];       // n in the local frame
   T cph, sph;    // axisymmetric kinds: e1 = (cph, sph, 0), e2 = (-sph, cph, 0)
@@ -325,7 +362,7 @@ RT_DEV void axisym_field(T iR, T psiR, T psiZ, T psiRRh, T psiRZ, T psiZZh, T F,
   }
 }
 
-template <class T, int EQ, int DISP, class Gather>
+template <class T, int EQ, int DISP, bool SC = false, class Gather>
 RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L, Gather& gather) {
   if (EQ == EQ_PARABOLIC) {
     // X = xs (1 + (x^2+y^2)/L^2)                                          (BASELINE.json config 1)
@@ -334,11 +371,11 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
   }
   if (EQ == EQ_LINEAR) {
     // n_e = n_ref (x_foot - x)/L_ramp ;  B = (B0 R0 / x) z^                (config 3; Eq. 4 profile)
-    const bool inside = x[0] > T(0);
+    const bool inside = rt_positive(x[0]);
     L.X = (x[0] - P.x_foot) * P.lin_gx;                                    // grad X = (lin_gx, 0, 0)
     if (DISP != DISP_O) {
       const T ix = rt_rcp(x[0]);
-      const T Bz = P.B0R0 * ix;
+      const T Bz = (SC ? P.sB0R0 : P.B0R0) * ix;
       L.B[2] = Bz;
       L.b2 = Bz * Bz;
       L.hgb2[0] = -L.b2 * ix;
@@ -364,25 +401,26 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
     // psi'(r) = B0 r / q, q = q0 + q1 rho^2, F = B0 R0, n_e = n_ref (1 - rho^2)^p       (config 4; reading A9)
     const T dR = R - P.R0;
     const T r2 = rt_fma(dR, dR, Z * Z);
-    const bool inside = (R > T(0)) && (r2 < P.rmax2);
+    // r^2 < (rho_max a)^2 implies R > 0 because rt_create_equilibrium requires a < R0 and rho_max < 1
+    const bool inside = rt_less_nonneg(r2, P.rmax2);
     const T t = rt_fma(-P.inv_a2, r2, T(1));                               // 1 - rho^2
-    T gx;                                                                  // grad X = gx (dR, 0, Z)
+    T gx;                                                                  // (1/2) grad X = gx (dR, 0, Z)
     if (EQ == EQ_TOKAMAK) {
-      const T sq = t * rt_rsqrt(t);
+      const T sq = rt_sqrt_fast(t);
       L.X = (P.xs * sq) * t;
-      gx = (T(-1.5) * P.two_xs_a2) * sq;
+      gx = P.tok_gxh * sq;
     } else {
       const T pw = rt_pow(t, P.p_exp - T(1));
       L.X = (P.xs * pw) * t;
-      gx = (-P.p_exp * P.two_xs_a2) * pw;
+      gx = P.tok_gxh * pw;
     }
-    L.gX[0] = gx * dR; L.gX[2] = gx * Z;
+    L.hgX[0] = gx * dR; L.hgX[2] = gx * Z;
     if (DISP != DISP_O) {
       // B = (-h Z, g, h dR), h = B0/(q R), g = B0 R0/R; with e = 1/R + c dR, c = q'/q = 2 q1/(a^2 q):
       //   h_R = -h e, h_Z = -h c Z, g_R = -g/R.
       const T iq = rt_rcp(rt_fma(P.q1_a2, r2, P.q0));
-      const T h = (P.B0 * iq) * iR;
-      const T g = P.B0R0 * iR;
+      const T h = ((SC ? P.sB0 : P.B0) * iq) * iR;
+      const T g = (SC ? P.sB0R0 : P.B0R0) * iR;
       const T c = P.two_q1_a2 * iq;
       const T e = rt_fma(c, dR, iR);
       const T h2 = h * h, g2 = g * g;
@@ -438,8 +476,8 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
   gather.prof_row(P, iP, 1, g);
   cubic01(g, ds, Ne, Nep);
   L.X = P.xs * Ne;
-  const T gx = P.xs * Nep;
-  L.gX[0] = gx * psiR; L.gX[2] = gx * psiZ;
+  const T gx = P.xsh * Nep;
+  L.hgX[0] = gx * psiR; L.hgX[2] = gx * psiZ;
   if (DISP != DISP_O) {
     T f[4], F, Fp;
     gather.prof_row(P, iP, 0, f);
@@ -455,7 +493,8 @@ template <class T, int EQ, int DISP, class Gather>
 RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, Gather& gather) {
   Local<T> L;
   const T* n = y + 3;
-  const bool inside = equilibrium<T, EQ, DISP>(P, y, n, L, gather);
+  constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
+  const bool inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
   if (DISP == DISP_O) {
     // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)   =>   dx/dtau = n r, dn/dtau = -grad X r/2, r = 1/(v+X)
@@ -465,18 +504,17 @@ RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, Gather& gather) {
       const T c = -P.par_g * r;
       f[3] = c * y[0]; f[4] = c * y[1]; f[5] = T(0);
     } else if (EQ == EQ_LINEAR) {
-      f[3] = (T(-0.5) * P.lin_gx) * r; f[4] = T(0); f[5] = T(0);
+      f[3] = -P.lin_gxh * r; f[4] = T(0); f[5] = T(0);
     } else {
-      const T hr = T(-0.5) * r;
-      const T fR = hr * L.gX[0];
-      f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = hr * L.gX[2];
+      const T fR = -r * L.hgX[0];
+      f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = -r * L.hgX[2];
     }
     return inside;
   }
-  const Coef<T> c = disp_coefs<T, DISP>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
+  const Coef<T> c = disp_coefs<T, DISP, SC>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
   f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
   if (EQ == EQ_LINEAR) {
-    T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gx);
+    T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gxh);
     if (DISP == DISP_FULL) {
       f[2] = rt_fma(c.C, L.B[2], f[2]);
       fn = rt_fma(-c.C, L.gG[0], fn);
@@ -485,8 +523,8 @@ RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, Gather& gather) {
     return inside;
   }
   // axisymmetric kinds: assemble in (R^, phi^, Z^), rotate to Cartesian
-  T fR = rt_fma(c.Ab, L.hgb2[0], c.Ax * L.gX[0]);
-  T fZ = rt_fma(c.Ab, L.hgb2[2], c.Ax * L.gX[2]);
+  T fR = rt_fma(c.Ab, L.hgb2[0], c.Ax * L.hgX[0]);
+  T fZ = rt_fma(c.Ab, L.hgb2[2], c.Ax * L.hgX[2]);
   if (DISP == DISP_FULL) {
     const T xR = c.C * L.B[0], xP = c.C * L.B[1];
     f[0] = rt_fma(xR, L.cph, rt_fma(-xP, L.sph, f[0]));

@@ -27,6 +27,7 @@ Params<T> fold_params(const rt_equilibrium_desc& d, double rho_max, double ne_sc
   const double nscale = (d.kind == RT_EQ_GRID_RZ) ? ne_scale : d.n_ref;
   const double xs = alpha * nscale;
   P.xs = (T)xs;
+  P.xsh = (T)(0.5 * xs);
   const double wce_per_T = kQe / (kMe * omega);
   P.beta = (T)(wce_per_T * wce_per_T);
   P.beta2 = (T)(2.0 * wce_per_T * wce_per_T);
@@ -38,7 +39,10 @@ Params<T> fold_params(const rt_equilibrium_desc& d, double rho_max, double ne_sc
   P.par_g = (T)(d.L != 0.0 ? xs / (d.L * d.L) : 0.0);
   P.x_foot = (T)d.x_foot;
   P.lin_gx = (T)(d.L_ramp != 0.0 ? -xs / d.L_ramp : 0.0);
+  P.lin_gxh = (T)(d.L_ramp != 0.0 ? -0.5 * xs / d.L_ramp : 0.0);
   P.B0R0 = (T)(d.B0 * d.R0);
+  P.sB0 = (T)(wce_per_T * d.B0);                 // sqrt(beta) B0: the field in units of the electron cyclotron ratio
+  P.sB0R0 = (T)(wce_per_T * d.B0 * d.R0);
   P.R0 = (T)d.R0;
   P.B0 = (T)d.B0;
   const double inv_a2 = d.a != 0.0 ? 1.0 / (d.a * d.a) : 0.0;
@@ -48,6 +52,7 @@ Params<T> fold_params(const rt_equilibrium_desc& d, double rho_max, double ne_sc
   P.two_q1_a2 = (T)(2.0 * d.q1 * inv_a2);
   P.p_exp = (T)d.p_exp;
   P.two_xs_a2 = (T)(2.0 * xs * inv_a2);
+  P.tok_gxh = (T)(-d.p_exp * xs * inv_a2);
   P.rmax2 = (T)(rho_max * rho_max * d.a * d.a);
   if (d.kind == RT_EQ_GRID_RZ) {
     const double hR = (d.Rmax - d.Rmin) / (d.nR - 1), hZ = (d.Zmax - d.Zmin) / (d.nZ - 1);
