@@ -45,10 +45,10 @@ UNIT = "ray-steps/s"
 # (its Newton refinement is NOT counted).  FP_INSTR_PER_RAY_STEP is what the FP64 / FP32 pipe actually issues per
 # ray-step (FMA, MUL, ADD, SETP instructions, refinements included).  Both tables are counted from the compiled kernels by
 # paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
-FLOPS_PER_RAY_STEP = {(1, "f64"): 132, (2, "f64"): 132, (3, "f64"): 264, (4, "f64"): 803, (5, "f64"): 1268,
-                      (1, "f32"): 132, (2, "f32"): 132, (3, "f32"): 267, (4, "f32"): 807, (5, "f32"): 1268}
-FP_INSTR_PER_RAY_STEP = {(1, "f64"): 92, (2, "f64"): 92, (3, "f64"): 218, (4, "f64"): 633, (5, "f64"): 896,
-                         (1, "f32"): 86, (2, "f32"): 86, (3, "f32"): 183, (4, "f32"): 547, (5, "f32"): 834}
+FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 259, (4, "f64"): 794, (5, "f64"): 1260,
+                      (1, "f32"): 115, (2, "f32"): 115, (3, "f32"): 262, (4, "f32"): 798, (5, "f32"): 1257}
+FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f64"): 624, (5, "f64"): 888,
+                         (1, "f32"): 69, (2, "f32"): 69, (3, "f32"): 178, (4, "f32"): 538, (5, "f32"): 823}
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None

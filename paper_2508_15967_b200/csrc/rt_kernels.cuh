@@ -31,7 +31,7 @@ namespace rt {
 constexpr int AUX_BLOCK = 128;
 template <class T, int EQ> struct TraceTune { static constexpr int BLOCK = 64, MAXNREG = 72; };
 template <int EQ> struct TraceTune<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
-template <> struct TraceTune<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 104; };
+template <> struct TraceTune<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 112; };
 #ifdef RT_TRACE_BLOCK       // experiments: one shape for every trace kernel
 template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = RT_TRACE_BLOCK, MAXNREG = RT_MAXNREG; };
 #else
@@ -69,41 +69,46 @@ RT_DEV constexpr bool rhs_component_active(int j) {
 template <class T, int EQ, int DISP, class Gather>
 RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
-  T k[6], acc[6], ys[6];
+  T k[6], acc[6], ys[6], r;          // the slope of a stage is r k (ray_rhs): r is folded into the step-size factors
   bool ok = true;
   if (EQ == EQ_GRID && RT_GRID_ROLLED) {
 #pragma unroll
     for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; }
+    T ar = T(0);                     // a_st r_{st-1}
 #pragma unroll 1
     for (int st = 0; st < 4; ++st) {
-      const T a = (st == 0) ? T(0) : ((st == 3) ? h : hh);
-      const T w = (st == 0 || st == 3) ? h6 : h3;
 #pragma unroll
-      for (int j = 0; j < 6; ++j) ys[j] = rt_fma(a, k[j], y[j]);
-      ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+      for (int j = 0; j < 6; ++j) ys[j] = rt_fma(ar, k[j], y[j]);
+      ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+      const T wr = ((st == 0 || st == 3) ? h6 : h3) * r;
+      ar = ((st == 2) ? h : hh) * r;
 #pragma unroll
-      for (int j = 0; j < 6; ++j) acc[j] = rt_fma(w, k[j], acc[j]);
+      for (int j = 0; j < 6; ++j) acc[j] = rt_fma(wr, k[j], acc[j]);
     }
 #pragma unroll
     for (int j = 0; j < 6; ++j) ys[j] = acc[j];
   } else {
 #pragma unroll
     for (int j = 0; j < 6; ++j) { ys[j] = y[j]; acc[j] = y[j]; }
-    ok = ray_rhs<T, EQ, DISP>(P, y, k, gather);
+    ok = ray_rhs<T, EQ, DISP>(P, y, k, r, gather);
+    T wr = h6 * r, ar = hh * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
-      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(h6, k[j], y[j]); ys[j] = rt_fma(hh, k[j], y[j]); }
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], y[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
+    ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+    wr = h3 * r; ar = hh * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
-      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(h3, k[j], acc[j]); ys[j] = rt_fma(hh, k[j], y[j]); }
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], acc[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
+    ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+    wr = h3 * r; ar = h * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
-      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(h3, k[j], acc[j]); ys[j] = rt_fma(h, k[j], y[j]); }
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k, gather) && ok;
+      if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], acc[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
+    ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+    wr = h6 * r;
 #pragma unroll
-    for (int j = 0; j < 6; ++j) ys[j] = rhs_component_active<EQ>(j) ? rt_fma(h6, k[j], acc[j]) : y[j];
+    for (int j = 0; j < 6; ++j) ys[j] = rhs_component_active<EQ>(j) ? rt_fma(wr, k[j], acc[j]) : y[j];
   }
   if (!ok) return 1;
   bool fin = true;
@@ -407,7 +412,7 @@ rhs_kernel(const __grid_constant__ Params<T> P, const T* __restrict__ x, const T
 #pragma unroll
   for (int c = 0; c < 3; ++c) { y[c] = x[c * n + i]; y[3 + c] = k[c * n + i] * P.k2n; }
   GatherDirect gather;
-  const bool inside = ray_rhs<T, EQ, DISP>(P, y, f, gather);
+  const bool inside = ray_rhs_scaled<T, EQ, DISP>(P, y, f, gather);
   if (rhs_out) {
 #pragma unroll
     for (int c = 0; c < 6; ++c) rhs_out[c * n + i] = inside ? f[c] : T(0);

@@ -258,8 +258,10 @@ RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2
 //   D_u = -b w - pw b - D_w.
 // With S_X = -sig, P_X = -(1+mu), (Dx^2)_X = q1 = 2 X Y2 del^2, S_Y2 = -X sig', (Dx^2)_Y2 = q2 = X^2 del (del + 2 Y2 del'):
 //   -D_X = DXn = sig D_S + (1+mu) D_P + q1 pw ,     -D_Y2 = DYn = X sig' D_S + q2 pw.
+// The coefficients are returned WITHOUT the common factor r = 1/s (Coef::r): rk4_step folds r into the step-size
+// factors (two multiplications per stage instead of one per coefficient), ray_rhs_scaled applies it for the diagnostics.
 template <class T>
-struct Coef { T A, C, Ax, Ab; };
+struct Coef { T A, C, Ax, Ab, r; };
 
 // SC: the caller's field is already in units of sqrt(beta) (Params::sB0), i.e. b2 IS Y2 and Ab multiplies (1/2) grad Y2.
 // Ax multiplies HALF the gradient of X (Local::hgX), which is where the 1/2 of the header comment has gone.
@@ -285,11 +287,11 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
     const T DXn = rt_fma(sig, DS, -q1);
     const T DYn = rt_fma(Xsp, DS, -q2);
     const T s = rt_fma(v, S, -rt_fma(Y2, DYn, X * DXn));
-    const T r = rt_rcp(s);
-    c.A = S * r;
+    c.r = rt_rcp(s);
+    c.A = S;
     c.C = T(0);
-    c.Ax = DXn * r;
-    c.Ab = SC ? r * DYn : (P.beta * r) * DYn;
+    c.Ax = DXn;
+    c.Ab = SC ? DYn : P.beta * DYn;
   } else {
     const T d2 = (T(0.5) * Xd) * XdY22;
     const T Pp = rt_fma(-X, P.one_plus_mu, T(1));
@@ -306,11 +308,11 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
     const T DXn = rt_fma(q1, pw, rt_fma(P.one_plus_mu, ab, sig * DS));
     const T DYn = rt_fma(q2, pw, Xsp * DS);
     const T s = rt_fma(v, Dv, rt_fma(u, Du, -rt_fma(Y2, DYn, X * DXn)));
-    const T r = rt_rcp(s);
-    c.A = Dv * r;
-    c.C = Bc * (Du * r);
-    c.Ax = DXn * r;
-    c.Ab = SC ? rt_fma(Bc, c.C, r * DYn) : rt_fma(Bc, c.C, (P.beta * r) * DYn);
+    c.r = rt_rcp(s);
+    c.A = Dv;
+    c.C = Bc * Du;
+    c.Ax = DXn;
+    c.Ab = SC ? rt_fma(Bc, c.C, DYn) : rt_fma(Bc, c.C, P.beta * DYn);
   }
   return c;
 }
@@ -487,31 +489,41 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
   return inside;
 }
 
-// ---- one evaluation of the ray right-hand side f(y), y = (x, n) --------------------------------------------------
-// Returns false (and f unspecified) if x is outside the equilibrium's domain.
+// ---- one evaluation of the ray right-hand side, y = (x, n) --------------------------------------------------------
+// Returns the right-hand side as (f, r): dy/dtau = r f, r = 1/s the reciprocal of the header comment.  Returns false
+// (and f, r unspecified) if x is outside the equilibrium's domain.
 template <class T, int EQ, int DISP, class Gather>
-RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, Gather& gather) {
+RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) {
   Local<T> L;
   const T* n = y + 3;
+  if (EQ == EQ_PARABOLIC) {
+    // O-mode in X = xs + par_g (x^2 + y^2) (config 1-2), written out so that the two products par_g x, par_g y serve
+    // both grad X / 2 and X itself:  s = v + X = n_x^2 + n_y^2 + (par_g x) x + (par_g y) y + (n_z^2 + xs), whose last
+    // term is constant along the ray (dn_z/dtau = 0).
+    const T gx = P.par_g * y[0], gy = P.par_g * y[1];
+    const T base = rt_fma(n[2], n[2], P.xs);
+    r = rt_rcp(rt_fma(n[0], n[0], rt_fma(n[1], n[1], rt_fma(gx, y[0], rt_fma(gy, y[1], base)))));
+    f[0] = n[0]; f[1] = n[1]; f[2] = n[2];
+    f[3] = -gx; f[4] = -gy; f[5] = T(0);
+    return true;
+  }
   constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
   const bool inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
   if (DISP == DISP_O) {
     // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)   =>   dx/dtau = n r, dn/dtau = -grad X r/2, r = 1/(v+X)
-    const T r = rt_rcp(v + L.X);
-    f[0] = n[0] * r; f[1] = n[1] * r; f[2] = n[2] * r;
-    if (EQ == EQ_PARABOLIC) {
-      const T c = -P.par_g * r;
-      f[3] = c * y[0]; f[4] = c * y[1]; f[5] = T(0);
-    } else if (EQ == EQ_LINEAR) {
-      f[3] = -P.lin_gxh * r; f[4] = T(0); f[5] = T(0);
+    r = rt_rcp(v + L.X);
+    f[0] = n[0]; f[1] = n[1]; f[2] = n[2];
+    if (EQ == EQ_LINEAR) {
+      f[3] = -P.lin_gxh; f[4] = T(0); f[5] = T(0);
     } else {
-      const T fR = -r * L.hgX[0];
-      f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = -r * L.hgX[2];
+      const T fR = -L.hgX[0];
+      f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = -L.hgX[2];
     }
     return inside;
   }
   const Coef<T> c = disp_coefs<T, DISP, SC>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
+  r = c.r;
   f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
   if (EQ == EQ_LINEAR) {
     T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gxh);
@@ -539,6 +551,16 @@ RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, Gather& gather) {
     f[3] = fR * L.cph; f[4] = fR * L.sph;
   }
   f[5] = fZ;
+  return inside;
+}
+
+// dy/dtau itself (diagnostics: rt_rhs)
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV bool ray_rhs_scaled(const Params<T>& P, const T* y, T* f, Gather& gather) {
+  T r;
+  const bool inside = ray_rhs<T, EQ, DISP>(P, y, f, r, gather);
+#pragma unroll
+  for (int j = 0; j < 6; ++j) f[j] *= r;
   return inside;
 }
 

@@ -2,9 +2,8 @@
 
     python -m paper_2508_15967_b200.sass_count            # table for every trace kernel in librt_b200.so
 
-A ray-step is one pass through the RK4 step region of the kernel (the ``if (status == 0) status = rk4_step(...)`` body:
-the reconvergence region inside the step loop that holds the most FP-pipe instructions -- the other one is the sample
-store); for the grid equilibrium the stage loop inside it is rolled and runs 4 times.
+A ray-step is one pass through the body of the kernel's step loop (the loops that hold FP-pipe instructions are nested:
+sample loop > step loop, and for the grid equilibrium > the rolled stage loop, which runs 4 times per step).
 Reported per kernel:
 
 * ``instr``     FP-pipe instructions per ray-step (DFMA + DMUL + DADD + DSETP, or the FP32 analogues) -- what the FP64
@@ -73,36 +72,28 @@ def count_kernels(lib: Path = LIB) -> dict:
             continue
         prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
         ins = _parse(fn)
-        loop = None                                         # the step loop: largest backward branch
+        fp_ops = _FP[prec]
+        # Loop nest of the kernel = its backward branches.  The loops that hold FP-pipe instructions are nested:
+        # sample loop > step loop (> stage loop, when the stages are rolled: grid equilibrium).  The small loops of the
+        # store staging and of the cooperative cell-cache refill hold no FP instruction and are ignored.
+        loops = []
         for a, op, rest in ins:
             if op.startswith("BRA"):
                 t = _target(rest)
-                if t is not None and t < a and (loop is None or a - t > loop[1] - loop[0]):
-                    loop = (t, a)
-        if loop is None:
+                if t is not None and t < a:
+                    loops.append((t, a + 16))
+        nfp = {l: sum(1 for b, o, _ in ins if l[0] <= b < l[1] and o.split(".")[0] in fp_ops) for l in loops}
+        chain = sorted((l for l in loops if nfp[l] > 0), key=lambda l: l[1] - l[0])
+        if not chain:
             continue
-        fp_ops = _FP[prec]
-        region, best = None, -1                             # the RK4 step: the BSSY ... BSYNC region inside the loop
-        for a, op, rest in ins:                             # that holds the most FP-pipe instructions
-            if op.startswith("BSSY") and loop[0] <= a < loop[1]:
-                t = _target(rest)
-                if t is None or not (a < t <= loop[1] + 16):
-                    continue
-                nfp = sum(1 for b, o, _ in ins if a <= b < t and o.split(".")[0] in fp_ops)
-                if nfp > best:
-                    region, best = (a, t), nfp
-        if region is None:
-            continue
+        for small, big in zip(chain, chain[1:]):
+            assert big[0] <= small[0] and small[1] <= big[1], "FP loops are not nested"
+        rolled = len(chain) >= 3
+        region = chain[1] if rolled else chain[0]          # the step loop's body = one ray-step
         c, rsq = _count(ins, *region)
         tot = Counter(c)
-        inner = None                                        # rolled stage loop (grid): largest backward branch inside
-        for a, op, rest in ins:
-            if op.startswith("BRA") and region[0] <= a < region[1]:
-                t = _target(rest)
-                if t is not None and region[0] <= t < a and (inner is None or a - t > inner[1] - inner[0]):
-                    inner = (t, a)
-        if inner is not None and inner[1] - inner[0] > (region[1] - region[0]) // 2:
-            ci, rsqi = _count(ins, *inner)
+        if rolled:                                          # the stage loop runs 4 times per step
+            ci, rsqi = _count(ins, *chain[0])
             for k, v in ci.items():
                 tot[k] += 3 * v
             rsq += 3 * rsqi
