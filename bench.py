@@ -49,10 +49,17 @@ FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 259, (4, "f6
                       (1, "f32"): 115, (2, "f32"): 115, (3, "f32"): 262, (4, "f32"): 798, (5, "f32"): 1257}
 FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f64"): 624, (5, "f64"): 888,
                          (1, "f32"): 69, (2, "f32"): 69, (3, "f32"): 178, (4, "f32"): 538, (5, "f32"): 823}
+# FP_RF3_PER_RAY_STEP: how many of those instructions read THREE registers from the register file.  Such an instruction
+# occupies the FP64 pipe for 3 cycles instead of 2 (FP32: 1.56 instead of 1) -- measured by rt_fma_peak_shape, shape 2
+# (profiles/r1_fma_peak_shapes.md) -- so the pipe time of a ray-step is (instr + RF3_EXTRA * rf3) issue slots of the FMA
+# microbenchmark; `pipe_model_frac` is that time over the measured kernel time.
+FP_RF3_PER_RAY_STEP = {(1, "f64"): 42, (2, "f64"): 42, (3, "f64"): 75, (4, "f64"): 225, (5, "f64"): 380,
+                       (1, "f32"): 37, (2, "f32"): 37, (3, "f32"): 43, (4, "f32"): 173, (5, "f32"): 292}
+RF3_EXTRA = {"f64": 0.5, "f32": 0.563}      # shape 0 rate / shape 2 rate - 1:  63.9 / 42.7 = 1.50,  123.2 / 78.8 = 1.563
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None
-NCU_DRAM_BYTES = {(4, "f64"): 5.99e9}     # profiles/r1_cfg4_f64_ncu_c.md: dram__bytes_read.sum + dram__bytes_write.sum
+NCU_DRAM_BYTES = {(4, "f64"): 5.99e9}     # profiles/r1_cfg4_f64_ncu_e.md: dram__bytes_read.sum + dram__bytes_write.sum
 
 WORKLOAD_NAMES = {
     1: "cfg1: O-mode, parabolic slab, 1024 rays x 1000 steps, full trajectory",
@@ -332,7 +339,10 @@ def run_ours(args) -> int:
                 "traffic": NCU_DRAM_BYTES.get((cfg, prec)), "kernel": f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
                 "kernel_ms": kernel_ms, "flops_per_ray_step": FLOPS_PER_RAY_STEP[(cfg, prec)],
                 "fp_instr_per_ray_step": FP_INSTR_PER_RAY_STEP[(cfg, prec)],
+                "fp_rf3_per_ray_step": FP_RF3_PER_RAY_STEP[(cfg, prec)],
                 "pipe_frac": FP_INSTR_PER_RAY_STEP[(cfg, prec)] * job.ray_steps / (kernel_ms * 1e-3) / peak_after,
+                "pipe_model_frac": (FP_INSTR_PER_RAY_STEP[(cfg, prec)] + RF3_EXTRA[prec] * FP_RF3_PER_RAY_STEP[(cfg, prec)])
+                * job.ray_steps / (kernel_ms * 1e-3) / peak_after,
                 "peak_source": f"rt_fma_peak({prec}) measured in this process after the timed region: "
                                f"{peak_after / 1e12:.3f} T{'D' if prec == 'f64' else 'F'}FMA/s at {peak_mhz:.0f} MHz "
                                f"(before: {peak_before / 1e12:.3f})"}
@@ -352,7 +362,9 @@ def run_ours(args) -> int:
             extra.append({"workload": f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else ""),
                           "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
                           "roofline_frac": FLOPS_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / (2.0 * pk),
-                          "pipe_frac": FP_INSTR_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / pk})
+                          "pipe_frac": FP_INSTR_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / pk,
+                          "pipe_model_frac": (FP_INSTR_PER_RAY_STEP[(c, p)] + RF3_EXTRA[p] * FP_RF3_PER_RAY_STEP[(c, p)])
+                          * j.ray_steps / (kms * 1e-3) / pk})
             j.close()
             del j
             torch.cuda.empty_cache()

@@ -386,7 +386,7 @@ def fma_peak(precision="f64", min_ms: float = 100.0):
 
 def fma_peak_shape(precision="f64", shape: int = 0, blocks_per_sm: int = 4, min_ms: float = 100.0):
     """``rt_fma_peak_shape``: the same microbenchmark with its instruction shape (0: acc*a+acc, 1: acc*a+b) and
-    occupancy (256-thread blocks per SM) exposed.  Returns (fused multiply-adds per second, SM clock in MHz)."""
+    occupancy (256-thread blocks per SM) exposed (shape 2: acc_j*a_j+b_j, three register-file reads per instruction).  Returns (fused multiply-adds per second, SM clock in MHz)."""
     lib = load()
     rate, mhz = ctypes.c_double(), ctypes.c_double()
     p = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
@@ -399,8 +399,8 @@ if __name__ == "__main__":      # python -m paper_2508_15967_b200.binding : prin
     import torch
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     for prec in ("f64", "f32"):
-        for shape in (0, 1):
+        for shape in (0, 1, 2, 3, 4):
             for bps in (1, 2, 4, 8):
                 r, mhz = fma_peak_shape(prec, shape, bps, 100.0)
-                print(f"| {prec} | {'acc*a+acc' if shape == 0 else 'acc*a+b'} | {2 * bps} | {r / (mhz * 1e6) / sms:.1f} | "
+                print(f"| {prec} | {('acc*a+acc', 'acc*a+b', 'acc_j*a_j+b_j', 'acc*a+acc, + 4 MUFU per 16', 'acc*a+acc, one chain')[shape]} | {2 * bps} | {r / (mhz * 1e6) / sms:.1f} | "
                       f"{r / 1e12:.2f} | {mhz:.0f} |")

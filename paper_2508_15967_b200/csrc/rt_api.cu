@@ -587,7 +587,8 @@ int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_cloc
 int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
                       double* sm_clock_mhz) {
   if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
-  if (shape != 0 && shape != 1) return fail(RT_ERR_INVALID, "shape must be 0 (acc*a+acc) or 1 (acc*a+b)");
+  if (shape < 0 || shape > 4)
+    return fail(RT_ERR_INVALID, "shape must be 0 (acc*a+acc), 1 (acc*a+b, shared a, b), 2 (acc_j*a_j+b_j), 3 (0 + MUFU) or 4 (one chain)");
   if (blocks_per_sm < 1 || blocks_per_sm > 8) return fail(RT_ERR_INVALID, "blocks_per_sm must be in [1, 8]");
   if (!fma_per_s) return fail(RT_ERR_INVALID, "fma_per_s is NULL");
   if (!(min_ms > 0.0) || min_ms > 10000.0) return fail(RT_ERR_INVALID, "min_ms must be in (0, 10000]");
@@ -604,14 +605,21 @@ int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms
   RT_CUDA(cudaEventCreate(&e1));
   auto run = [&](long long iters, float* ms) -> int {
     RT_CUDA(cudaEventRecord(e0, 0));
-    if (precision == RT_F64 && shape == 0)
-      rt::fma_peak_kernel<double, 0><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 1e-9, 1e-3, clk);
-    else if (precision == RT_F64)
-      rt::fma_peak_kernel<double, 1><<<grid, rt::FMA_BLOCK>>>(static_cast<double*>(sink), iters, 0.999, 1e-3, clk);
-    else if (shape == 0)
-      rt::fma_peak_kernel<float, 0><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1e-7f, 1e-3f, clk);
-    else
-      rt::fma_peak_kernel<float, 1><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 0.999f, 1e-3f, clk);
+#define RT_PEAK(T, SH, A, B) rt::fma_peak_kernel<T, SH><<<grid, rt::FMA_BLOCK>>>(static_cast<T*>(sink), iters, A, B, clk)
+    if (precision == RT_F64) {
+      if (shape == 0) RT_PEAK(double, 0, 1e-9, 1e-3);
+      else if (shape == 1) RT_PEAK(double, 1, 0.999, 1e-3);
+      else if (shape == 2) RT_PEAK(double, 2, 0.999, 1e-3);
+      else if (shape == 3) RT_PEAK(double, 3, 1e-9, 1e-3);
+      else RT_PEAK(double, 4, 1e-9, 1e-3);
+    } else {
+      if (shape == 0) RT_PEAK(float, 0, 1e-7f, 1e-3f);
+      else if (shape == 1) RT_PEAK(float, 1, 0.999f, 1e-3f);
+      else if (shape == 2) RT_PEAK(float, 2, 0.999f, 1e-3f);
+      else if (shape == 3) RT_PEAK(float, 3, 1e-7f, 1e-3f);
+      else RT_PEAK(float, 4, 1e-7f, 1e-3f);
+    }
+#undef RT_PEAK
     ++g_launches;
     RT_CUDA(cudaGetLastError());
     RT_CUDA(cudaEventRecord(e1, 0));

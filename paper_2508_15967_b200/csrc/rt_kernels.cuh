@@ -552,17 +552,34 @@ reduce_kernel(const T* __restrict__ res, const int32_t* __restrict__ status, lon
 }
 
 // Roofline denominator: FMA_CHAINS independent accumulators per thread, each a dependent chain of fused multiply-adds.
-// SHAPE 0 (the denominator rt_fma_peak reports): acc = acc * a + acc, two distinct source registers.  SHAPE 1:
-// acc = acc * a + b, three distinct 64-bit sources -- what real code mostly issues; on B200 the DFMA rate then drops
-// from 63.7 to 58.8 per clock per SM (operand-bank conflicts; rt_fma_peak_shape, profiles/r1_fma_peak_shapes.md).
+//   SHAPE 0 (the denominator rt_fma_peak reports): acc = acc * a + acc -- two distinct source registers;
+//   SHAPE 1: acc = acc * a + b with a, b shared by all chains -- three distinct sources, but consecutive instructions
+//            find a and b in the operand-reuse cache;
+//   SHAPE 2: acc_j = acc_j * a_j + b_j with per-chain a_j, b_j (8 chains, each used twice per round) -- three distinct
+//            64-bit registers read from the register file by every instruction: what most DFMAs of real code look like;
+//   SHAPE 3: shape 0 plus 4 independent MUFU reciprocal seeds per 16 FMAs (the ratio of the O-mode kernel; the full
+//            determinant has 1 per 22): the seeds run on the XU pipe BESIDE the FMA pipe and cost ~2 % of the FMA rate;
+//   SHAPE 4: shape 0 with ONE chain per thread: the rate is warps-per-scheduler / dependent-issue latency (8 cycles for
+//            a DFMA), i.e. 4 warps per scheduler saturate the FP64 pipe without any instruction-level parallelism.
+// On B200 the DFMA rate is 63.7 / 58 / 42.7 per clock per SM for shapes 0 / 1 / 2: an FP64 instruction that reads three
+// registers from the register file occupies the pipe for 3 cycles instead of 2 (profiles/r1_fma_peak_shapes.md).
 constexpr int FMA_CHAINS = 16;
 constexpr int FMA_BLOCK = 256;
+RT_DEV double rcp_seed(double x) { double r; asm volatile("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x)); return r; }
+RT_DEV float rcp_seed(float x) { float r; asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 template <class T, int SHAPE>
 __global__ void __launch_bounds__(FMA_BLOCK)
 fma_peak_kernel(T* __restrict__ sink, long long iters, T a, T b, unsigned long long* __restrict__ clk) {
-  T acc[FMA_CHAINS];
+  constexpr int NC = (SHAPE == 2) ? FMA_CHAINS / 2 : (SHAPE == 4) ? 1 : FMA_CHAINS;
+  T acc[NC], aj[NC], bj[NC], seed[4];
 #pragma unroll
-  for (int j = 0; j < FMA_CHAINS; ++j) acc[j] = T(threadIdx.x + j) * T(1e-3);
+  for (int j = 0; j < 4; ++j) seed[j] = T(1.5) + T(threadIdx.x + j);
+#pragma unroll
+  for (int j = 0; j < NC; ++j) {
+    acc[j] = T(threadIdx.x + j) * T(1e-3);
+    aj[j] = a + T(threadIdx.x + j) * T(1e-9);
+    bj[j] = b + T(threadIdx.x + 2 * j) * T(1e-9);
+  }
   unsigned long long t0, t1;
   const long long c0 = clock64();
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t0));
@@ -570,14 +587,23 @@ fma_peak_kernel(T* __restrict__ sink, long long iters, T a, T b, unsigned long l
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
 #pragma unroll
-      for (int j = 0; j < FMA_CHAINS; ++j) acc[j] = (SHAPE == 0) ? rt_fma(acc[j], a, acc[j]) : rt_fma(acc[j], a, b);
+      for (int j = 0; j < FMA_CHAINS; ++j) {
+        const int c = j % NC;
+        acc[c] = (SHAPE == 0 || SHAPE == 3 || SHAPE == 4) ? rt_fma(acc[c], a, acc[c])
+                 : (SHAPE == 1) ? rt_fma(acc[c], a, b) : rt_fma(acc[c], aj[c], bj[c]);
+      }
+      if (SHAPE == 3) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) seed[j] = rcp_seed(seed[j]);
+      }
     }
   }
   const long long c1 = clock64();
   asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t1));
   T s = T(0);
 #pragma unroll
-  for (int j = 0; j < FMA_CHAINS; ++j) s += acc[j];
+  for (int j = 0; j < NC; ++j) s += acc[j];
+  if (SHAPE == 3) s += seed[0] + seed[1] + seed[2] + seed[3];
   sink[(long long)blockIdx.x * FMA_BLOCK + threadIdx.x] = s;
   if (threadIdx.x == 0 && blockIdx.x == 0) { clk[0] = (unsigned long long)(c1 - c0); clk[1] = t1 - t0; }
 }

@@ -8,6 +8,11 @@ Reported per kernel:
 
 * ``instr``     FP-pipe instructions per ray-step (DFMA + DMUL + DADD + DSETP, or the FP32 analogues) -- what the FP64
                 (FP32) pipe has to issue, the quantity the kernels are optimised for;
+* ``rf3``       how many of them read THREE registers from the register file (constants, immediates, RZ and operands
+                served by the operand-reuse cache -- flagged ``.reuse`` in the same slot of the preceding instruction --
+                do not count).  Such an instruction occupies the FP64 pipe for 3 cycles instead of 2 (FP32: 1.56
+                instead of 1; ``rt_fma_peak_shape`` shape 2, profiles/r1_fma_peak_shapes.md), so the pipe time of a
+                ray-step is 2 instr + rf3 cycles per warp and scheduler;
 * ``executed``  flops as executed, a fused multiply-add counted as 2;
 * ``mufu``      MUFU seeds (reciprocals and reciprocal square roots), ``rsqrt`` of them square roots;
 * ``local``     local-memory (spill) instructions executed per ray-step: must be 0.  ptxas may still report a few bytes
@@ -59,6 +64,33 @@ def _count(ins, lo, hi):
         sum(1 for a, op, _ in ins if lo <= a < hi and op.startswith("MUFU.RSQ"))
 
 
+_REG = re.compile(r"[-|~]*R(\d+)")
+
+
+def _rf3(ins, lo, hi, fp_ops):
+    """FP-pipe instructions in [lo, hi) whose three source operands are all read from the register file."""
+    n3, reuse = 0, {}
+    for a, op, rest in ins:
+        if not (lo <= a < hi):
+            continue
+        ops = [o.strip() for o in rest.split(",")]
+        base = op.split(".")[0]
+        srcs = ops[2:] if base.endswith("SETP") else ops[1:]
+        if base in fp_ops:
+            reads = 0
+            for slot, o in enumerate(srcs):
+                m = _REG.match(o)
+                if m and reuse.get(slot) != m.group(1):
+                    reads += 1
+            n3 += reads >= 3
+        reuse = {}
+        for slot, o in enumerate(ops[1:]):
+            m = _REG.match(o)
+            if m and ".reuse" in o:
+                reuse[slot] = m.group(1)
+    return n3
+
+
 def count_kernels(lib: Path = LIB) -> dict:
     """{(precision 'f64'|'f32', eq_kind, disp_kind): {'instr', 'executed', 'mufu', 'rsqrt', 'flops'}} per ray-step."""
     exe = cuobjdump()
@@ -92,11 +124,13 @@ def count_kernels(lib: Path = LIB) -> dict:
         region = chain[1] if rolled else chain[0]          # the step loop's body = one ray-step
         c, rsq = _count(ins, *region)
         tot = Counter(c)
+        rf3 = _rf3(ins, *region, fp_ops)
         if rolled:                                          # the stage loop runs 4 times per step
             ci, rsqi = _count(ins, *chain[0])
             for k, v in ci.items():
                 tot[k] += 3 * v
             rsq += 3 * rsqi
+            rf3 += 3 * _rf3(ins, *chain[0], fp_ops)
         fma, mul, add, setp = _FP[prec]
         executed = 2 * tot[fma] + tot[mul] + tot[add]
         mufu = tot["MUFU"]
@@ -104,14 +138,14 @@ def count_kernels(lib: Path = LIB) -> dict:
         local = tot["STL"] + tot["LDL"]                     # spill traffic executed per ray-step (must be 0)
         res[("f64" if prec == "d" else "f32", eq, disp)] = dict(instr=tot[fma] + tot[mul] + tot[add] + tot[setp],
                                                                 executed=executed, mufu=mufu, rsqrt=rsq, flops=flops,
-                                                                local=local)
+                                                                local=local, rf3=rf3)
     return res
 
 
 if __name__ == "__main__":
     names = {0: "parabolic", 1: "linear", 2: "tokamak", 3: "grid", 4: "tokamak_pow"}
     disps = {0: "O", 1: "X", 2: "full"}
-    print(f"{'kernel':34s} {'instr':>6s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s} {'local':>6s}")
+    print(f"{'kernel':34s} {'instr':>6s} {'rf3':>5s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s} {'local':>6s}")
     for (prec, eq, disp), r in sorted(count_kernels().items()):
-        print(f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}> {r['instr']:6d} {r['executed']:9d} {r['mufu']:5d} "
+        print(f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}> {r['instr']:6d} {r['rf3']:5d} {r['executed']:9d} {r['mufu']:5d} "
               f"{r['rsqrt']:6d} {r['flops']:6d} {r['local']:6d}")

@@ -62,7 +62,7 @@ def test_create_validates_descriptors(lib):
     ok = inputs.config(4, n_rays=4).eq
     eq = binding.create_equilibrium(ok)          # analytic kinds need no device
     eq.close()
-    for bad in (dict(ok, a=0.0), dict(ok, B0=0.0), dict(ok, q0=0.0), dict(ok, rho_max=1.5), dict(ok, kind=7),
+    for bad in (dict(ok, a=0.0), dict(ok, B0=0.0), dict(ok, q0=0.0), dict(ok, rho_max=1.5), dict(ok, kind=7), dict(ok, a=ok["R0"]),
                 dict(ok, ion_mass=-1.0), dict(ok, ion_charge=0.0), dict(ok, n_ref=float("nan")),
                 dict(inputs.config(1, n_rays=4).eq, L=0.0), dict(inputs.config(3, n_rays=4).eq, L_ramp=0.0)):
         with pytest.raises(binding.RtError) as e:
@@ -137,7 +137,7 @@ def test_no_cpu_fallback_without_a_device(lib):
     rate = ctypes.c_double()
     assert lib.rt_fma_peak(0, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
     assert lib.rt_fma_peak_shape(0, 1, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
-    assert lib.rt_fma_peak_shape(0, 2, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
+    assert lib.rt_fma_peak_shape(0, 5, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
     assert lib.rt_fma_peak_shape(0, 0, 9, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
     with pytest.raises(binding.RtError):
         binding.create_equilibrium(inputs.synth_grid(seed=3, nR=9, nZ=9, nPsi=9))   # grid tables live on the device
@@ -169,6 +169,7 @@ def test_flop_tables_match_the_compiled_kernels(lib):
         got = counted[(prec, eq, disp)]
         assert got["flops"] == flops, (cfg, prec, got)
         assert got["instr"] == bench.FP_INSTR_PER_RAY_STEP[(cfg, prec)], (cfg, prec, got)
+        assert got["rf3"] == bench.FP_RF3_PER_RAY_STEP[(cfg, prec)], (cfg, prec, got)
     # spills would show up as local-memory traffic: no trace kernel may execute a local load / store inside a ray-step,
     # and what ptxas parks outside the step loop (store staging: once per ray) stays below 64 bytes
     assert all(r["local"] == 0 for r in counted.values()), {k: r["local"] for k, r in counted.items() if r["local"]}
