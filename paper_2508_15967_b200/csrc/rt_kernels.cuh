@@ -16,15 +16,16 @@
 
 namespace rt {
 
-// Launch shapes.  The trace kernels are bound by the FP64 (FP32) pipe and by registers, not by memory, so what is tuned is
-// how many warps fit beside each other: 64-thread blocks with a per-kernel register cap (`__maxnreg__`) chosen by
-// measurement on B200 (profiles/r1_tuning.md):
-//   fp64, analytic equilibria   112 registers -> 9 blocks = 18 warps per SM (128 registers / 16 warps: +1.7 % time;
-//                                96 registers / 20 warps spills 112 B and is 2.8 % slower)
-//   fp64, grid equilibrium       96 registers -> 10 blocks = 20 warps per SM (the LDS latency of the cell cache wants
-//                                more warps: 2.9 % faster than 128 registers; no spills)
-//   fp32                         72 registers -> 14 blocks = 28 warps per SM
-// The diagnostic kernels (rhs, launch) use plain 128-thread blocks.
+// Launch shapes.  The trace kernels are bound by the FP64 (FP32) pipe, not by memory and not by latency: 4 warps per
+// scheduler saturate the FP64 pipe even without instruction-level parallelism (8-cycle dependent-issue latency, one
+// instruction per 2 cycles), and every shape between 12 and 18 warps per SM runs within 0.3 % of the others as long as it
+// does not spill (profiles/r1_tuning.md).  So the register cap (`__maxnreg__`) is simply the smallest one without spills
+// inside the step, with 64-thread blocks so that the register file divides evenly:
+//   fp64, analytic equilibria   120 registers -> 8 blocks = 16 warps per SM
+//   fp64, grid equilibrium      112 registers -> 9 blocks = 18 warps per SM (96 spills inside the stage loop)
+//   fp32                         72 registers -> 14 blocks = 28 warps per SM (the grid kernel's LDS latency likes warps:
+//                                321 ms at 72 registers, 344 ms at 128)
+// The diagnostic kernels (rhs, launch, diag) use plain 128-thread blocks.
 #ifndef RT_GRID_ROLLED
 #define RT_GRID_ROLLED 1      // grid equilibrium: one copy of the stage code (stage loop not unrolled)
 #endif
