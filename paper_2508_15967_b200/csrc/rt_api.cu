@@ -598,9 +598,17 @@ int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms
   const int grid = sms * blocks_per_sm;                      // 256-thread blocks: 2 warps per scheduler each
   void* sink = nullptr;
   unsigned long long* clk = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  struct Cleanup {                                           // every early return below releases what was acquired
+    void*& sink; unsigned long long*& clk; cudaEvent_t& e0; cudaEvent_t& e1;
+    ~Cleanup() {
+      if (e0) cudaEventDestroy(e0);
+      if (e1) cudaEventDestroy(e1);
+      cudaFree(sink); cudaFree(clk);
+    }
+  } cleanup{sink, clk, e0, e1};
   RT_CUDA(cudaMalloc(&sink, (size_t)grid * rt::FMA_BLOCK * 8));
   RT_CUDA(cudaMalloc(reinterpret_cast<void**>(&clk), 16));
-  cudaEvent_t e0, e1;
   RT_CUDA(cudaEventCreate(&e0));
   RT_CUDA(cudaEventCreate(&e1));
   auto run = [&](long long iters, float* ms) -> int {
@@ -640,12 +648,10 @@ int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms
     *fma_per_s = fmas / (ms * 1e-3);
     if (sm_clock_mhz) {
       unsigned long long h[2] = {0, 0};
-      cudaMemcpy(h, clk, 16, cudaMemcpyDeviceToHost);
+      RT_CUDA(cudaMemcpy(h, clk, 16, cudaMemcpyDeviceToHost));
       *sm_clock_mhz = h[1] ? (double)h[0] / (double)h[1] * 1e3 : 0.0;
     }
   }
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(sink); cudaFree(clk);
   return rc;
 }
 
