@@ -139,7 +139,10 @@ def oracle_rate(cfg: int, target_s: float, n_threads: int = 0):
     at the config's full step count, n sized from a short calibration so the run takes about `target_s` seconds."""
     import oracle
     oracle.build()
-    cores = oracle.max_threads() if n_threads <= 0 else n_threads
+    # all host cores this process may run on (torchrun exports OMP_NUM_THREADS=1, which omp_get_max_threads() would obey;
+    # under torchrun only rank 0 runs the oracle, so the cores are its own)
+    avail = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    cores = max(avail, oracle.max_threads()) if n_threads <= 0 else n_threads
     n_steps = inputs.FULL_SIZES[cfg][1]
     probe_n = 8 * cores
     w = inputs.config(cfg, n_rays=probe_n, n_steps=n_steps)
