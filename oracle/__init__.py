@@ -71,6 +71,7 @@ def _load():
         lib.oracle_dispersion_value.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, P]
         lib.oracle_plasma.argtypes = [ctypes.POINTER(_CEq), P, D, I64, P, P, P, P]
         lib.oracle_launch.argtypes = [ctypes.POINTER(_CEq), I32, I32, P, P, D, I64, P, P]
+        lib.oracle_launch_kx.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, P, I64, I32, D, P, P, P]
         lib.oracle_max_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -237,6 +238,26 @@ def launch(eq, disp, x0, dirs, omega, branch=0):
     if rc != 0:
         raise ValueError("oracle_launch rejected its arguments")
     return k0, D
+
+
+def launch_kx(eq, disp, x0, k_guess, omega, max_iter=50, tol=1e-15):
+    """The paper's own launch iteration (L159): w, x, k_y, k_z fixed (rows 1, 2 of ``k_guess`` [3,n]); k_x found by
+    Newton's method from the initial guess in row 0, which selects the root, until |D| < tol.  Returns (k0 [3,n], D [n],
+    iters [n]: Newton updates used, -1 = not converged / outside the domain).  ``omega``: scalar or per ray [n]."""
+    lib, e = _load(), _eq(eq)
+    x0, kg = _soa(x0), _soa(k_guess)
+    n = x0.shape[1]
+    k0, D, it = np.empty((3, n)), np.empty(n), np.empty(n, dtype=np.int32)
+    w = None
+    if np.ndim(omega) > 0:
+        w = np.ascontiguousarray(omega, dtype=np.float64)
+        assert w.shape == (n,), w.shape
+    rc = lib.oracle_launch_kx(ctypes.byref(e.c), _disp(disp), x0.ctypes.data, kg.ctypes.data,
+                              0.0 if w is not None else float(omega), w.ctypes.data if w is not None else None, n,
+                              int(max_iter), float(tol), k0.ctypes.data, D.ctypes.data, it.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_launch_kx rejected its arguments")
+    return k0, D, it
 
 
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")

@@ -27,10 +27,11 @@
 // if any of its 4 stage points lies outside the equilibrium's domain (status 1) or if the new state
 // is not finite (status 2).  |D| at a saved state outside the domain is NaN.
 //
-// Also here: per-ray frequencies and critical-surface diagnostics and the second ensemble workload,
-// full-orbit charged particles in the same equilibria (oracle_orbit).
+// Also here: per-ray frequencies and critical-surface diagnostics, the second ensemble workload,
+// full-orbit charged particles in the same equilibria (oracle_orbit), and the paper's own launch
+// iteration (L159: Newton on k_x at fixed k_y, k_z; oracle_launch_kx).
 //
-// Parity pins: tests/test_oracle_*.py (P1..P19 in DESIGN.md).  No function here is "parity unpinned".
+// Parity pins: tests/test_oracle_*.py (P1..P20 in DESIGN.md).  No function here is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
@@ -546,6 +547,39 @@ int oracle_launch_w(const orc_equilibrium* eq, int disp, int branch, const doubl
                     const double* omega, int64_t n, double* k0, double* D_out) {
   if (!omega) return -1;
   return launch_impl(eq, disp, branch, x0, dir, 0.0, omega, n, k0, D_out);
+}
+
+// Launch states exactly as the paper states them (L159): "choosing fixed values for w, x, k_y and k_z.  The remaining
+// value k_x is determined using a Newton method to a tolerance of |D(k, w)| < 1e-15.  Since the dispersion functions are
+// multi-valued, an initial guess for k_x selects among the possible roots."
+//   k_guess [3][n]: rows 1, 2 = the fixed k_y, k_z; row 0 = the initial guess for k_x.   omega_rays [n] or NULL.
+// Iteration, in the paper's order: evaluate D and dD/dk_x (dual numbers) at the current k_x; stop if |D| < tol; otherwise
+// k_x <- k_x - D / (dD/dk_x); at most max_iter updates.  Returned: k0 = (k_x, k_y, k_z) at the last iterate, D there, and
+// iters = number of updates made if |D| < tol was reached, -1 if not (also for points outside the domain or a
+// non-finite iterate: k_x = NaN then).
+int oracle_launch_kx(const orc_equilibrium* eq, int disp, const double* x0, const double* k_guess, double omega_all,
+                     const double* omega_rays, int64_t n, int max_iter, double tol, double* k0, double* D_out,
+                     int32_t* iters_out) {
+  if (!eq || !combo_supported(*eq, disp) || max_iter < 0 || !(tol > 0.0)) return -1;
+  for (int64_t i = 0; i < n; ++i) {
+    const double omega = omega_rays ? omega_rays[i] : omega_all;
+    const double xi[3] = {x0[i], x0[n + i], x0[2 * n + i]};
+    double kk[3] = {k_guess[i], k_guess[n + i], k_guess[2 * n + i]};
+    double D = std::numeric_limits<double>::quiet_NaN(), g[ND];
+    int iters = -1;
+    for (int it = 0; it <= max_iter; ++it) {
+      const bool inside = eval_D(*eq, disp, xi, kk, omega, &D, g);
+      if (!inside || !std::isfinite(D)) { kk[0] = D = std::numeric_limits<double>::quiet_NaN(); break; }
+      if (std::fabs(D) < tol) { iters = it; break; }
+      if (it == max_iter) break;
+      kk[0] -= D / g[3];
+      if (!std::isfinite(kk[0])) { kk[0] = D = std::numeric_limits<double>::quiet_NaN(); break; }
+    }
+    for (int c = 0; c < 3; ++c) k0[c * n + i] = kk[c];
+    if (D_out) D_out[i] = D;
+    if (iters_out) iters_out[i] = iters;
+  }
+  return 0;
 }
 
 // ---- second ensemble workload of the same shape: full-orbit charged particles in the same equilibrium -------------
