@@ -132,6 +132,24 @@ int rt_launch(const rt_equilibrium* eq, int disp, int branch, const double* x0, 
 int rt_launch_w(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, const double* omega,
                 int64_t n, double* k0, double* D_out, void* cuda_stream);
 
+/* Launch conditions exactly as the paper states them: "choosing fixed values for w, x, k_y and k_z.  The
+ * remaining value k_x is determined using a Newton method to a tolerance of |D(k, w)| < 1e-15.  Since the dispersion
+ * functions are multi-valued, an initial guess for k_x selects among the possible roots."  Per ray: evaluate D and
+ * dD/dk_x at the current k_x; stop if |D| < tol; otherwise k_x <- k_x - D / (dD/dk_x); at most max_iter updates.  fp64.
+ *   x0            DEVICE double [3][n]
+ *   k_guess       DEVICE double [3][n]: rows 1, 2 = the fixed k_y, k_z [rad/m]; row 0 = the initial guess for k_x
+ *   omega         rad/s, used when omega_rays == NULL;  omega_rays  DEVICE double [n] per-ray frequencies, or NULL
+ *   max_iter      0..1000 Newton updates at most;  tol > 0 (the paper's value: 1e-15)
+ *   k0            DEVICE double [3][n]: (k_x at the last iterate, k_y, k_z); k_x = NaN at points outside the domain or after
+ *                 a non-finite iterate.  May alias k_guess.
+ *   D_out         DEVICE double [n] D at the returned state (signed; NaN with k_x); or NULL
+ *   iters_out     DEVICE int32 [n]: number of updates made if |D| < tol was reached, -1 if it was not; or NULL
+ * Errors: RT_ERR_INVALID (NULL / host / misaligned pointers, bad omega, n < 0, max_iter or tol out of range),
+ * RT_ERR_UNSUPPORTED (dispersion not defined on the equilibrium), RT_ERR_CUDA.  Asynchronous on cuda_stream. */
+int rt_launch_kx(const rt_equilibrium* eq, int disp, const double* x0, const double* k_guess, double omega,
+                 const double* omega_rays, int64_t n, int max_iter, double tol, double* k0, double* D_out,
+                 int32_t* iters_out, void* cuda_stream);
+
 /* Critical-surface diagnostics at n points, e.g. the samples of a trajectory (cut-offs and resonances
  * "denote important changes in wave behavior, and the behavior of rays in their vicinity is an indication of the
  * correctness of the solution"; Fig. 3-4).  fp64.

@@ -25,7 +25,7 @@ PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
 SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_launch", "rt_launch_w",
-           "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_launch_count", "rt_last_error", "rt_version")
+           "rt_launch_kx", "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_launch_count", "rt_last_error", "rt_version")
 NDIAG = 10
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
 
@@ -93,6 +93,7 @@ def load() -> ctypes.CDLL:
         lib.rt_trace_w.argtypes = [P, I32, I32, P, P, P, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_launch_w.argtypes = [P, I32, I32, P, P, P, I64, P, P, P]
         lib.rt_diagnostics.argtypes = [P, P, P, D, P, I64, P, P]
+        lib.rt_launch_kx.argtypes = [P, I32, P, P, D, P, I64, I32, D, P, P, P, P]
         lib.rt_orbit.argtypes = [P, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_trace_host.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P]
         lib.rt_launch.argtypes = [P, I32, I32, P, P, D, I64, P, P, P]
@@ -295,6 +296,26 @@ def launch(eq: Equilibrium, disp, x0, dirs, omega, branch: int = 0):
         _check(lib.rt_launch_w(eq.handle, _disp(disp), int(branch), _ptr(x0), _ptr(dirs), _ptr(w), n, _ptr(k0), _ptr(D),
                                _stream()))
     return k0, D
+
+
+def launch_kx(eq: Equilibrium, disp, x0, k_guess, omega, max_iter: int = 50, tol: float = 1e-15):
+    """``rt_launch_kx``: the paper's own launch iteration.  ``k_guess`` [3, n] float64 CUDA tensor: rows 1, 2
+    the fixed k_y, k_z, row 0 the initial guess for k_x; ``omega`` a float or a float64 CUDA tensor [n].  Returns
+    (k0 [3, n], D [n], iters int32 [n]: Newton updates used, -1 = tolerance not reached)."""
+    import torch
+    lib = load()
+    x0 = _dev_soa(x0, 3)
+    n = x0.shape[1]
+    kg = _dev_soa(k_guess, 3, n)
+    if x0.dtype != torch.float64 or kg.dtype != torch.float64:
+        raise TypeError("rt_launch_kx is fp64 only")
+    k0 = torch.empty((3, n), dtype=torch.float64, device=x0.device)
+    D = torch.empty((n,), dtype=torch.float64, device=x0.device)
+    it = torch.empty((n,), dtype=torch.int32, device=x0.device)
+    w = _omega_rays(omega, n)
+    _check(lib.rt_launch_kx(eq.handle, _disp(disp), _ptr(x0), _ptr(kg), 0.0 if w is not None else float(omega), _ptr(w), n,
+                            int(max_iter), float(tol), _ptr(k0), _ptr(D), _ptr(it), _stream()))
+    return k0, D, it
 
 
 def diagnostics(eq: Equilibrium, x, k, omega):

@@ -152,6 +152,28 @@ int launch_launch(const rt_equilibrium* eq, int disp, const rt::Params<double>& 
   return fail(RT_ERR_UNSUPPORTED, "no kernel for this equilibrium / dispersion combination");
 }
 
+int launch_launch_kx(const rt_equilibrium* eq, int disp, const rt::Params<double>& P, const double* x0, const double* kg,
+                     const double* omega, double omega_ref, long long n, int max_iter, double tol, double* k0, double* D_out,
+                     int32_t* iters_out, cudaStream_t st) {
+  if (n == 0) return RT_OK;
+  const unsigned grid = grid_for(n, rt::AUX_BLOCK);
+#define M(E, D)                                                                                                             \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                                                              \
+    if (omega)                                                                                                              \
+      rt::launch_kx_kernel<E, D, true><<<grid, rt::AUX_BLOCK, 0, st>>>(P, x0, kg, omega, omega_ref, n, max_iter, tol, k0,   \
+                                                                       D_out, iters_out);                                   \
+    else                                                                                                                    \
+      rt::launch_kx_kernel<E, D, false><<<grid, rt::AUX_BLOCK, 0, st>>>(P, x0, kg, omega, omega_ref, n, max_iter, tol, k0,  \
+                                                                        D_out, iters_out);                                  \
+    ++g_launches;                                                                                                           \
+    RT_CUDA(cudaGetLastError());                                                                                            \
+    return RT_OK;                                                                                                           \
+  }
+  RT_FOR_COMBOS(M)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no kernel for this equilibrium / dispersion combination");
+}
+
 // Per-ray frequencies: the per-call constants are folded at this reference and rescaled per thread (rt_kernels.cuh:
 // params_at_frequency).  1 rad/s keeps every folded constant finite in fp32 and needs no knowledge of the device array.
 constexpr double kOmegaRefPerRay = 1.0;
@@ -507,6 +529,25 @@ int rt_launch_w(const rt_equilibrium* eq, int disp, int branch, const double* x0
     return rc;
   const rt::Params<double> P = make_params<double>(eq, kOmegaRefPerRay);
   return launch_launch(eq, disp, P, branch, x0, dir, omega, kOmegaRefPerRay, n, k0, D_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rt_launch_kx(const rt_equilibrium* eq, int disp, const double* x0, const double* k_guess, double omega,
+                 const double* omega_rays, int64_t n, int max_iter, double tol, double* k0, double* D_out,
+                 int32_t* iters_out, void* cuda_stream) {
+  int rc = check_combo(eq, disp);
+  if (rc) return rc;
+  if (!omega_rays && (rc = check_omega(omega))) return rc;
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  if (max_iter < 0 || max_iter > 1000) return fail(RT_ERR_INVALID, "max_iter must be in [0, 1000]");
+  if (!(tol > 0.0) || !std::isfinite(tol)) return fail(RT_ERR_INVALID, "tol must be positive and finite");
+  if (n == 0) return RT_OK;
+  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(k_guess, "k_guess", false)) ||
+      (rc = require_device_ptr(omega_rays, "omega_rays", true)) || (rc = require_device_ptr(k0, "k0", false)) ||
+      (rc = require_device_ptr(D_out, "D_out", true)) || (rc = require_device_ptr(iters_out, "iters_out", true)))
+    return rc;
+  const rt::Params<double> P = make_params<double>(eq, omega_rays ? kOmegaRefPerRay : omega);
+  return launch_launch_kx(eq, disp, P, x0, k_guess, omega_rays, kOmegaRefPerRay, n, max_iter, tol, k0, D_out, iters_out,
+                          static_cast<cudaStream_t>(cuda_stream));
 }
 
 int rt_diagnostics(const rt_equilibrium* eq, const double* x, const double* k, double omega, const double* omega_rays,

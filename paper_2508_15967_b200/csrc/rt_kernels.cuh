@@ -6,6 +6,7 @@
 //   orbit_kernel   the second ensemble workload: full-orbit particles, same structure as trace_kernel.
 //   rhs_kernel     one stage evaluation per point (diagnostics and gradient parity tests).
 //   launch_kernel  launch conditions: closed-form |n| on D = 0 plus Newton polish.
+//   launch_kx_kernel  the paper's own launch iteration: k_y, k_z fixed, Newton on k_x from an initial guess.
 //   reduce_kernel  max / sum of |D| and status counts (PAPER.md L76 reduction kernels).
 //   fma_peak_kernel  the roofline denominator: independent FMA chains.
 #pragma once
@@ -483,6 +484,62 @@ launch_kernel(const __grid_constant__ Params<double> P0, int branch, const doubl
     const double v = sn * sn;
     D_out[i] = disp_value<double, DISP>(P, X, Y2, v * c2, v);
   }
+}
+
+// Launch conditions exactly as the paper states them: w, x, k_y, k_z fixed; k_x by Newton's method from
+// the caller's initial guess (which selects the root) until |D| < tol, at most max_iter updates.  x is fixed, so the
+// equilibrium is evaluated once; only n^2 and n.B change with k_x.  dD/dn_x = 2 D_v n_x + (2 G D_u / |B|^2) B_x.
+// Outputs: k0 = (k_x, k_y, k_z) at the last iterate (k_y, k_z copied bit for bit), D there, iters = updates made if
+// |D| < tol was reached, -1 if not; outside the domain or on a non-finite iterate k_x = D = NaN and iters = -1.
+template <int EQ, int DISP, bool PW>
+__global__ void __launch_bounds__(AUX_BLOCK)
+launch_kx_kernel(const __grid_constant__ Params<double> P0, const double* __restrict__ x0, const double* __restrict__ kg,
+                 const double* __restrict__ omega, double omega_ref, long long n, int max_iter, double tol,
+                 double* __restrict__ k0, double* __restrict__ D_out, int32_t* __restrict__ iters_out) {
+  const long long i = (long long)blockIdx.x * AUX_BLOCK + threadIdx.x;
+  if (i >= n) return;
+  const Params<double> P = PW ? params_at_frequency(P0, omega_ref / omega[i]) : P0;
+  double x[3], nn[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { x[c] = x0[c * n + i]; nn[c] = kg[c * n + i] * P.k2n; }
+  Local<double> L;
+  GatherDirect gather;
+  const bool inside = equilibrium<double, EQ, DISP>(P, x, nn, L, gather);
+  double B[3] = {0.0, 0.0, 0.0}, ib2 = 0.0, Y2 = 0.0;
+  if (DISP != DISP_O) Y2 = P.beta * L.b2;
+  if (DISP == DISP_FULL) {
+    if (EQ == EQ_LINEAR) {
+      B[2] = L.B[2];
+    } else {                                  // axisymmetric kinds: (R^, phi^, Z^) components -> Cartesian
+      B[0] = L.B[0] * L.cph - L.B[1] * L.sph;
+      B[1] = L.B[0] * L.sph + L.B[1] * L.cph;
+      B[2] = L.B[2];
+    }
+    ib2 = 1.0 / L.b2;
+  }
+  const double qnan = rt_nan<double>();
+  double nx = inside ? nn[0] : qnan, D = qnan;
+  int iters = -1;
+  bool updated = false;                       // no update made: k_x goes back bit for bit
+  for (int it = 0; it <= max_iter && inside; ++it) {
+    const double v = nx * nx + nn[1] * nn[1] + nn[2] * nn[2];
+    const double G = nx * B[0] + nn[1] * B[1] + nn[2] * B[2];
+    const double u = G * G * ib2;
+    D = disp_value<double, DISP>(P, L.X, Y2, u, v);
+    if (!isfinite(D)) { nx = qnan; D = qnan; break; }
+    if (fabs(D) < tol) { iters = it; break; }
+    if (it == max_iter) break;
+    double DX, DY2, Du, Dv;
+    disp_partials<double, DISP>(P, L.X, Y2, u, v, DX, DY2, Du, Dv);
+    nx -= D / (2.0 * Dv * nx + 2.0 * G * Du * ib2 * B[0]);
+    updated = true;
+    if (!isfinite(nx)) { nx = qnan; D = qnan; break; }
+  }
+  k0[i] = (updated || !inside) ? nx * P.n2k : kg[i];
+  k0[n + i] = kg[n + i];
+  k0[2 * n + i] = kg[2 * n + i];
+  if (D_out) D_out[i] = D;
+  if (iters_out) iters_out[i] = iters;
 }
 
 // Critical-surface diagnostics (cut-offs and resonances along the ray).

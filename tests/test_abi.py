@@ -119,6 +119,17 @@ def test_orbit_and_diagnostics_argument_checks_come_before_cuda(lib):
     assert lib.rt_trace_w(slab.handle, 1, 0, None, None, None, 0, 4, 1e-3, 1, None, None, None, None, None) == binding.RT_OK
     assert lib.rt_trace_w(slab.handle, 7, 0, None, None, None, 8, 4, 1e-3, 1, None, None, None, None, None) == binding.RT_ERR_INVALID
     assert lib.rt_launch_w(slab.handle, 1, 2, None, None, None, 8, None, None, None) == binding.RT_ERR_INVALID
+    kx = lambda eq=slab, disp=2, omega=1e11, n=8, it=50, tol=1e-15: lib.rt_launch_kx(
+        eq.handle if eq else None, disp, P(buf.ctypes.data), P(buf.ctypes.data), omega, None, n, it, tol,
+        P(buf.ctypes.data), None, None, None)
+    assert kx(eq=None) == binding.RT_ERR_INVALID
+    assert kx(eq=par, disp=1) == binding.RT_ERR_UNSUPPORTED
+    assert kx(omega=0.0) == binding.RT_ERR_INVALID
+    assert kx(n=-1) == binding.RT_ERR_INVALID
+    assert kx(it=-1) == binding.RT_ERR_INVALID and kx(it=1001) == binding.RT_ERR_INVALID
+    assert kx(tol=0.0) == binding.RT_ERR_INVALID and kx(tol=float("nan")) == binding.RT_ERR_INVALID
+    assert kx(n=0) == binding.RT_OK
+    assert kx() in (binding.RT_ERR_INVALID, binding.RT_ERR_CUDA)            # host pointers: no CPU fallback
     slab.close()
     par.close()
 
