@@ -144,7 +144,7 @@ def oracle_rate(cfg: int, target_s: float, n_threads: int = 0):
     avail = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
     cores = max(avail, oracle.max_threads()) if n_threads <= 0 else n_threads
     n_steps = inputs.FULL_SIZES[cfg][1]
-    probe_n = 8 * cores
+    probe_n = 64 * cores          # enough rays that every thread of the dynamic schedule (chunks of 16) is busy
     w = inputs.config(cfg, n_rays=probe_n, n_steps=n_steps)
     oeq = oracle.Equilibrium(w.eq)
     k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
