@@ -8,7 +8,7 @@ Reported per kernel:
 
 * ``instr``     FP-pipe instructions per ray-step (DFMA + DMUL + DADD + DSETP, or the FP32 analogues) -- what the FP64
                 (FP32) pipe has to issue, the quantity the kernels are optimised for;
-* ``rf3``       how many of them read THREE registers from the register file (constants, immediates, RZ and operands
+* ``rf3``       how many of them read THREE DISTINCT registers from the register file (constants, immediates, RZ and operands
                 served by the operand-reuse cache -- flagged ``.reuse`` in the same slot of the preceding instruction --
                 do not count).  Such an instruction occupies the FP64 pipe for 3 cycles instead of 2 (FP32: 1.56
                 instead of 1; ``rt_fma_peak_shape`` shape 2, profiles/r1_fma_peak_shapes.md), so the pipe time of a
@@ -77,12 +77,12 @@ def _rf3(ins, lo, hi, fp_ops):
         base = op.split(".")[0]
         srcs = ops[2:] if base.endswith("SETP") else ops[1:]
         if base in fp_ops:
-            reads = 0
-            for slot, o in enumerate(srcs):
-                m = _REG.match(o)
+            regs = set()                                    # distinct registers read from the register file: the same
+            for slot, o in enumerate(srcs):                 # register in two slots is read once (measured: fma(b, b, acc)
+                m = _REG.match(o)                           # runs at the full rate)
                 if m and reuse.get(slot) != m.group(1):
-                    reads += 1
-            n3 += reads >= 3
+                    regs.add(m.group(1))
+            n3 += len(regs) >= 3
         reuse = {}
         for slot, o in enumerate(ops[1:]):
             m = _REG.match(o)
