@@ -449,3 +449,29 @@ def test_fma_peak_shapes_order_as_documented(rt):
     assert r2 < r1 < r0, (r0, r1, r2)
     assert r3 / r0 > 0.93, (r0, r3)
     assert rt.fma_peak("f64", 50.0)[0] == pytest.approx(r0, rel=0.03)
+
+
+def test_calls_are_enqueued_on_the_callers_stream(rt, oracle):
+    """The ABI enqueues on the stream it is given and returns without synchronising (include/rt.h): two traces issued
+    back to back on two side streams give the results of the same calls on the default stream, bit for bit."""
+    import torch
+    jobs = []
+    for cfg, steps in ((4, 300), (2, 600)):
+        w, oeq, k0 = _workload(oracle, cfg, 4096 + 37, steps)
+        eq = rt.create_equilibrium(w.eq)
+        x0d, k0d = _dev(w.x0), _dev(k0)
+        ref = rt.trace(eq, w.disp, x0d, k0d, w.omega, steps, w.dt, 100, traj=True)
+        jobs.append((w, eq, x0d, k0d, steps, ref))
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = []
+    for (w, eq, x0d, k0d, steps, _), st in zip(jobs, streams):
+        st.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(st):
+            outs.append(rt.trace(eq, w.disp, x0d, k0d, w.omega, steps, w.dt, 100, traj=True))
+    for st in streams:
+        st.synchronize()
+    for (w, eq, _, _, _, ref), out in zip(jobs, outs):
+        for key in ("traj", "final", "residual", "status"):
+            assert torch.equal(out[key], ref[key]) or (key == "residual" and torch.equal(out[key].nan_to_num(), ref[key].nan_to_num()))
+        eq.close()
