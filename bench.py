@@ -47,14 +47,14 @@ UNIT = "ray-steps/s"
 # paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
 FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 259, (4, "f64"): 794, (5, "f64"): 1260,
                       (1, "f32"): 115, (2, "f32"): 115, (3, "f32"): 262, (4, "f32"): 798, (5, "f32"): 1257}
-FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f64"): 624, (5, "f64"): 888,
-                         (1, "f32"): 69, (2, "f32"): 69, (3, "f32"): 178, (4, "f32"): 538, (5, "f32"): 823}
+FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f64"): 624, (5, "f64"): 884,
+                         (1, "f32"): 69, (2, "f32"): 69, (3, "f32"): 178, (4, "f32"): 538, (5, "f32"): 819}
 # FP_RF3_PER_RAY_STEP: how many of those instructions read THREE DISTINCT registers from the register file.  Such an instruction
 # occupies the FP64 pipe for 3 cycles instead of 2 (FP32: 1.56 instead of 1) -- measured by rt_fma_peak_shape, shape 2
 # (profiles/r1_fma_peak_shapes.md) -- so the pipe time of a ray-step is (instr + RF3_EXTRA * rf3) issue slots of the FMA
 # microbenchmark; `pipe_model_frac` is that time over the measured kernel time.
 FP_RF3_PER_RAY_STEP = {(1, "f64"): 26, (2, "f64"): 26, (3, "f64"): 39, (4, "f64"): 169, (5, "f64"): 328,
-                       (1, "f32"): 29, (2, "f32"): 29, (3, "f32"): 39, (4, "f32"): 157, (5, "f32"): 272}
+                       (1, "f32"): 29, (2, "f32"): 29, (3, "f32"): 39, (4, "f32"): 157, (5, "f32"): 268}
 RF3_EXTRA = {"f64": 0.5, "f32": 0.563}      # shape 0 rate / shape 2 rate - 1:  63.9 / 42.7 = 1.50,  123.2 / 78.8 = 1.563
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}

@@ -443,11 +443,13 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
     return inside;
   }
   // EQ_GRID: bicubic psi(R,Z), cubic F(psi), n_e(psi)                                    (config 5)
-  bool inside = (R >= P.Rmin) && (R <= P.Rmax) && (Z >= P.Zmin) && (Z <= P.Zmax) && (R > T(0));
-  int iRc = (int)rt_floor((R - P.Rmin) * P.inv_hR), iZc = (int)rt_floor((Z - P.Zmin) * P.inv_hZ);
-  iRc = iRc < 0 ? 0 : (iRc > P.nRc - 1 ? P.nRc - 1 : iRc);
-  iZc = iZc < 0 ? 0 : (iZc > P.nZc - 1 ? P.nZc - 1 : iZc);
-  if (!inside) { iRc = 0; iZc = 0; }      // NaN positions convert to unspecified ints: keep the gather in bounds
+  // R > 0 is implied by R >= Rmin: rt_create_equilibrium requires Rmin > 0.  Inside the rectangle R - Rmin >= +0 exactly,
+  // so the cell index is >= 0 and only needs the upper clamp (R = Rmax belongs to the last cell); outside -- including NaN
+  // positions, which convert to unspecified ints -- the index is forced to 0 to keep the gather in bounds.
+  bool inside = (R >= P.Rmin) && (R <= P.Rmax) && (Z >= P.Zmin) && (Z <= P.Zmax);
+  int iRc = min((int)rt_floor((R - P.Rmin) * P.inv_hR), P.nRc - 1);
+  int iZc = min((int)rt_floor((Z - P.Zmin) * P.inv_hZ), P.nZc - 1);
+  if (!inside) { iRc = 0; iZc = 0; }
   const T dR = R - rt_fma(T(iRc), P.hR, P.Rmin), dZ = Z - rt_fma(T(iZc), P.hZ, P.Zmin);
   const int cell = iRc * P.nZc + iZc;
   gather.psi_select(P, cell);
@@ -469,8 +471,7 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
     psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
   }
   inside = inside && (psi >= P.psi_min) && (psi <= P.psi_max);
-  int iP = (int)rt_floor((psi - P.psi_min) * P.inv_hP);
-  iP = iP < 0 ? 0 : (iP > P.nPc - 1 ? P.nPc - 1 : iP);
+  int iP = min((int)rt_floor((psi - P.psi_min) * P.inv_hP), P.nPc - 1);      // same argument: psi >= psi_min when inside
   if (!inside) iP = 0;
   const T ds = psi - rt_fma(T(iP), P.hP, P.psi_min);
   T g[4], Ne, Nep;
