@@ -1,0 +1,101 @@
+"""Host logic of the product on CPU: the library's not-a-knot spline fit (csrc/spline_fit.cpp, run once per
+rt_create_equilibrium; reading A10) against scipy's CubicSpline / RectBivariateSpline and against the exactness
+properties of not-a-knot splines.  Compiled with g++ through a small shim (tests/spline_shim.cpp); no GPU, no oracle."""
+import ctypes
+import subprocess
+from pathlib import Path
+
+import numpy as np
+import pytest
+from scipy.interpolate import CubicSpline, RectBivariateSpline
+
+HERE = Path(__file__).resolve().parent
+CSRC = HERE.parent / "paper_2508_15967_b200" / "csrc"
+
+
+@pytest.fixture(scope="module")
+def shim(tmp_path_factory):
+    so = tmp_path_factory.mktemp("spline") / "libspline_shim.so"
+    subprocess.run(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", str(HERE / "spline_shim.cpp"),
+                    str(CSRC / "spline_fit.cpp"), "-o", str(so)], check=True)
+    lib = ctypes.CDLL(str(so))
+    P = ctypes.c_void_p
+    lib.shim_fit_cubic.argtypes = [P, P, ctypes.c_long, ctypes.c_int, P]
+    lib.shim_fit_bicubic.argtypes = [P, P, P, ctypes.c_int, ctypes.c_int, P]
+    return lib
+
+
+def _fit1(lib, x, y, stride=1):
+    pp = np.empty((len(x) - 1, 4))
+    assert lib.shim_fit_cubic(x.ctypes.data, y.ctypes.data, stride, len(x), pp.ctypes.data) == 0
+    return pp
+
+
+def _fit2(lib, R, Z, f):
+    pp = np.empty((len(R) - 1, len(Z) - 1, 4, 4))
+    assert lib.shim_fit_bicubic(R.ctypes.data, Z.ctypes.data, np.ascontiguousarray(f).ctypes.data, len(R), len(Z),
+                                pp.ctypes.data) == pp.size
+    return pp
+
+
+@pytest.mark.parametrize("n", [4, 5, 9, 257])
+def test_cubic_pieces_equal_scipy_not_a_knot(shim, n):
+    rng = np.random.default_rng(n)
+    x = np.linspace(0.0, 0.1977, n)
+    y = np.cos(7 * x) + 0.3 * rng.standard_normal(n)
+    pp = _fit1(shim, x, y)
+    ref = CubicSpline(x, y, bc_type="not-a-knot").c[::-1].T          # scipy stores the highest power first
+    scale = np.abs(ref).max(axis=0)
+    assert (np.abs(pp - ref).max(axis=0) / scale).max() < 1e-10
+
+
+def test_cubic_fit_reproduces_cubics_exactly_and_honours_the_stride(shim):
+    x = np.linspace(-1.0, 2.0, 17)
+    c = np.array([0.3, -1.2, 0.7, 2.1])
+    y2 = np.zeros((17, 3))
+    y2[:, 1] = c[0] + c[1] * x + c[2] * x**2 + c[3] * x**3
+    pp = _fit1(shim, x, np.ascontiguousarray(y2[:, 1]))
+    for i in range(16):                                               # Taylor coefficients of the cubic about x_i
+        xi = x[i]
+        tay = [c[0] + c[1] * xi + c[2] * xi**2 + c[3] * xi**3, c[1] + 2 * c[2] * xi + 3 * c[3] * xi**2,
+               c[2] + 3 * c[3] * xi, c[3]]
+        np.testing.assert_allclose(pp[i], tay, rtol=0, atol=2e-12)
+    yy = np.ascontiguousarray(y2)
+    pp_strided = np.empty((16, 4))
+    assert shim.shim_fit_cubic(x.ctypes.data, yy.ctypes.data + 8, 3, 17, pp_strided.ctypes.data) == 0
+    np.testing.assert_array_equal(pp_strided, pp)
+    assert shim.shim_fit_cubic(x.ctypes.data, yy.ctypes.data, 1, 3, pp_strided.ctypes.data) == -1      # n < 4
+
+
+def test_bicubic_pieces_against_scipy_and_polynomial_exactness(shim):
+    R = np.linspace(0.95, 2.45, 33)
+    Z = np.linspace(-0.75, 0.75, 29)
+    RR, ZZ = np.meshgrid(R, Z, indexing="ij")
+    f = np.log1p(2 * ((RR - 1.7) ** 2 + ZZ**2) / 0.36) * (1 + 1e-3 * np.cos(5 * RR) * np.sin(3 * ZZ))
+    pp = _fit2(shim, R, Z, f)
+    ref = RectBivariateSpline(R, Z, f, kx=3, ky=3, s=0)
+    rng = np.random.default_rng(1)
+    r = rng.uniform(R[0], R[-1], 4000)
+    z = rng.uniform(Z[0], Z[-1], 4000)
+    i = np.minimum(((r - R[0]) / (R[1] - R[0])).astype(int), len(R) - 2)
+    j = np.minimum(((z - Z[0]) / (Z[1] - Z[0])).astype(int), len(Z) - 2)
+    dr, dz = r - R[i], z - Z[j]
+    p = np.arange(4)
+
+    def ev(dp, dq):       # d^dp/dR^dp d^dq/dZ^dq of sum c[p][q] dR^p dZ^q
+        out = np.zeros_like(r)
+        for a in range(dp, 4):
+            for b in range(dq, 4):
+                fa = np.prod(np.arange(a, a - dp, -1)) if dp else 1.0
+                fb = np.prod(np.arange(b, b - dq, -1)) if dq else 1.0
+                out += pp[i, j, a, b] * fa * fb * dr ** (a - dp) * dz ** (b - dq)
+        return out
+
+    for dp, dq, tol in ((0, 0, 1e-13), (1, 0, 1e-11), (0, 1, 1e-11), (1, 1, 1e-10), (2, 0, 1e-9), (0, 2, 1e-9)):
+        np.testing.assert_allclose(ev(dp, dq), ref.ev(r, z, dx=dp, dy=dq), rtol=0, atol=tol * max(1.0, np.abs(f).max()))
+    # a bicubic polynomial is reproduced exactly by a not-a-knot tensor spline
+    poly = 0.4 - RR + 0.5 * ZZ + 0.3 * RR * ZZ**2 - 0.2 * RR**3 * ZZ + 0.1 * RR**3 * ZZ**3
+    pp = _fit2(shim, R, Z, poly)
+    val = sum(pp[i, j, a, b] * dr**a * dz**b for a in range(4) for b in range(4))
+    exact = 0.4 - r + 0.5 * z + 0.3 * r * z**2 - 0.2 * r**3 * z + 0.1 * r**3 * z**3
+    np.testing.assert_allclose(val, exact, rtol=0, atol=5e-13)
