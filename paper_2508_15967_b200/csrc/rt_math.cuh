@@ -68,6 +68,7 @@ struct Params {
   const T* prof_pp;             // [nPc][8]: F = sum f[m] ds^m (m = 0..3), then n_e/ne_scale likewise
 };
 
+RT_DEV int rt_imin(int a, int b) { return a < b ? a : b; }
 RT_DEV double rt_sqrt(double a) { return sqrt(a); }
 RT_DEV float rt_sqrt(float a) { return sqrtf(a); }
 RT_DEV double rt_pow(double a, double b) { return pow(a, b); }
@@ -447,8 +448,8 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
   // so the cell index is >= 0 and only needs the upper clamp (R = Rmax belongs to the last cell); outside -- including NaN
   // positions, which convert to unspecified ints -- the index is forced to 0 to keep the gather in bounds.
   bool inside = (R >= P.Rmin) && (R <= P.Rmax) && (Z >= P.Zmin) && (Z <= P.Zmax);
-  int iRc = min((int)rt_floor((R - P.Rmin) * P.inv_hR), P.nRc - 1);
-  int iZc = min((int)rt_floor((Z - P.Zmin) * P.inv_hZ), P.nZc - 1);
+  int iRc = rt_imin((int)rt_floor((R - P.Rmin) * P.inv_hR), P.nRc - 1);
+  int iZc = rt_imin((int)rt_floor((Z - P.Zmin) * P.inv_hZ), P.nZc - 1);
   if (!inside) { iRc = 0; iZc = 0; }
   const T dR = R - rt_fma(T(iRc), P.hR, P.Rmin), dZ = Z - rt_fma(T(iZc), P.hZ, P.Zmin);
   const int cell = iRc * P.nZc + iZc;
@@ -471,7 +472,7 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
     psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
   }
   inside = inside && (psi >= P.psi_min) && (psi <= P.psi_max);
-  int iP = min((int)rt_floor((psi - P.psi_min) * P.inv_hP), P.nPc - 1);      // same argument: psi >= psi_min when inside
+  int iP = rt_imin((int)rt_floor((psi - P.psi_min) * P.inv_hP), P.nPc - 1);      // same argument: psi >= psi_min when inside
   if (!inside) iP = 0;
   const T ds = psi - rt_fma(T(iP), P.hP, P.psi_min);
   T g[4], Ne, Nep;

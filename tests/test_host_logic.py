@@ -1,6 +1,9 @@
-"""Host logic of the product on CPU: the library's not-a-knot spline fit (csrc/spline_fit.cpp, run once per
-rt_create_equilibrium; reading A10) against scipy's CubicSpline / RectBivariateSpline and against the exactness
-properties of not-a-knot splines.  Compiled with g++ through a small shim (tests/spline_shim.cpp); no GPU, no oracle."""
+"""Host logic of the product on CPU, compiled with g++ through a small shim (tests/host_shim.cpp); no GPU, no oracle:
+
+* the library's not-a-knot spline fit (csrc/spline_fit.cpp, run once per rt_create_equilibrium; reading A10)
+  against scipy's CubicSpline / RectBivariateSpline and against the exactness properties of not-a-knot splines;
+* the per-call constant folding (csrc/rt_params.h, step a0 of the hot path) against the definitions of X, Y and n
+  (Eq. 6; L189) written out with scipy.constants."""
 import ctypes
 import subprocess
 from pathlib import Path
@@ -16,12 +19,13 @@ CSRC = HERE.parent / "paper_2508_15967_b200" / "csrc"
 @pytest.fixture(scope="module")
 def shim(tmp_path_factory):
     so = tmp_path_factory.mktemp("spline") / "libspline_shim.so"
-    subprocess.run(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", str(HERE / "spline_shim.cpp"),
+    subprocess.run(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", str(HERE / "host_shim.cpp"),
                     str(CSRC / "spline_fit.cpp"), "-o", str(so)], check=True)
     lib = ctypes.CDLL(str(so))
     P = ctypes.c_void_p
     lib.shim_fit_cubic.argtypes = [P, P, ctypes.c_long, ctypes.c_int, P]
     lib.shim_fit_bicubic.argtypes = [P, P, P, ctypes.c_int, ctypes.c_int, P]
+    lib.shim_fold_params.argtypes = [P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P]
     return lib
 
 
@@ -99,3 +103,40 @@ def test_bicubic_pieces_against_scipy_and_polynomial_exactness(shim):
     val = sum(pp[i, j, a, b] * dr**a * dz**b for a in range(4) for b in range(4))
     exact = 0.4 - r + 0.5 * z + 0.3 * r * z**2 - 0.2 * r**3 * z + 0.1 * r**3 * z**3
     np.testing.assert_allclose(val, exact, rtol=0, atol=5e-13)
+
+
+@pytest.mark.parametrize("fp32", [0, 1])
+def test_constant_folding_matches_the_definitions(shim, fp32):
+    """Step a0: X = wpe^2/w^2 = xs * shape, Y^2 = beta |B|^2, n = c k / w, ion terms through mu = Z m_e / m_i; the derived
+    constants of the reformulated stage (half gradients, field in units of sqrt(beta)) are consistent with them."""
+    import scipy.constants as sc
+    from paper_2508_15967_b200 import binding, inputs
+    w = inputs.config(4, n_rays=1)
+    desc, keep = binding.make_desc(w.eq)
+    out = np.empty(16)
+    rho_max = 0.98
+    shim.shim_fold_params(ctypes.addressof(desc), rho_max, w.omega, fp32, out.ctypes.data)
+    xs, xsh, beta, beta2, mu, mu2, opm, k2n, n2k, par_g, lin_gx, lin_gxh, sB0, sB0R0, tok_gxh, rmax2 = out
+    t = inputs.TOKAMAK
+    mD = sc.physical_constants["deuteron mass"][0]
+    rtol = 2e-7 if fp32 else 1e-9                 # CODATA numerals typed in three places agree to < 1e-9
+    assert xs == pytest.approx(t["n_ref"] * sc.e**2 / (sc.epsilon_0 * sc.m_e * w.omega**2), rel=rtol)
+    assert beta == pytest.approx((sc.e / (sc.m_e * w.omega)) ** 2, rel=rtol)
+    assert mu == pytest.approx(sc.m_e / mD, rel=rtol) and mu2 == pytest.approx(mu * mu, rel=rtol)
+    assert opm == pytest.approx(1 + mu, rel=rtol)
+    assert k2n == pytest.approx(sc.c / w.omega, rel=rtol) and k2n * n2k == pytest.approx(1.0, rel=rtol)
+    assert xsh == pytest.approx(0.5 * xs, rel=rtol) and beta2 == pytest.approx(2 * beta, rel=rtol)
+    assert sB0 == pytest.approx(np.sqrt(beta) * t["B0"], rel=rtol)
+    assert sB0R0 == pytest.approx(np.sqrt(beta) * t["B0"] * t["R0"], rel=rtol)
+    assert tok_gxh == pytest.approx(-t["p_exp"] * xs / t["a"] ** 2, rel=rtol)
+    assert rmax2 == pytest.approx((rho_max * t["a"]) ** 2, rel=rtol)
+    # slab constants
+    w3 = inputs.config(3, n_rays=1)
+    desc, keep = binding.make_desc(w3.eq)
+    shim.shim_fold_params(ctypes.addressof(desc), 0.98, w3.omega, fp32, out.ctypes.data)
+    xs3 = 5e19 * sc.e**2 / (sc.epsilon_0 * sc.m_e * w3.omega**2)
+    assert out[10] == pytest.approx(-xs3 / 0.5, rel=rtol) and out[11] == pytest.approx(-0.5 * xs3 / 0.5, rel=rtol)
+    w1 = inputs.config(1, n_rays=1)
+    desc, keep = binding.make_desc(w1.eq)
+    shim.shim_fold_params(ctypes.addressof(desc), 0.98, w1.omega, fp32, out.ctypes.data)
+    assert out[0] == pytest.approx(0.5, rel=rtol) and out[9] == pytest.approx(0.5 / 1.0**2, rel=rtol)    # X = 1/2 (1 + r^2/L^2)
