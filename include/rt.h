@@ -15,8 +15,10 @@
  * Conventions
  *   - All functions return RT_OK (0) or a negative RT_ERR_* code; they never throw and never abort.
  *     rt_last_error() returns a thread-local message for the last non-zero return on the calling thread.
- *   - "DEVICE" pointers are CUDA device pointers on the current device, 16-byte aligned, owned by the caller
- *     (e.g. PyTorch tensors); buffers must not alias.  "HOST" pointers are ordinary host memory.
+ *   - "DEVICE" pointers are CUDA device pointers on the current device, owned by the caller (e.g. PyTorch tensors);
+ *     buffers must not alias.  Inputs need the alignment of their element type; the sample outputs of rt_trace /
+ *     rt_trace_w / rt_orbit (out_traj, out_final, out_residual / out_drift) must be 16-byte aligned: they are written
+ *     with 128-bit stores.  "HOST" pointers are ordinary host memory.
  *   - Ray arrays are structure-of-arrays: x0[c*n_rays + i], c = 0..2 (x, y, z), i = ray.
  *   - Element type of every ray buffer follows `precision`: double for RT_F64, float for RT_F32.
  *   - Units are the paper's: x [m], k [rad/m], w [rad/s].  The step `dt` is given in tau = c*t metres

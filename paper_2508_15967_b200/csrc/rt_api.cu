@@ -35,8 +35,6 @@ int cuda_fail(cudaError_t e, const char* what) {
     if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
   } while (0)
 
-bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
-
 }  // namespace
 
 // ---- the handle ---------------------------------------------------------------------------------------------------
@@ -215,9 +213,12 @@ int check_trace_args(const rt_equilibrium* eq, int disp, int precision, const vo
   return RT_OK;
 }
 
-int require_device_ptr(const void* p, const char* name, bool may_be_null) {
+// align: input arrays and the scalar outputs of the diagnostic kernels are read / written element by element and need the
+// alignment of their element type; the sample outputs of rt_trace / rt_orbit are written with 128-bit stores (16).
+int require_device_ptr(const void* p, const char* name, bool may_be_null, size_t align = 8) {
   if (!p) return may_be_null ? RT_OK : fail(RT_ERR_INVALID, std::string(name) + " is NULL");
-  if (!aligned16(p)) return fail(RT_ERR_INVALID, std::string(name) + " is not 16-byte aligned");
+  if (reinterpret_cast<uintptr_t>(p) & (align - 1))
+    return fail(RT_ERR_INVALID, std::string(name) + " is not " + std::to_string(align) + "-byte aligned");
   cudaPointerAttributes at;
   cudaError_t e = cudaPointerGetAttributes(&at, p);
   if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cudaPointerGetAttributes"); }
@@ -380,9 +381,11 @@ int rt_trace(const rt_equilibrium* eq, int disp, int precision, const void* x0, 
   int rc = check_trace_args(eq, disp, precision, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj);
   if (rc) return rc;
   if (n_rays == 0) return RT_OK;
-  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(k0, "k0", false)) ||
-      (rc = require_device_ptr(out_traj, "out_traj", true)) || (rc = require_device_ptr(out_final, "out_final", true)) ||
-      (rc = require_device_ptr(out_residual, "out_residual", true)) || (rc = require_device_ptr(out_status, "out_status", true)))
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  if ((rc = require_device_ptr(x0, "x0", false, es)) || (rc = require_device_ptr(k0, "k0", false, es)) ||
+      (rc = require_device_ptr(out_traj, "out_traj", true, 16)) || (rc = require_device_ptr(out_final, "out_final", true, 16)) ||
+      (rc = require_device_ptr(out_residual, "out_residual", true, 16)) ||
+      (rc = require_device_ptr(out_status, "out_status", true, 4)))
     return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (precision == RT_F64)
@@ -396,10 +399,12 @@ int rt_trace_w(const rt_equilibrium* eq, int disp, int precision, const void* x0
   int rc = check_trace_args(eq, disp, precision, x0, k0, 1.0, n_rays, n_steps, dt, save_stride, out_traj);
   if (rc) return rc;
   if (n_rays == 0) return RT_OK;
-  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(k0, "k0", false)) ||
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  if ((rc = require_device_ptr(x0, "x0", false, es)) || (rc = require_device_ptr(k0, "k0", false, es)) ||
       (rc = require_device_ptr(omega, "omega", false)) ||
-      (rc = require_device_ptr(out_traj, "out_traj", true)) || (rc = require_device_ptr(out_final, "out_final", true)) ||
-      (rc = require_device_ptr(out_residual, "out_residual", true)) || (rc = require_device_ptr(out_status, "out_status", true)))
+      (rc = require_device_ptr(out_traj, "out_traj", true, 16)) || (rc = require_device_ptr(out_final, "out_final", true, 16)) ||
+      (rc = require_device_ptr(out_residual, "out_residual", true, 16)) ||
+      (rc = require_device_ptr(out_status, "out_status", true, 4)))
     return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (precision == RT_F64)
@@ -422,9 +427,10 @@ int rt_orbit(const rt_equilibrium* eq, int precision, const void* x0, const void
     return fail(RT_ERR_INVALID, "n_steps must be a multiple of save_stride when out_traj is given");
   if (n == 0) return RT_OK;
   int rc;
-  if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(v0, "v0", false)) ||
-      (rc = require_device_ptr(out_traj, "out_traj", true)) || (rc = require_device_ptr(out_final, "out_final", true)) ||
-      (rc = require_device_ptr(out_drift, "out_drift", true)) || (rc = require_device_ptr(out_status, "out_status", true)))
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  if ((rc = require_device_ptr(x0, "x0", false, es)) || (rc = require_device_ptr(v0, "v0", false, es)) ||
+      (rc = require_device_ptr(out_traj, "out_traj", true, 16)) || (rc = require_device_ptr(out_final, "out_final", true, 16)) ||
+      (rc = require_device_ptr(out_drift, "out_drift", true, 16)) || (rc = require_device_ptr(out_status, "out_status", true, 4)))
     return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (precision == RT_F64)
@@ -543,7 +549,7 @@ int rt_launch_kx(const rt_equilibrium* eq, int disp, const double* x0, const dou
   if (n == 0) return RT_OK;
   if ((rc = require_device_ptr(x0, "x0", false)) || (rc = require_device_ptr(k_guess, "k_guess", false)) ||
       (rc = require_device_ptr(omega_rays, "omega_rays", true)) || (rc = require_device_ptr(k0, "k0", false)) ||
-      (rc = require_device_ptr(D_out, "D_out", true)) || (rc = require_device_ptr(iters_out, "iters_out", true)))
+      (rc = require_device_ptr(D_out, "D_out", true)) || (rc = require_device_ptr(iters_out, "iters_out", true, 4)))
     return rc;
   const rt::Params<double> P = make_params<double>(eq, omega_rays ? kOmegaRefPerRay : omega);
   return launch_launch_kx(eq, disp, P, x0, k_guess, omega_rays, kOmegaRefPerRay, n, max_iter, tol, k0, D_out, iters_out,
@@ -588,9 +594,10 @@ int rt_rhs(const rt_equilibrium* eq, int disp, int precision, const void* x, con
   if ((rc = check_omega(omega))) return rc;
   if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
   if (n == 0) return RT_OK;
-  if ((rc = require_device_ptr(x, "x", false)) || (rc = require_device_ptr(k, "k", false)) ||
-      (rc = require_device_ptr(D_out, "D_out", true)) || (rc = require_device_ptr(rhs_out, "rhs_out", true)) ||
-      (rc = require_device_ptr(inside_out, "inside_out", true)))
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  if ((rc = require_device_ptr(x, "x", false, es)) || (rc = require_device_ptr(k, "k", false, es)) ||
+      (rc = require_device_ptr(D_out, "D_out", true, es)) || (rc = require_device_ptr(rhs_out, "rhs_out", true, es)) ||
+      (rc = require_device_ptr(inside_out, "inside_out", true, 4)))
     return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (precision == RT_F64)
@@ -604,8 +611,9 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
   if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
   if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
   int rc;
-  if ((rc = require_device_ptr(out, "out", false)) || (rc = require_device_ptr(residual, "residual", true)) ||
-      (rc = require_device_ptr(status, "status", true)))
+  if ((rc = require_device_ptr(out, "out", false)) ||
+      (rc = require_device_ptr(residual, "residual", true, (precision == RT_F64) ? 8 : 4)) ||
+      (rc = require_device_ptr(status, "status", true, 4)))
     return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   RT_CUDA(cudaMemsetAsync(out, 0, 6 * sizeof(double), st));

@@ -475,3 +475,27 @@ def test_calls_are_enqueued_on_the_callers_stream(rt, oracle):
         for key in ("traj", "final", "residual", "status"):
             assert torch.equal(out[key], ref[key]) or (key == "residual" and torch.equal(out[key].nan_to_num(), ref[key].nan_to_num()))
         eq.close()
+
+
+@pytest.mark.parametrize("cfg,prec", [(4, "f64"), (5, "f64"), (2, "f32")])
+def test_resuming_from_the_final_state(rt, oracle, cfg, prec):
+    """SURVEY section 5 (checkpoint / resume): the state carried between launches is (x, k) itself, so tracing N steps in
+    two launches -- the second started straight from the rows of the first one's out_final, which for an odd ray count are
+    only element-aligned (inputs need no more, include/rt.h) -- reproduces the N-step result.  k makes the round trip
+    n -> k -> n through one multiplication each way, which re-rounds it once; the perturbation then grows like any other
+    (pin P12), so the test allows a few hundred ulp and requires equal status."""
+    import torch
+    w, oeq, k0 = _workload(oracle, cfg, 2048 + 5, 400)
+    eq = rt.create_equilibrium(w.eq)
+    x0d, k0d = _dev(w.x0, prec), _dev(k0, prec)
+    full = rt.trace(eq, w.disp, x0d, k0d, w.omega, 400, w.dt)
+    a = rt.trace(eq, w.disp, x0d, k0d, w.omega, 150, w.dt)
+    assert a["final"][3:].data_ptr() % 16 != 0                     # 2053 rays: the k rows are not 16-byte aligned
+    b = rt.trace(eq, w.disp, a["final"][:3], a["final"][3:], w.omega, 250, w.dt)
+    torch.cuda.synchronize()
+    assert torch.equal(b["status"], full["status"])
+    fa, fb = _host(full["final"]), _host(b["final"])
+    eps = np.finfo(np.float64 if prec == "f64" else np.float32).eps
+    scale = np.maximum(np.abs(fa).max(axis=1, keepdims=True), 1e-300)      # config 2: z and k_z are identically zero
+    assert (np.abs(fa - fb) / scale).max() < 2000 * eps
+    eq.close()
