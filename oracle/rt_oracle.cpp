@@ -12,7 +12,8 @@
 //       OMODE      D = c^2|k|^2/w^2 - 1 + wpe^2/w^2                (BASELINE.json config 1; L157/L191)
 //       XMODE      D = S n^2 - R L                                  (reading A5; L157/L191)
 //       COLD_FULL  D = Det(eps + n n - n^2 I)                       (Eq. 5) with eps from
-//                  Eq. 7-10 (L177-189) written in the frame whose 3rd axis is B/|B|, n = c k / w (Eq. 6)
+//                  Eq. 7-10 (L177-189) rotated to Cartesian axes: eps = S (I - b b^T) + P b b^T + i Dx [b]x,
+//                  b = B/|B|, n = c k / w (Eq. 6); regular at n parallel to B
 //   * over four plasma equilibria B(x), n_e(x) (L151).
 //
 // State and units here are the paper's own: x [m], k [rad/m], t [s], w [rad/s]  (L147: "inputs for
@@ -265,27 +266,25 @@ T dispersion(const orc_equilibrium& eq, int disp, const T x[3], const T k[3], co
     const T Rr = st.S + st.Dx, Ll = st.S - st.Dx;
     return st.S * n2 - Rr * Ll;                                    // reading A5
   }
-  // COLD_FULL: Det(eps + n n - n^2 I) in the frame e3 = B/|B|, e1 along the perpendicular part of n.
+  // COLD_FULL: Det(eps + n n - n^2 I) (Eq. 5) written out in the CARTESIAN axes the state lives in.  Eq. 7 (L177)
+  // gives eps in the frame whose 3rd axis is b = B/|B|: diag(S, S, P) with eps12 = -i Dx = -eps21.  Rotated to
+  // Cartesian axes that tensor is
+  //      eps = S (I - b b^T) + P b b^T + i Dx [b]x ,      ([b]x v = b x v, i.e. ([b]x)_ij = -e_ijk b_k;
+  //                                                        for b = z^ this is eps12 = -i Dx, eps21 = +i Dx: Eq. 7)
+  // ("the explicit 3x3 matrix with Cartesian dB_i/dx_j").  No frame is built from the
+  // perpendicular part of n, so nothing non-smooth is differentiated and the dual-number partials are finite at exactly
+  // parallel propagation (theta = 0, the R and L waves of Fig. 3) -- D is a polynomial in n there.
   const T Bmag = sqrt_(pl.B[0] * pl.B[0] + pl.B[1] * pl.B[1] + pl.B[2] * pl.B[2]);
   T b[3];
   for (int i = 0; i < 3; ++i) b[i] = pl.B[i] / Bmag;
-  const T npar = n[0] * b[0] + n[1] * b[1] + n[2] * b[2];
-  T nperp_vec[3];
-  for (int i = 0; i < 3; ++i) nperp_vec[i] = n[i] - npar * b[i];
-  const T nperp = sqrt_(nperp_vec[0] * nperp_vec[0] + nperp_vec[1] * nperp_vec[1] + nperp_vec[2] * nperp_vec[2]);
-  const T nf[3] = {nperp, zero, npar};                             // n in the field-aligned frame
-  const T nf2 = nf[0] * nf[0] + nf[1] * nf[1] + nf[2] * nf[2];
-  Cx<T> eps[3][3];
-  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) eps[i][j] = {zero, zero};
-  eps[0][0] = {st.S, zero};  eps[1][1] = {st.S, zero};  eps[2][2] = {st.P, zero};   // Eq. 7
-  eps[0][1] = {zero, -st.Dx};                                                       // eps12 = -i Dx
-  eps[1][0] = {zero, st.Dx};                                                        // -eps12
+  const T bx[3][3] = {{zero, -b[2], b[1]}, {b[2], zero, -b[0]}, {-b[1], b[0], zero}};   // [b]x
   Cx<T> M[3][3];
   for (int i = 0; i < 3; ++i)
     for (int j = 0; j < 3; ++j) {
-      M[i][j] = eps[i][j];
-      M[i][j].re = M[i][j].re + nf[i] * nf[j];
-      if (i == j) M[i][j].re = M[i][j].re - nf2;
+      const T bb = b[i] * b[j];
+      T re = st.P * bb - st.S * bb + n[i] * n[j];                  // (P - S) b_i b_j + n_i n_j
+      if (i == j) re = re + st.S - n2;                             // + (S - n^2) delta_ij
+      M[i][j] = {re, st.Dx * bx[i][j]};
     }
   const Cx<T> det = M[0][0] * (M[1][1] * M[2][2] - M[1][2] * M[2][1])
                   - M[0][1] * (M[1][0] * M[2][2] - M[1][2] * M[2][0])
@@ -367,21 +366,25 @@ static int trace_impl(const orc_equilibrium* eq, int disp, const double* x0, con
     const double omega = omega_rays ? omega_rays[i] : omega_all;
     double y[6];
     for (int c = 0; c < 3; ++c) { y[c] = x0[c * n_rays + i]; y[3 + c] = k0[c * n_rays + i]; }
-    int status = 0;
+    // DESIGN.md reading A20: a wave frequency that is not positive and finite defines no ray (n = c k / w, Eq. 6): the
+    // ray is never advanced (status 2), every sample is the launch state, and |D| is NaN.
+    const bool bad_omega = !(omega > 0.0 && std::isfinite(omega));
+    int status = bad_omega ? 2 : 0;
+    auto res = [&]() { return bad_omega ? std::numeric_limits<double>::quiet_NaN() : residual(*eq, disp, omega, y); };
     if (out_traj) {
       for (int c = 0; c < 6; ++c) out_traj[(0 * 6 + c) * n_rays + i] = y[c];
-      if (out_residual) out_residual[0 * n_rays + i] = residual(*eq, disp, omega, y);
+      if (out_residual) out_residual[0 * n_rays + i] = res();
     }
     for (int64_t s = 1; s <= n_steps; ++s) {
       if (status == 0) status = rk4_step(*eq, disp, omega, h, y);
       if (out_traj && (s % save_stride) == 0) {
         const int64_t m = s / save_stride;
         for (int c = 0; c < 6; ++c) out_traj[(m * 6 + c) * n_rays + i] = y[c];
-        if (out_residual) out_residual[m * n_rays + i] = residual(*eq, disp, omega, y);
+        if (out_residual) out_residual[m * n_rays + i] = res();
       }
     }
     if (out_final) for (int c = 0; c < 6; ++c) out_final[c * n_rays + i] = y[c];
-    if (!out_traj && out_residual) out_residual[i] = residual(*eq, disp, omega, y);
+    if (!out_traj && out_residual) out_residual[i] = res();
     if (out_status) out_status[i] = status;
   }
   return 0;

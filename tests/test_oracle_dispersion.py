@@ -115,6 +115,14 @@ def test_cold_full_equals_numpy_determinant_and_biquadratic(oracle):
         C = P * (S * S - Dx * Dx)
         n2 = n @ n
         assert D[i] == pytest.approx(A * n2 * n2 - Bq * n2 + C, abs=2e-13)
+        # Eq. 7 literally, in its own frame (e1, e2 = b x e1, e3 = b) with e1 along the perpendicular part of n:
+        # eps = [[S, -iDx, 0], [iDx, S, 0], [0, 0, P]], n = (n_perp, 0, n_par)
+        npar = n @ b
+        nperp = np.linalg.norm(n - npar * b)
+        nf = np.array([nperp, 0.0, npar])
+        eps_f = np.array([[S, -1j * Dx, 0], [1j * Dx, S, 0], [0, 0, P]])
+        det_f = np.linalg.det(eps_f + np.outer(nf, nf) - (nf @ nf) * np.eye(3))
+        assert D[i] == pytest.approx(det_f.real, abs=2e-13)
 
 
 def test_cold_full_roots_at_special_angles_and_appleton_hartree(oracle):
@@ -213,6 +221,56 @@ def test_dual_number_gradients_match_central_differences(oracle, case):
             fd = (oracle.dispersion_value(eq, disp, x, k, w + h) - oracle.dispersion_value(eq, disp, x, k, w - h)) / (2 * h)
         err = np.abs(fd - g[j]) / scale[j]
         assert err.max() < 2e-7, (case, j, err.max())
+
+
+@pytest.mark.parametrize("eqname", ["slab", "tok", "grid"])
+@pytest.mark.parametrize("sign", [+1.0, -1.0])
+def test_gradients_at_exactly_parallel_propagation(oracle, eqname, sign):
+    """P4 at theta = 0 (k = +-|k| B/|B|, the R and L waves of Fig. 3): D (Eq. 5) is a polynomial in n, so all 7
+    partials are finite there and equal central differences of the plain-double D.  (A determinant written in a frame
+    built from the perpendicular part of n differentiates sqrt(n_perp^2) at 0 and returns NaN: VERDICT r1 weak 1.)"""
+    n = 16
+    rng = np.random.default_rng(43)
+    if eqname == "slab":
+        eq, w = _slab_eq(), 60 * GHZ
+        x = np.stack([rng.uniform(2.19, 2.29, n), rng.uniform(-0.2, 0.2, n), rng.uniform(-0.1, 0.1, n)])
+    elif eqname == "tok":
+        eq, w = _tok_eq(), 110 * GHZ
+        x, _ = _tok_points(n, seed=47)
+    else:
+        eq, w = oracle.Equilibrium(_grid_eq_small()), 110 * GHZ
+        x, _ = _tok_points(n, seed=53, rho_lo=0.2, rho_hi=0.85)
+    B = oracle.plasma(eq, x, w)[1]
+    b = B / np.linalg.norm(B, axis=0)
+    if eqname == "slab":
+        assert np.array_equal(b[:2], np.zeros((2, n))) and np.all(b[2] == 1.0)       # k along z^ exactly
+    k = sign * b * rng.uniform(0.3, 1.1, n) * w / sc.c
+    D, g, ins = oracle.dispersion(eq, "cold_full", x, k, w)
+    assert ins.all() and np.isfinite(D).all() and np.isfinite(g).all()
+    grp = [np.abs(g[0:3]).max(), np.abs(g[3:6]).max(), np.abs(g[6]).max()]
+    for j in range(7):
+        scale = np.maximum(np.abs(g[j]), 1e-3 * grp[min(j // 3, 2)])
+        if j < 3:
+            h = 1e-6
+            xp, xm = x.copy(), x.copy()
+            xp[j] += h
+            xm[j] -= h
+            fd = (oracle.dispersion_value(eq, "cold_full", xp, k, w) - oracle.dispersion_value(eq, "cold_full", xm, k, w)) / (2 * h)
+        elif j < 6:
+            h = 1e-6 * w / sc.c
+            kp, km = k.copy(), k.copy()
+            kp[j - 3] += h
+            km[j - 3] -= h
+            fd = (oracle.dispersion_value(eq, "cold_full", x, kp, w) - oracle.dispersion_value(eq, "cold_full", x, km, w)) / (2 * h)
+        else:
+            h = 1e-6 * w
+            fd = (oracle.dispersion_value(eq, "cold_full", x, k, w + h) - oracle.dispersion_value(eq, "cold_full", x, k, w - h)) / (2 * h)
+        err = np.abs(fd - g[j]) / scale
+        assert err.max() < 2e-7, (eqname, sign, j, err.max())
+    # the group velocity of a parallel wave in a slab is along B: dD/dk has no component across z^ (k_x = k_y = 0
+    # makes D even in k_x and k_y separately)
+    if eqname == "slab":
+        assert np.abs(g[3:5]).max() == 0.0
 
 
 def test_omega_derivative_closed_form_omode(oracle):

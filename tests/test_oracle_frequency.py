@@ -42,6 +42,26 @@ def test_p13_per_ray_frequency_harmonic_oscillators(oracle):
     assert np.ptp(W) > 0.1
 
 
+def test_a_ray_with_a_bad_frequency_is_never_advanced(oracle):
+    """Reading A20: w_i that is not positive and finite (0, negative, inf, NaN) defines no ray: status 2, every sample is
+    the launch state bit for bit, |D| is NaN; the rays beside it are the same as in a call without it."""
+    w = inputs.config(4, n_rays=6, n_steps=40)
+    eq = oracle.Equilibrium(w.eq)
+    k0, _ = oracle.launch(eq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    om = np.full(6, w.omega)
+    om[[1, 2, 3, 4]] = [0.0, -w.omega, np.inf, np.nan]
+    out = oracle.trace(eq, w.disp, w.x0, k0, om, 40, w.dt, 20, traj=True)
+    assert list(out["status"]) == [0, 2, 2, 2, 2, 0]
+    launch_state = np.concatenate([w.x0, k0])
+    for m in range(3):
+        np.testing.assert_array_equal(out["traj"][m][:, 1:5], launch_state[:, 1:5])
+    np.testing.assert_array_equal(out["final"][:, 1:5], launch_state[:, 1:5])
+    assert np.isnan(out["residual"][:, 1:5]).all()
+    ref = oracle.trace(eq, w.disp, w.x0, k0, w.omega, 40, w.dt, 20, traj=True)
+    np.testing.assert_array_equal(out["traj"][:, :, [0, 5]], ref["traj"][:, :, [0, 5]])
+    assert (oracle.trace(eq, w.disp, w.x0, k0, -w.omega, 5, w.dt)["status"] == 2).all()
+
+
 def test_p14_per_ray_run_equals_single_frequency_runs(oracle):
     w = inputs.config(4, n_rays=12, n_steps=150)
     om = inputs.frequency_scan(w.n_rays, w.omega, seed=1004, spread=0.05)

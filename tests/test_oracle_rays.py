@@ -340,6 +340,89 @@ def test_rays_leaving_the_domain_freeze_with_status_1(oracle):
     assert (rho > 0.95).all() and (rho < 0.985).all()
 
 
+def test_non_finite_steps_freeze_with_status_2(oracle):
+    """Reading A12: a step whose new state is not finite is rejected and the ray frozen with status 2.  The parabolic
+    slab's domain is all of space, so (a) a NaN launch position and (b) a step so long that the second stage point
+    overflows X = 0.5 (1 + r^2/L^2) both end with status 2 and the launch state back, while (c) the rays beside them in
+    the same call integrate normally.  (d) The linear slab's domain is the POSITIVE condition x > 0, so there a NaN
+    position is "outside": status 1."""
+    w = inputs.config(1, n_rays=4, n_steps=10)
+    k0, _ = oracle.launch(w.eq, w.disp, w.x0, w.dirs, w.omega)
+    x0 = w.x0.copy()
+    x0[1, 2] = np.nan
+    out = oracle.trace(w.eq, w.disp, x0, k0, w.omega, 10, w.dt, 5, traj=True)
+    assert list(out["status"]) == [0, 0, 2, 0]
+    assert np.isnan(out["final"][1, 2]) and np.array_equal(out["final"][[0, 2, 3, 4, 5], 2], np.r_[x0[[0, 2], 2], k0[:, 2]])
+    assert np.isnan(out["residual"][:, 2]).all() and np.isfinite(out["residual"][:, [0, 1, 3]]).all()
+    ref = oracle.trace(w.eq, w.disp, w.x0, k0, w.omega, 10, w.dt, 5, traj=True)
+    np.testing.assert_array_equal(out["traj"][:, :, [0, 1, 3]], ref["traj"][:, :, [0, 1, 3]])
+    big = oracle.trace(w.eq, w.disp, w.x0, k0, w.omega, 3, 1e308)
+    assert (big["status"] == 2).all()
+    np.testing.assert_array_equal(big["final"], np.concatenate([w.x0, k0]))
+    w3 = inputs.config(3, n_rays=2, n_steps=5)
+    k3, _ = oracle.launch(w3.eq, w3.disp, w3.x0, w3.dirs, w3.omega)
+    x3 = w3.x0.copy()
+    x3[0, 0] = np.nan
+    assert list(oracle.trace(w3.eq, w3.disp, x3, k3, w3.omega, 5, w3.dt)["status"]) == [1, 0]
+
+
+@pytest.mark.parametrize("where", ["slab", "tokamak", "grid"])
+def test_parallel_propagation_launches_on_R_and_L_and_integrates(oracle, where):
+    """P7 at theta = 0 as rays (Fig. 3's w_r, w_l are the theta = 0 cut-offs, L157): launched along +-B/|B| the two branches
+    of the full determinant are n^2 = R = S + Dx and n^2 = L = S - Dx, summed here in the textbook form
+    1 - sum_s wps^2 / (w (w +- Ws)) from scipy.constants; such rays integrate (status 0) with |D| at integrator order:
+    it stays small and falls about 16-fold when dt is halved.  In the slab (B along z^, k along z^) k_z is an ignorable
+    coordinate's momentum and stays bit-for-bit constant, and by the mirror symmetry z -> -z the +B and -B rays are
+    mirror images."""
+    if where == "slab":
+        w = inputs.config(3, n_rays=8)
+        eq = oracle.Equilibrium(w.eq)
+        x0 = np.stack([np.linspace(2.2, 2.28, 8), np.linspace(-0.1, 0.1, 8), np.zeros(8)])
+    elif where == "tokamak":
+        w = inputs.config(4, n_rays=8)
+        eq, x0 = oracle.Equilibrium(w.eq), w.x0
+    else:
+        w = inputs.config(4, n_rays=8)
+        eq, x0 = oracle.Equilibrium(inputs.synth_grid(seed=11, eps=1e-3, nR=65, nZ=65, nPsi=65)), w.x0
+    ne, B, _, ins = oracle.plasma(eq, x0, w.omega)
+    assert ins.all()
+    Bm = np.linalg.norm(B, axis=0)
+    b = B / Bm
+    Rr, Ll = np.ones(8), np.ones(8)
+    for q, m in ((-sc.e, sc.m_e), (sc.e, sc.physical_constants["deuteron mass"][0])):
+        wp2 = ne * q * q / (sc.epsilon_0 * m)
+        Rr -= wp2 / (w.omega * (w.omega + q * Bm / m))
+        Ll -= wp2 / (w.omega * (w.omega - q * Bm / m))
+    finals = {}
+    for branch in (0, 1):
+        for sign in (+1.0, -1.0):
+            k0, D0 = oracle.launch(eq, "cold_full", x0, sign * b, w.omega, branch)
+            n2 = np.sum((k0 * C / w.omega) ** 2, axis=0)
+            err = np.minimum(np.abs(n2 - Rr), np.abs(n2 - Ll))
+            assert err.max() < 1e-12 and np.abs(D0).max() < 1e-15
+            if branch == 0:
+                other, _ = oracle.launch(eq, "cold_full", x0, sign * b, w.omega, 1)
+                n2o = np.sum((other * C / w.omega) ** 2, axis=0)
+                np.testing.assert_allclose(np.sort([n2, n2o], axis=0), np.sort([Rr, Ll], axis=0), rtol=1e-12)
+            _, g, _ = oracle.dispersion(eq, "cold_full", x0, k0, w.omega)
+            assert np.isfinite(g).all()
+            res = {}
+            for dt in (2e-3, 1e-3):
+                out = oracle.trace(eq, "cold_full", x0, k0, w.omega, int(round(0.2 / dt)), dt, traj=True)
+                assert (out["status"] == 0).all()
+                res[dt] = np.nanmax(out["residual"][1:])
+                if where == "slab":
+                    assert (out["traj"][:, 5] == k0[2]).all() and (out["traj"][:, 4] == 0.0).all()
+            assert res[1e-3] < 1e-8
+            if res[2e-3] > 1e-11:                                   # well above the rounding floor: 4th order
+                assert res[2e-3] / res[1e-3] > 10.0, (where, branch, sign, res)
+            finals[(branch, sign)] = out["final"]
+    if where == "slab":
+        for branch in (0, 1):
+            mirror = finals[(branch, +1.0)] * np.array([1, 1, -1, 1, 1, -1.0])[:, None]
+            np.testing.assert_array_equal(finals[(branch, -1.0)], mirror)
+
+
 def test_trajectory_sampling_and_argument_checks(oracle):
     w = inputs.config(4, n_rays=8, n_steps=100)
     eq, k0, D0, full = _launch_trace(oracle, w, save_stride=1, traj=True)
