@@ -253,7 +253,13 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
   }
   __shared__ __align__(16) T stage[7 * BLOCK];
   Params<T> Pw;                                    // PW only: this ray's own copy of the w-dependent constants
-  if constexpr (PW) Pw = params_at_frequency(P0, valid ? A.omega_ref / A.omega[i] : 1.0);
+  bool bad_w = false;                              // PW only: w_i not positive and finite defines no ray (reading A20):
+  if constexpr (PW) {                              // status 2, never advanced, launch state back bit for bit, |D| = NaN
+    const double wi = valid ? A.omega[i] : A.omega_ref;
+    bad_w = !(wi > 0.0 && wi < __longlong_as_double(0x7ff0000000000000LL));
+    Pw = params_at_frequency(P0, bad_w ? 1.0 : A.omega_ref / wi);
+    if (bad_w) { Pw.k2n = T(1); Pw.n2k = T(1); }
+  }
   const Params<T>& P = PW ? Pw : P0;
   T y[6];
 #pragma unroll
@@ -261,7 +267,7 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
     y[c] = valid ? A.x0[c * N + i] : T(0);
     y[3 + c] = valid ? A.k0[c * N + i] * P.k2n : T(0);          // n = c k / w  (Eq. 6)
   }
-  int status = valid ? 0 : 3;                      // 3: padding lane of the last block, never stored
+  int status = valid ? (bad_w ? 2 : 0) : 3;        // 3: padding lane of the last block, never stored
   // Everything the store needs is recomputed here from threadIdx / the kernel arguments, so that nothing of it stays
   // live across the step loop (the loop is register-bound).
   auto save = [&](T* rows6, T* res_row) {
@@ -274,7 +280,8 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
     T v[6];
 #pragma unroll
     for (int c = 0; c < 3; ++c) { v[c] = y[c]; v[3 + c] = y[3 + c] * P.n2k; }
-    const T r = res_row ? abs_residual<T, EQ, DISP>(P, y, gather) : T(0);
+    T r = res_row ? abs_residual<T, EQ, DISP>(P, y, gather) : T(0);
+    if (PW && bad_w) r = rt_nan<T>();
     out.store(rows6, res_row, v, r, out.i0 + out.lane < A.n_rays);
   };
   // Sample m = state after m * stride steps (sample 0 = launch state).  The inner loop holds the step and nothing else.

@@ -93,12 +93,36 @@ def test_per_ray_frequency_argument_errors(rt, oracle):
         rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), _dev(np.full(15, w.omega)), 5, w.dt)          # wrong length
     with pytest.raises(ValueError):
         rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), torch.full((16,), w.omega), 5, w.dt)           # host tensor
-    # a non-positive frequency makes that ray (only) non-finite: status 2, as in the oracle
-    om = np.full(16, w.omega)
-    om[3] = 0.0
-    ref = oracle.trace(w.eq, w.disp, w.x0, k0, om, 5, w.dt)
-    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), _dev(om), 5, w.dt)
-    assert ref["status"][3] == 2 and np.array_equal(_host(out["status"]), ref["status"])
+    eq.close()
+
+
+@pytest.mark.parametrize("cfg,prec", [(1, "f64"), (4, "f64"), (5, "f32")])
+def test_a_ray_with_a_bad_frequency_is_never_advanced(rt, oracle, cfg, prec):
+    """Reading A20 / include/rt.h (rt_trace_w): w_i that is not positive and finite (0, negative, inf, NaN) gives status 2,
+    the launch state back bit for bit at every sample and |D| = NaN -- for that ray only; as in the oracle."""
+    n = 70
+    w = inputs.config(cfg, n_rays=n, n_steps=20)
+    oeq = oracle.Equilibrium(w.eq)
+    k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    om = np.full(n, w.omega)
+    bad = [3, 31, 32, 69]
+    om[bad] = [0.0, -w.omega, np.inf, np.nan]
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, om, 20, w.dt, 10, traj=True)
+    assert (ref["status"][bad] == 2).all() and ref["status"].sum() == 8
+    eq = rt.create_equilibrium(w.eq)
+    x0d, k0d = _dev(w.x0, prec), _dev(k0, prec)
+    out = rt.trace(eq, w.disp, x0d, k0d, _dev(om), 20, w.dt, 10, traj=True)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    launch_state = np.concatenate([_host(x0d), _host(k0d)])
+    tr, res = _host(out["traj"]), _host(out["residual"])
+    for m in range(3):
+        assert np.array_equal(tr[m][:, bad], launch_state[:, bad])
+    assert np.array_equal(_host(out["final"])[:, bad], launch_state[:, bad])
+    assert np.isnan(res[:, bad]).all() and np.array_equal(np.isnan(res), np.isnan(ref["residual"]))
+    good = np.setdiff1d(np.arange(n), bad)
+    ex, ek = rel_err_xk(_host(out["final"])[:, good], ref["final"][:, good])
+    tol = 1e-10 if prec == "f64" else 1e-4
+    assert ex < tol and ek < tol, (ex, ek)
     eq.close()
 
 
