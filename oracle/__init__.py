@@ -64,6 +64,7 @@ def _load():
         P, D, I64, I32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_int
         lib.oracle_trace.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, I64, I64, D, I64, P, P, P, P, I32]
         lib.oracle_trace_w.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, I64, D, I64, P, P, P, P, I32]
+        lib.oracle_trace_until.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, I64, I64, I64, D, D, P, P, P, P, P, I32]
         lib.oracle_launch_w.argtypes = [ctypes.POINTER(_CEq), I32, I32, P, P, P, I64, P, P]
         lib.oracle_diagnostics.argtypes = [ctypes.POINTER(_CEq), P, P, P, I64, P]
         lib.oracle_orbit.argtypes = [ctypes.POINTER(_CEq), P, P, D, I64, I64, D, I64, P, P, P, P, I32]
@@ -178,6 +179,24 @@ def trace(eq, disp, x0, k0, omega, n_steps, dt, save_stride=1, *, traj=False, fi
     if rc != 0:
         raise ValueError(f"oracle_trace rejected its arguments (rc={rc})")
     return out
+
+
+def trace_until(eq, disp, x0, k0, omega, chunk_steps, max_chunks, dt, tol=np.inf, n_threads=0) -> dict:
+    """The convergence workflow (L80): advance the ensemble in chunks of ``chunk_steps`` steps until every
+    ray is frozen, max |D| exceeds ``tol``, or ``max_chunks`` chunks have run.  Returns 'final' [6,n], 'residual' [n],
+    'status' [n], 'chunks', 'n_active', 'reason' (0 max_chunks, 1 all frozen, 2 tolerance exceeded) and 'max_D'."""
+    lib, e = _load(), _eq(eq)
+    x0, k0 = _soa(x0), _soa(k0)
+    n = x0.shape[1]
+    fin, res, st = np.empty((6, n)), np.empty(n), np.empty(n, dtype=np.int32)
+    info, mx = np.zeros(4, dtype=np.int64), np.zeros(1)
+    rc = lib.oracle_trace_until(ctypes.byref(e.c), _disp(disp), x0.ctypes.data, k0.ctypes.data, float(omega), n,
+                                int(chunk_steps), int(max_chunks), float(dt), float(tol), fin.ctypes.data, res.ctypes.data,
+                                st.ctypes.data, info.ctypes.data, mx.ctypes.data, int(n_threads))
+    if rc != 0:
+        raise ValueError(f"oracle_trace_until rejected its arguments (rc={rc})")
+    return dict(final=fin, residual=res, status=st, chunks=int(info[0]), n_active=int(info[1]), reason=int(info[2]),
+                max_D=float(mx[0]))
 
 
 def dispersion(eq, disp, x, k, omega):

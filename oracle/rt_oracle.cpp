@@ -406,6 +406,64 @@ int oracle_trace_w(const orc_equilibrium* eq, int disp, const double* x0, const 
                     out_status, n_threads);
 }
 
+// The convergence workflow (L80, section 2.3: "workflows ... can be implemented by chaining calls to evaluation and
+// reduction kernels until a tolerance is met"; L76: reduction kernels; SURVEY 8(f)-2 "stop-when-all-frozen"), stated for
+// the ray tracer: advance the ensemble in chunks of `chunk_steps` RK4 steps; after each chunk reduce over the rays
+//      n_active = number of rays with status 0,        max_D = max |D| over the rays whose |D| is finite,
+// and stop after the first chunk at which n_active == 0 (every ray is frozen), or max_D > tol (the ensemble has drifted
+// off the dispersion surface by more than the tolerance), or `max_chunks` chunks have run.  A frozen ray stays frozen
+// across chunks (reading A12).  Outputs: out_final [6][n], out_residual [n] (|D| at the final state), out_status [n],
+// out_info [4] = {chunks run, n_active at the stop, reason (0 max_chunks reached, 1 all rays frozen, 2 tolerance
+// exceeded; 1 wins if both hold), 0} and *out_maxD = max_D at the stop (0 if no ray has a finite |D|).
+int oracle_trace_until(const orc_equilibrium* eq, int disp, const double* x0, const double* k0, double omega, int64_t n_rays,
+                       int64_t chunk_steps, int64_t max_chunks, double dt, double tol, double* out_final,
+                       double* out_residual, int32_t* out_status, int64_t* out_info, double* out_maxD, int n_threads) {
+  if (!eq || !combo_supported(*eq, disp) || n_rays < 0 || chunk_steps < 1 || max_chunks < 0 || !(tol > 0.0)) return -1;
+  if (!out_final || !out_residual || !out_status || !out_info || !out_maxD) return -1;
+  for (int64_t i = 0; i < n_rays; ++i) {
+    for (int c = 0; c < 3; ++c) { out_final[c * n_rays + i] = x0[c * n_rays + i]; out_final[(3 + c) * n_rays + i] = k0[c * n_rays + i]; }
+    out_status[i] = (omega > 0.0 && std::isfinite(omega)) ? 0 : 2;           // reading A20
+  }
+  const double h = dt / C_LIGHT;
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+  int64_t chunks = 0, n_active = 0, reason = 0;
+  double max_D = 0.0;
+  while (chunks < max_chunks) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < n_rays; ++i) {                                   // the "evaluation kernel": one chunk
+      double y[6];
+      for (int c = 0; c < 6; ++c) y[c] = out_final[c * n_rays + i];
+      int status = out_status[i];
+      for (int64_t s = 0; s < chunk_steps && status == 0; ++s) status = rk4_step(*eq, disp, omega, h, y);
+      for (int c = 0; c < 6; ++c) out_final[c * n_rays + i] = y[c];
+      out_status[i] = status;
+      out_residual[i] = (status == 2 && !(omega > 0.0 && std::isfinite(omega))) ? std::numeric_limits<double>::quiet_NaN()
+                                                                               : residual(*eq, disp, omega, y);
+    }
+    ++chunks;
+    n_active = 0; max_D = 0.0;                                               // the "reduction kernel"
+    for (int64_t i = 0; i < n_rays; ++i) {
+      if (out_status[i] == 0) ++n_active;
+      if (std::isfinite(out_residual[i]) && out_residual[i] > max_D) max_D = out_residual[i];
+    }
+    if (n_active == 0) { reason = 1; break; }
+    if (max_D > tol) { reason = 2; break; }
+  }
+  if (chunks == 0)                                                           // max_chunks == 0: report the launch state
+    for (int64_t i = 0; i < n_rays; ++i) {
+      double y[6];
+      for (int c = 0; c < 6; ++c) y[c] = out_final[c * n_rays + i];
+      out_residual[i] = (out_status[i] == 2) ? std::numeric_limits<double>::quiet_NaN() : residual(*eq, disp, omega, y);
+      if (out_status[i] == 0) ++n_active;
+      if (std::isfinite(out_residual[i]) && out_residual[i] > max_D) max_D = out_residual[i];
+    }
+  out_info[0] = chunks; out_info[1] = n_active; out_info[2] = reason; out_info[3] = 0;
+  *out_maxD = max_D;
+  return 0;
+}
+
 // Critical-surface diagnostics (L149: cut-offs and resonances; Fig. 3-4 L157/L175) at n points with one frequency per
 // point: out [10][n] = n_e, |B|, X = wpe^2/w^2, Y = |Wce|/w (electrons), S, Dx, P (Eq. 8-10), R = S + Dx, L = S - Dx,
 // n_par^2 = (n.B/|B|)^2 with n = c k / w (Eq. 6); n_par^2 = 0 where B = 0.  NaN outside the domain.
