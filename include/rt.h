@@ -200,6 +200,29 @@ int rt_rhs(const rt_equilibrium* eq, int disp, int precision, const void* x, con
  * int32 [n] or NULL.  out: DEVICE double [6] = {max |D|, sum |D|, count finite, #status0, #status1, #status2}. */
 int rt_reduce(int precision, const void* residual, const int32_t* status, int64_t n, double* out, void* cuda_stream);
 
+/* The convergence workflow (section 2.3: "workflows ... can be implemented by chaining calls to evaluation
+ * and reduction kernels until a tolerance is met"; L76: reduction kernels; SURVEY 8(f)-2 "stop-when-all-frozen").  The
+ * ensemble is advanced in chunks of `chunk_steps` RK4 steps; after each chunk a device-side reduction counts the rays
+ * still active (status 0) and takes max |D| over the rays whose |D| is finite; the loop stops after the first chunk at
+ * which no ray is active, or max |D| > tol, or `max_chunks` chunks have run.  The loop is a CUDA-graph WHILE node whose
+ * body is {trace kernel on the state in out_final, reduce kernel, decision kernel}: the condition is set ON THE DEVICE,
+ * there is no host round trip between chunks, and the call returns as soon as the graph is enqueued on `cuda_stream`
+ * (which must not be capturing).  A frozen ray stays frozen (and bit for bit unchanged) across chunks.
+ *   x0, k0         DEVICE [3][n_rays] launch state (not modified)
+ *   chunk_steps    >= 1;  max_chunks >= 0 (0: report the launch state);  tol > 0, +inf switches the |D| criterion off
+ *   out_final      DEVICE [6][n_rays]: the state, advanced in place chunk by chunk; required
+ *   out_residual   DEVICE [n_rays] |D| at the current state; required      out_status  DEVICE int32 [n_rays]; required
+ *   out_info       DEVICE int64 [RT_UNTIL_INFO_WORDS], 8-byte aligned; on completion
+ *                    [0] chunks run   [1] rays still active   [2] max |D| at the stop (bit pattern of a double)
+ *                    [3] reason: 0 = max_chunks reached, 1 = every ray frozen, 2 = max |D| > tol (1 wins over 2)
+ *                    [4..9] the last reduction as rt_reduce writes it (doubles);  [10..15] reserved
+ * State rows hold k in rad/m; an active ray's k is re-rounded once per chunk by the exchange k <-> n = c k / w.
+ * Errors: RT_ERR_INVALID (as rt_trace, and chunk_steps < 1, max_chunks < 0, tol not > 0, a NULL output), UNSUPPORTED, CUDA. */
+#define RT_UNTIL_INFO_WORDS 16
+int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                   int64_t n_rays, int64_t chunk_steps, int64_t max_chunks, double dt, double tol, void* out_final,
+                   void* out_residual, int32_t* out_status, int64_t* out_info, void* cuda_stream);
+
 /* Measured roofline denominator: run >= min_ms milliseconds of independent dependent-chain FMA accumulators (DFMA
  * for RT_F64, FFMA for RT_F32) on every SM and report the sustained rate.  Synchronous.
  *   fma_per_s     HOST out: fused multiply-adds per second (flop/s = 2x)

@@ -24,7 +24,7 @@ DISP_KINDS = {"omode": 0, "xmode": 1, "cold_full": 2}
 PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
-SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_launch", "rt_launch_w",
+SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_trace_until", "rt_launch", "rt_launch_w",
            "rt_launch_kx", "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_launch_count", "rt_last_error", "rt_version")
 NDIAG = 10
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
@@ -91,6 +91,7 @@ def load() -> ctypes.CDLL:
         lib.rt_destroy.argtypes = [P]
         lib.rt_trace.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_trace_w.argtypes = [P, I32, I32, P, P, P, I64, I64, D, I64, P, P, P, P, P]
+        lib.rt_trace_until.argtypes = [P, I32, I32, P, P, D, I64, I64, I64, D, D, P, P, P, P, P]
         lib.rt_launch_w.argtypes = [P, I32, I32, P, P, P, I64, P, P, P]
         lib.rt_diagnostics.argtypes = [P, P, P, D, P, I64, P, P]
         lib.rt_launch_kx.argtypes = [P, I32, P, P, D, P, I64, I32, D, P, P, P, P]
@@ -230,6 +231,41 @@ def trace(eq: Equilibrium, disp, x0, k0, omega, n_steps: int, dt: float, save_st
         _check(lib.rt_trace_w(eq.handle, _disp(disp), prec, _ptr(x0), _ptr(k0), _ptr(w), n, int(n_steps), float(dt),
                               int(save_stride), *outs, _stream()))
     return o
+
+
+UNTIL_INFO_WORDS = 16
+UNTIL_REASONS = ("max_chunks", "all_frozen", "tolerance")
+
+
+def trace_until(eq: Equilibrium, disp, x0, k0, omega: float, chunk_steps: int, max_chunks: int, dt: float,
+                tol: float = float("inf"), out: dict | None = None) -> dict:
+    """``rt_trace_until`` on the current CUDA stream: advance the ensemble in chunks of ``chunk_steps`` steps until every
+    ray is frozen, max |D| > ``tol`` or ``max_chunks`` chunks have run; the loop runs on the device (CUDA-graph WHILE node)
+    and the call does not synchronise.  Returns device tensors 'final' [6, n], 'residual' [n], 'status' [n] int32 and
+    'info' int64 [16] (see ``until_info``)."""
+    import torch
+    lib = load()
+    x0 = _dev_soa(x0, 3)
+    n = x0.shape[1]
+    k0 = _dev_soa(k0, 3, n)
+    if k0.dtype != x0.dtype:
+        raise TypeError("x0 and k0 must have the same dtype")
+    o = {} if out is None else out
+    o.setdefault("final", torch.empty((6, n), dtype=x0.dtype, device=x0.device))
+    o.setdefault("residual", torch.empty((n,), dtype=x0.dtype, device=x0.device))
+    o.setdefault("status", torch.empty((n,), dtype=torch.int32, device=x0.device))
+    o.setdefault("info", torch.empty((UNTIL_INFO_WORDS,), dtype=torch.int64, device=x0.device))
+    _check(lib.rt_trace_until(eq.handle, _disp(disp), _prec_of(x0), _ptr(x0), _ptr(k0), float(omega), n, int(chunk_steps),
+                              int(max_chunks), float(dt), float(tol), _ptr(o["final"]), _ptr(o["residual"]),
+                              _ptr(o["status"]), _ptr(o["info"]), _stream()))
+    return o
+
+
+def until_info(info) -> dict:
+    """Decode ``rt_trace_until``'s out_info (synchronises: it copies the 16 words to the host)."""
+    import torch
+    h = info.cpu()
+    return dict(chunks=int(h[0]), n_active=int(h[1]), max_D=float(h[2:3].view(torch.float64)[0]), reason=int(h[3]))
 
 
 def trace_host(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: float, save_stride: int = 1, *,

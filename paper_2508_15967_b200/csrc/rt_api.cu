@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -102,6 +103,8 @@ int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, con
     constexpr int block = rt::TraceShape<T, E>::BLOCK;                                     \
     if (A.omega)                                                                           \
       rt::trace_kernel<T, E, D, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A);  \
+    else if (A.status_in)                                                                  \
+      rt::trace_kernel<T, E, D, false, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
     else                                                                                   \
       rt::trace_kernel<T, E, D, false><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
     ++g_launches;                                                                          \
@@ -180,9 +183,11 @@ constexpr double kOmegaRefPerRay = 1.0;
 template <class T>
 int trace_device(const rt_equilibrium* eq, int disp, const void* x0, const void* k0, double omega,
                  const double* omega_rays, long long n_rays, long long n_steps, double dt, long long save_stride,
-                 void* out_traj, void* out_final, void* out_residual, int32_t* out_status, cudaStream_t st) {
+                 void* out_traj, void* out_final, void* out_residual, int32_t* out_status, cudaStream_t st,
+                 const int32_t* status_in = nullptr) {
   const rt::Params<T> P = make_params<T>(eq, omega_rays ? kOmegaRefPerRay : omega);
   rt::TraceArgs<T> A;
+  A.status_in = status_in;
   A.omega = omega_rays;
   A.omega_ref = kOmegaRefPerRay;
   A.x0 = static_cast<const T*>(x0);
@@ -278,6 +283,74 @@ int orbit_device(const rt_equilibrium* eq, const void* x0, const void* v0, doubl
 }
 }  // namespace
 
+namespace {
+// zero out[6], then one grid-stride pass over residual / status (8 blocks of 256 threads per SM at most)
+int launch_reduce(int precision, const void* residual, const int32_t* status, long long n, double* out, cudaStream_t st) {
+  RT_CUDA(cudaMemsetAsync(out, 0, 6 * sizeof(double), st));
+  if (n == 0) return RT_OK;
+  static int sms = 0;
+  if (sms == 0) {
+    int dev = 0, v = 0;
+    RT_CUDA(cudaGetDevice(&dev));
+    RT_CUDA(cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev));
+    sms = v > 0 ? v : 1;
+  }
+  long long blocks = (n + 255) / 256;
+  if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;
+  if (precision == RT_F64)
+    rt::reduce_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(static_cast<const double*>(residual), status, n, out);
+  else
+    rt::reduce_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(static_cast<const float*>(residual), status, n, out);
+  ++g_launches;
+  RT_CUDA(cudaGetLastError());
+  return RT_OK;
+}
+}  // namespace
+
+namespace {
+// rt_trace_until's graphs.  Destroying an executable graph that is still running blocks the host until it has finished
+// (measured: the call took as long as the device work), so a launched graph is parked here with an event recorded behind
+// it and released by a later call (or rt_destroy) once that event has completed -- the call itself never waits.
+struct PendingGraph {
+  cudaGraphExec_t ex;
+  cudaGraph_t g;
+  cudaEvent_t done;
+};
+std::mutex g_pending_mu;
+std::vector<PendingGraph> g_pending;
+
+void release_finished_graphs(bool wait) {
+  std::lock_guard<std::mutex> lock(g_pending_mu);
+  size_t keep = 0;
+  for (size_t i = 0; i < g_pending.size(); ++i) {
+    PendingGraph& p = g_pending[i];
+    const cudaError_t q = wait ? cudaEventSynchronize(p.done) : cudaEventQuery(p.done);
+    if (q == cudaErrorNotReady) { g_pending[keep++] = p; continue; }
+    if (q != cudaSuccess) cudaGetLastError();
+    cudaGraphExecDestroy(p.ex);
+    cudaGraphDestroy(p.g);
+    cudaEventDestroy(p.done);
+  }
+  g_pending.resize(keep);
+}
+
+// Releases what rt_trace_until has acquired on its error paths (and the capture stream on every path).
+struct UntilCleanup {
+  cudaGraph_t g = nullptr;
+  cudaGraphExec_t ex = nullptr;
+  cudaStream_t cs = nullptr;
+  cudaEvent_t done = nullptr;
+  bool capturing = false;
+  ~UntilCleanup() {
+    if (capturing) { cudaGraph_t dead = nullptr; cudaStreamEndCapture(cs, &dead); }
+    if (done) cudaEventDestroy(done);
+    if (ex) cudaGraphExecDestroy(ex);
+    if (g) cudaGraphDestroy(g);
+    if (cs) cudaStreamDestroy(cs);
+  }
+};
+}  // namespace
+
 // ==== C ABI ===========================================================================================================
 extern "C" {
 
@@ -371,6 +444,7 @@ int rt_create_equilibrium(const rt_equilibrium_desc* desc, rt_equilibrium** out)
 int rt_destroy(rt_equilibrium* eq) {
   if (!eq) return RT_OK;
   if (eq->psi_pp64 || eq->slot[0] || eq->streams[0]) cudaDeviceSynchronize();
+  release_finished_graphs(true);
   free_handle(eq);
   return RT_OK;
 }
@@ -507,6 +581,96 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
   return RT_OK;
 }
 
+int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                   int64_t n_rays, int64_t chunk_steps, int64_t max_chunks, double dt, double tol, void* out_final,
+                   void* out_residual, int32_t* out_status, int64_t* out_info, void* cuda_stream) {
+  int rc = check_trace_args(eq, disp, precision, x0, k0, omega, n_rays, chunk_steps, dt, 1, nullptr);
+  if (rc) return rc;
+  if (chunk_steps < 1) return fail(RT_ERR_INVALID, "chunk_steps must be >= 1");
+  if (max_chunks < 0) return fail(RT_ERR_INVALID, "max_chunks must be >= 0");
+  if (!(tol > 0.0)) return fail(RT_ERR_INVALID, "tol must be > 0 (+inf switches the |D| criterion off)");
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  if ((rc = require_device_ptr(out_info, "out_info", false, 8))) return rc;
+  if (n_rays > 0 &&
+      ((rc = require_device_ptr(x0, "x0", false, es)) || (rc = require_device_ptr(k0, "k0", false, es)) ||
+       (rc = require_device_ptr(out_final, "out_final", false, 16)) ||
+       (rc = require_device_ptr(out_residual, "out_residual", false, 16)) ||
+       (rc = require_device_ptr(out_status, "out_status", false, 4))))
+    return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  long long* info = reinterpret_cast<long long*>(out_info);
+  double* red = reinterpret_cast<double*>(info + 4);
+  if (n_rays == 0) {                               // nothing to advance: 0 chunks, 0 active rays, "every ray frozen"
+    RT_CUDA(cudaMemsetAsync(info, 0, RT_UNTIL_INFO_WORDS * 8, st));
+    rt::until_decide_kernel<<<1, 1, 0, st>>>(info, tol, 0, 0, 0);
+    ++g_launches;
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+  }
+  char* fin = static_cast<char*>(out_final);
+  const size_t row3 = 3 * (size_t)n_rays * es;
+  auto chunk = [&](long long steps, cudaStream_t s, const int32_t* status_in) -> int {
+    const void* xs = status_in ? fin : x0;
+    const void* ks = status_in ? fin + row3 : k0;
+    if (precision == RT_F64)
+      return trace_device<double>(eq, disp, xs, ks, omega, nullptr, n_rays, steps, dt, 1, nullptr, out_final, out_residual,
+                                  out_status, s, status_in);
+    return trace_device<float>(eq, disp, xs, ks, omega, nullptr, n_rays, steps, dt, 1, nullptr, out_final, out_residual,
+                               out_status, s, status_in);
+  };
+  if (max_chunks == 0) {                           // report the launch state: one zero-step pass, reduce, record
+    RT_CUDA(cudaMemsetAsync(info, 0, RT_UNTIL_INFO_WORDS * 8, st));
+    if ((rc = chunk(0, st, nullptr))) return rc;
+    if ((rc = launch_reduce(precision, out_residual, out_status, n_rays, red, st))) return rc;
+    rt::until_decide_kernel<<<1, 1, 0, st>>>(info, tol, 0, 0, 0);
+    ++g_launches;
+    RT_CUDA(cudaGetLastError());
+    return RT_OK;
+  }
+  // graph:  {copy x0, k0 into out_final; zero out_status and out_info}  ->  WHILE (cond) { chunk; reduce; decide }
+  release_finished_graphs(false);
+  UntilCleanup u;
+  RT_CUDA(cudaGraphCreate(&u.g, 0));
+  cudaGraphNode_t pro[4];
+  RT_CUDA(cudaGraphAddMemcpyNode1D(&pro[0], u.g, nullptr, 0, fin, x0, row3, cudaMemcpyDeviceToDevice));
+  RT_CUDA(cudaGraphAddMemcpyNode1D(&pro[1], u.g, nullptr, 0, fin + row3, k0, row3, cudaMemcpyDeviceToDevice));
+  cudaMemsetParams ms = {};
+  ms.dst = out_status; ms.value = 0; ms.elementSize = 4; ms.width = (size_t)n_rays; ms.height = 1;
+  RT_CUDA(cudaGraphAddMemsetNode(&pro[2], u.g, nullptr, 0, &ms));
+  ms.dst = info; ms.width = RT_UNTIL_INFO_WORDS * 2;
+  RT_CUDA(cudaGraphAddMemsetNode(&pro[3], u.g, nullptr, 0, &ms));
+  cudaGraphConditionalHandle cond;
+  RT_CUDA(cudaGraphConditionalHandleCreate(&cond, u.g, 1, cudaGraphCondAssignDefault));
+  cudaGraphNodeParams np = {};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = cond;
+  np.conditional.type = cudaGraphCondTypeWhile;
+  np.conditional.size = 1;
+  cudaGraphNode_t loop;
+  RT_CUDA(cudaGraphAddNode(&loop, u.g, pro, 4, &np));
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  RT_CUDA(cudaStreamCreateWithFlags(&u.cs, cudaStreamNonBlocking));
+  RT_CUDA(cudaStreamBeginCaptureToGraph(u.cs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+  u.capturing = true;
+  if ((rc = chunk(chunk_steps, u.cs, out_status))) return rc;
+  if ((rc = launch_reduce(precision, out_residual, out_status, n_rays, red, u.cs))) return rc;
+  rt::until_decide_kernel<<<1, 1, 0, u.cs>>>(info, tol, max_chunks, cond, 1);
+  ++g_launches;
+  RT_CUDA(cudaGetLastError());
+  u.capturing = false;
+  RT_CUDA(cudaStreamEndCapture(u.cs, nullptr));
+  RT_CUDA(cudaGraphInstantiate(&u.ex, u.g, 0));
+  RT_CUDA(cudaEventCreateWithFlags(&u.done, cudaEventDisableTiming));
+  RT_CUDA(cudaGraphLaunch(u.ex, st));
+  RT_CUDA(cudaEventRecord(u.done, st));
+  {
+    std::lock_guard<std::mutex> lock(g_pending_mu);
+    g_pending.push_back({u.ex, u.g, u.done});
+  }
+  u.ex = nullptr; u.g = nullptr; u.done = nullptr;        // now owned by the pending list
+  return RT_OK;
+}
+
 int rt_launch(const rt_equilibrium* eq, int disp, int branch, const double* x0, const double* dir, double omega,
               int64_t n, double* k0, double* D_out, void* cuda_stream) {
   int rc = check_combo(eq, disp);
@@ -615,18 +779,7 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
       (rc = require_device_ptr(residual, "residual", true, (precision == RT_F64) ? 8 : 4)) ||
       (rc = require_device_ptr(status, "status", true, 4)))
     return rc;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  RT_CUDA(cudaMemsetAsync(out, 0, 6 * sizeof(double), st));
-  if (n == 0) return RT_OK;
-  long long blocks = (n + 255) / 256;
-  if (blocks > 148 * 8) blocks = 148 * 8;
-  if (precision == RT_F64)
-    rt::reduce_kernel<double><<<(unsigned)blocks, 256, 0, st>>>(static_cast<const double*>(residual), status, n, out);
-  else
-    rt::reduce_kernel<float><<<(unsigned)blocks, 256, 0, st>>>(static_cast<const float*>(residual), status, n, out);
-  ++g_launches;
-  RT_CUDA(cudaGetLastError());
-  return RT_OK;
+  return launch_reduce(precision, residual, status, n, out, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz) {

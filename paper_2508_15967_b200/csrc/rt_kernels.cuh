@@ -54,6 +54,8 @@ struct TraceArgs {
   T h;                  // step in tau = c t
   const double* omega;  // per-ray frequencies [n_rays] (PW kernels only), rad/s
   double omega_ref;     // the frequency the Params were folded at
+  const int32_t* status_in;   // resume (rt_trace_until's chunks): each ray's status at entry, or NULL = every ray starts
+                              // active.  May alias `status`; x0 / k0 may then alias the rows of `fin` (in-place chunk).
 };
 
 // One classical RK4 step (reading A7): stage abscissae (0, 1/2, 1/2, 1), weights (1, 2, 2, 1)/6, written so that every
@@ -237,8 +239,10 @@ struct RowStore {
   }
 };
 
-template <class T, int EQ, int DISP, bool PW>
-__global__ void __maxnreg__((TraceShape<T, EQ>::MAXNREG + (PW ? 16 : 0)))
+// RESUME: the chunk kernel of rt_trace_until -- each ray's status at entry comes from A.status_in (a separate
+// instantiation, so that the plain kernels' register allocation is untouched).
+template <class T, int EQ, int DISP, bool PW, bool RESUME = false>
+__global__ void __maxnreg__((TraceShape<T, EQ>::MAXNREG + (PW ? 16 : 0) + (RESUME ? 8 : 0)))
 trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ TraceArgs<T> A) {
   constexpr int BLOCK = TraceShape<T, EQ>::BLOCK;
   const long long N = A.n_rays;
@@ -268,6 +272,7 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
     y[3 + c] = valid ? A.k0[c * N + i] * P.k2n : T(0);          // n = c k / w  (Eq. 6)
   }
   int status = valid ? (bad_w ? 2 : 0) : 3;        // 3: padding lane of the last block, never stored
+  if (RESUME && status == 0) status = A.status_in[i];
   // Everything the store needs is recomputed here from threadIdx / the kernel arguments, so that nothing of it stays
   // live across the step loop (the loop is register-bound).
   auto save = [&](T* rows6, T* res_row) {
@@ -280,6 +285,16 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
     T v[6];
 #pragma unroll
     for (int c = 0; c < 3; ++c) { v[c] = y[c]; v[3 + c] = y[3 + c] * P.n2k; }
+    // Resume mode: a ray that was already frozen at entry has never been advanced; its k rows go back bit for bit
+    // (re-read here; out_status is only written after the last store) instead of through the round trip k -> n -> k, so
+    // a frozen ray stays frozen however many chunks follow.  Nothing of this is live across the step loop.
+    if (RESUME) {
+      const long long ii = (long long)blockIdx.x * BLOCK + threadIdx.x;
+      if (ii < A.n_rays && A.status_in[ii] != 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) v[3 + c] = A.k0[c * A.n_rays + ii];
+      }
+    }
     T r = res_row ? abs_residual<T, EQ, DISP>(P, y, gather) : T(0);
     if (PW && bad_w) r = rt_nan<T>();
     out.store(rows6, res_row, v, r, out.i0 + out.lane < A.n_rays);
@@ -614,6 +629,27 @@ reduce_kernel(const T* __restrict__ res, const int32_t* __restrict__ status, lon
     atomicAdd(out + 4, s1);
     atomicAdd(out + 5, s2);
   }
+}
+
+// The convergence workflow's decision step (rt_trace_until; "chaining calls to evaluation and reduction
+// kernels until a tolerance is met").  Runs as the last node of the body of a CUDA-graph WHILE node, after the chunk's
+// trace_kernel and reduce_kernel: one thread reads the reduction, counts the chunk, records why the loop stops and
+// sets the WHILE condition on the device -- no host round trip between chunks.
+//   info[0] chunks run   info[1] rays still active (status 0)   info[2] max |D| (bit pattern of a double)
+//   info[3] reason: 0 max_chunks reached, 1 every ray frozen, 2 max |D| > tol        info[4..9]: reduce_kernel's out[6]
+__global__ void until_decide_kernel(long long* __restrict__ info, double tol, long long max_chunks,
+                                    cudaGraphConditionalHandle cond, int in_graph) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const double* red = reinterpret_cast<const double*>(info + 4);
+  const long long chunks = info[0] + (in_graph ? 1 : 0);
+  const long long n_active = (long long)red[3];
+  const double max_D = red[0];
+  long long reason = 0;
+  bool go = chunks < max_chunks;
+  if (n_active == 0) { reason = 1; go = false; }
+  else if (max_D > tol) { reason = 2; go = false; }
+  info[0] = chunks; info[1] = n_active; info[2] = __double_as_longlong(max_D); info[3] = reason;
+  if (in_graph) cudaGraphSetConditional(cond, go ? 1u : 0u);
 }
 
 // Roofline denominator: FMA_CHAINS independent accumulators per thread, each a dependent chain of fused multiply-adds.

@@ -99,7 +99,7 @@ def count_kernels(lib: Path = LIB) -> dict:
     sass = subprocess.run([exe, "-sass", str(lib)], capture_output=True, text=True, check=True).stdout
     res = {}
     for fn in re.split(r"\n\s*Function : ", sass):
-        m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)ELb0E", fn)      # the single-frequency kernels
+        m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)ELb0ELb0E", fn)      # the plain single-frequency kernels
         if not m:
             continue
         prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
