@@ -2,6 +2,7 @@
 """bench.py -- ray-steps/s of the batched RF ray tracer on B200 (BASELINE.json's metric), one JSON line on stdout.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--precision f64] [--impl ours|reference]
+                    [--scaling weak|strong]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 A "step" is one pass of the whole hot path over one batch: one ``rt_trace`` call that loads the launch states, runs all
@@ -10,7 +11,10 @@ config 4 -- the configuration the north-star target is quoted on (2^20 rays x 10
 analytic tokamak, fp64, trajectories decimated every 10 steps).  Inputs are seeded and synthetic (inputs.py) and are
 resident in HBM when the timed region starts; launch wave vectors come from the library's own ``rt_launch`` kernel.
 
-`value`        = n_gpus * n_rays * n_steps * K / (max-over-ranks device time of K steps)
+`value`        = (rays all ranks traced) * n_steps * K / (max-over-ranks device time of K steps).  ``--scaling weak``
+                 (default): every rank traces its own full-size seeded batch; ``--scaling strong``: ONE seeded ensemble of
+                 the config's size is split into contiguous ray ranges, rank r traces ``sharding.ray_range(n, r, world)``
+                 (the paper's own multi-device experiment).  No collective on the data path either way.
 `e2e`          = the same metric through ``rt_trace_host`` with pinned HOST buffers (H2D + kernel + D2H per step)
 `roofline`     = bound "alu": algorithmic flops per launch / mean kernel time (CUDA events on the launch stream) against
                  2 x the DFMA (FFMA) rate measured by ``rt_fma_peak`` in this process
@@ -56,6 +60,10 @@ FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f
 FP_RF3_PER_RAY_STEP = {(1, "f64"): 26, (2, "f64"): 26, (3, "f64"): 39, (4, "f64"): 169, (5, "f64"): 328,
                        (1, "f32"): 29, (2, "f32"): 29, (3, "f32"): 39, (4, "f32"): 157, (5, "f32"): 268}
 RF3_EXTRA = {"f64": 0.5, "f32": 0.563}      # shape 0 rate / shape 2 rate - 1:  63.9 / 42.7 = 1.50,  123.2 / 78.8 = 1.563
+# The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from
+# sass_count.py's orbit_kernel rows (pinned by the same test).
+ORBIT_COUNTS = {"f64": dict(flops=248, instr=188, rf3=44), "f32": dict(flops=248, instr=166, rf3=32)}
+ORBIT_KERNEL = (2, "orbit")
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None
@@ -78,6 +86,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--n-rays", type=int, default=None, help="override the config's ray count (debugging only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -134,17 +143,32 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ CPU oracle legs
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    import platform
+    return platform.processor() or platform.machine()
+
+
+def host_cores() -> int:
+    """All host cores this process may run on (torchrun exports OMP_NUM_THREADS=1, which omp_get_max_threads() would obey;
+    under torchrun only rank 0 runs the oracle, so the cores are its own)."""
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
 def oracle_rate(cfg: int, target_s: float, n_threads: int = 0):
     """Time the CPU oracle, as it stands, on a bounded sample of config `cfg`: the first n rays of the seeded launch set
-    at the config's full step count, n sized from a short calibration so the run takes about `target_s` seconds."""
+    at the config's full step count, n sized from a short calibration so the run takes about `target_s` seconds.
+    n_threads = 0: every host core; 1: the single-thread leg."""
     import oracle
     oracle.build()
-    # all host cores this process may run on (torchrun exports OMP_NUM_THREADS=1, which omp_get_max_threads() would obey;
-    # under torchrun only rank 0 runs the oracle, so the cores are its own)
-    avail = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
-    cores = max(avail, oracle.max_threads()) if n_threads <= 0 else n_threads
+    cores = max(host_cores(), oracle.max_threads()) if n_threads <= 0 else n_threads
     n_steps = inputs.FULL_SIZES[cfg][1]
-    probe_n = 64 * cores          # enough rays that every thread of the dynamic schedule (chunks of 16) is busy
+    probe_n = 64 * cores if cores > 1 else 16    # enough rays that every thread of the dynamic schedule (chunks of 16) is busy
     w = inputs.config(cfg, n_rays=probe_n, n_steps=n_steps)
     oeq = oracle.Equilibrium(w.eq)
     k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
@@ -167,10 +191,25 @@ def oracle_rate(cfg: int, target_s: float, n_threads: int = 0):
 
 
 def cpu_baseline(cfg: int) -> dict:
-    run_once, n, n_steps, cores = oracle_rate(cfg, target_s=15.0)
+    """the oracle timed (a) on one thread and (b) on every host core, core count and CPU model stated."""
+    run_once, n, n_steps, cores = oracle_rate(cfg, target_s=12.0)
     t = run_once()
+    run1, n1, _, _ = oracle_rate(cfg, target_s=6.0, n_threads=1)
+    t1 = run1()
     return {"value": n * n_steps / t, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": round(t, 2),
-            "sample": f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps (fp64, OpenMP over rays)"}
+            "sample": f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps (fp64, OpenMP over rays)",
+            "single_thread": {"value": n1 * n_steps / t1, "unit": UNIT, "cores": 1, "seconds": round(t1, 2),
+                              "sample": f"first {n1} rays of the same launch set x {n_steps} steps"},
+            "cpu_model": cpu_model()}
+
+
+def workload_config(cfg: int, scaling: str) -> dict:
+    """The `config` object of the JSON line: the same keys and values on both arms (the reference arm times a bounded
+    sample of this workload; what the sample was is said under `cpu_baseline.sample`)."""
+    n_rays, n_steps = inputs.FULL_SIZES[cfg]
+    return {"workload": WORKLOAD_NAMES[cfg], "n_rays": n_rays, "n_steps": n_steps, "rays_per_gpu": "n_rays (weak: one "
+            "seeded batch per rank)" if scaling == "weak" else "n_rays / n_gpus (strong: contiguous ranges of one ensemble)",
+            "l2": "flushed between steps (256 MiB memset)", "sharding": "independent rays, no collective"}
 
 
 def run_reference(args) -> int:
@@ -185,10 +224,10 @@ def run_reference(args) -> int:
     value = n * n_steps * args.steps / t
     sample = f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps per step (fp64, OpenMP over rays)"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD_NAMES[cfg], "n_rays_per_step": n, "n_steps": n_steps},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": args.scaling,
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args.scaling),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
     return 0
@@ -196,21 +235,24 @@ def run_reference(args) -> int:
 
 # ------------------------------------------------------------------------------------------------ the CUDA arm
 class Job:
-    """One config resident on the current device: equilibrium handle, launch states, preallocated outputs."""
+    """One config resident on the current device: equilibrium handle, launch states, preallocated outputs.
+    ray_range = (begin, end): trace only that contiguous range of the seeded ensemble (strong scaling)."""
 
-    def __init__(self, rt, torch, cfg: int, prec: str, n_rays, rank: int, scan: bool = False):
+    def __init__(self, rt, torch, cfg: int, prec: str, n_rays, seed: int, scan: bool = False, ray_range=None):
         self.rt, self.torch, self.cfg, self.prec = rt, torch, cfg, prec
-        seed = 1000 + cfg + 7919 * rank                       # rank r traces its own batch (weak scaling, no exchange)
         self.w = w = inputs.config(cfg, n_rays=n_rays, seed=seed)
+        b, e = ray_range if ray_range is not None else (0, w.n_rays)
+        self.n = e - b
         self.eq = rt.create_equilibrium(w.eq)
         dt = torch.float64 if prec == "f64" else torch.float32
-        x0 = torch.from_numpy(w.x0).cuda()
+        x0 = torch.from_numpy(np.ascontiguousarray(w.x0[:, b:e])).cuda()
         # scan: a frequency scan, one w per ray (rt_launch_w / rt_trace_w); else the config's single frequency
-        self.omega = torch.from_numpy(inputs.frequency_scan(w.n_rays, w.omega, seed)).cuda() if scan else w.omega
-        k0, D0 = rt.launch(self.eq, w.disp, x0, torch.from_numpy(w.dirs).cuda(), self.omega, w.branch)
+        self.omega = torch.from_numpy(inputs.frequency_scan(w.n_rays, w.omega, seed)[b:e].copy()).cuda() if scan else w.omega
+        k0, D0 = rt.launch(self.eq, w.disp, x0, torch.from_numpy(np.ascontiguousarray(w.dirs[:, b:e])).cuda(), self.omega,
+                           w.branch)
         if not bool(torch.isfinite(k0).all()):
             raise RuntimeError("rt_launch returned non-finite launch states for a bench workload")
-        self.launch_residual = float(D0.abs().max())
+        self.launch_residual = float(D0.abs().max()) if self.n else 0.0
         self.x0, self.k0 = x0.to(dt).contiguous(), k0.to(dt).contiguous()
         self.traj = w.save_stride > 0
         self.stride = w.save_stride if self.traj else 1
@@ -219,7 +261,7 @@ class Job:
 
     @property
     def ray_steps(self) -> int:
-        return self.w.n_rays * self.w.n_steps
+        return self.n * self.w.n_steps
 
     def step(self):
         w = self.w
@@ -229,7 +271,7 @@ class Job:
     def host_buffers(self):
         torch, w = self.torch, self.w
         x0h, k0h = self.x0.cpu().pin_memory(), self.k0.cpu().pin_memory()
-        n, dt = w.n_rays, self.x0.dtype
+        n, dt = self.n, self.x0.dtype
         n_saved = w.n_steps // self.stride + 1
         out = {"final": torch.empty((6, n), dtype=dt, pin_memory=True),
                "residual": torch.empty((n_saved, n) if self.traj else (n,), dtype=dt, pin_memory=True),
@@ -243,6 +285,33 @@ class Job:
     def step_host(self, x0h, k0h, out):
         w = self.w
         return self.rt.trace_host(self.eq, w.disp, x0h, k0h, w.omega, w.n_steps, w.dt, self.stride, traj=self.traj, out=out)
+
+    def close(self):
+        self.out = {}
+        self.eq.close()
+
+
+class OrbitJob:
+    """The second ensemble workload: rt_orbit on inputs.orbit_config(4), 2^20 particles x 1000 steps,
+    trajectories every 10 steps.  Same interface as Job as far as time_steps needs it."""
+
+    def __init__(self, rt, torch, prec: str):
+        self.rt, self.prec = rt, prec
+        self.w = w = inputs.orbit_config(4)
+        self.eq = rt.create_equilibrium(w.eq)
+        dt = torch.float64 if prec == "f64" else torch.float32
+        self.x0 = torch.from_numpy(w.x0).to(dt).cuda().contiguous()
+        self.v0 = torch.from_numpy(w.v0).to(dt).cuda().contiguous()
+        self.out = {}
+
+    @property
+    def ray_steps(self) -> int:
+        return self.w.n * self.w.n_steps
+
+    def step(self):
+        w = self.w
+        return self.rt.orbit(self.eq, self.x0, self.v0, w.charge_over_mass, w.n_steps, w.dt, w.save_stride, traj=True,
+                             out=self.out)
 
     def close(self):
         self.out = {}
@@ -273,6 +342,13 @@ def time_steps(torch, job: Job, steps: int, warmup: int, flush, barrier=None):
     return t0.elapsed_time(t1), statistics.fmean(a.elapsed_time(b) for a, b in ev)
 
 
+def fractions(counts: dict, units: float, kernel_ms: float, fma_rate: float, prec: str) -> dict:
+    """The three fractions of DESIGN.md section 6 for one kernel launch of `units` ray-steps (particle-steps)."""
+    per_s = units / (kernel_ms * 1e-3)
+    return {"roofline_frac": counts["flops"] * per_s / (2.0 * fma_rate), "pipe_frac": counts["instr"] * per_s / fma_rate,
+            "pipe_model_frac": (counts["instr"] + RF3_EXTRA[prec] * counts["rf3"]) * per_s / fma_rate}
+
+
 def run_ours(args) -> int:
     import torch
     if not torch.cuda.is_available():
@@ -280,6 +356,7 @@ def run_ours(args) -> int:
         return 2
     from paper_2508_15967_b200 import binding as rt
     from paper_2508_15967_b200 import build as rt_build
+    from paper_2508_15967_b200 import sharding
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
@@ -295,7 +372,10 @@ def run_ours(args) -> int:
     cfg, prec = args.config, args.precision
     n_rays = args.n_rays if args.n_rays else inputs.FULL_SIZES[cfg][0]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB of L2
-    job = Job(rt, torch, cfg, prec, n_rays, rank)
+    if args.scaling == "strong":      # ONE seeded ensemble, rank r traces its contiguous range
+        job = Job(rt, torch, cfg, prec, n_rays, 1000 + cfg, ray_range=sharding.ray_range(n_rays, rank, world))
+    else:                             # every rank traces its own full-size batch
+        job = Job(rt, torch, cfg, prec, n_rays, sharding.rank_seed(1000 + cfg, rank))
 
     peak_before, _ = rt.fma_peak(prec, 200.0)
     sampler = ClockSampler(local)
@@ -309,17 +389,15 @@ def run_ours(args) -> int:
     # a reduction over the last step's outputs: the run's own correctness summary (max |D|, status counts)
     red = rt.reduce(job.out["residual"].reshape(-1)).cpu().tolist()[:3] + rt.reduce(None, job.out["status"]).cpu().tolist()[3:]
 
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if dist:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
-    value = world * job.ray_steps * args.steps / (total_ms_max * 1e-3)
+    total_ms_max = sharding.max_over_ranks(total_ms, dist, "cuda")
+    all_ray_steps = sharding.sum_over_ranks(float(job.ray_steps), dist, "cuda")
+    value = all_ray_steps * args.steps / (total_ms_max * 1e-3)
 
     e2e = None
     if not args.no_e2e:
         x0h, k0h, hout, h2d, d2h = job.host_buffers()
         job.step_host(x0h, k0h, hout)                                       # warm-up (allocates the pipeline workspace)
-        k_e2e = max(1, min(args.steps, 3))
+        k_e2e = max(1, args.steps)
         torch.cuda.synchronize()
         if barrier:
             barrier()
@@ -327,25 +405,23 @@ def run_ours(args) -> int:
         for _ in range(k_e2e):
             job.step_host(x0h, k0h, hout)
         torch.cuda.synchronize()
-        te = torch.tensor([time.perf_counter() - w0], dtype=torch.float64, device="cuda")
-        if dist:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * job.ray_steps * k_e2e / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "steps": k_e2e, "api": "rt_trace_host (pinned host buffers, 2-stream chunk pipeline)"}
+        t_e2e = sharding.max_over_ranks(time.perf_counter() - w0, dist, "cuda")
+        e2e = {"value": all_ray_steps * k_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "steps": k_e2e, "ms_per_step": 1e3 * t_e2e / k_e2e,
+               "pcie_gb_per_s": (h2d + d2h) * k_e2e / t_e2e / 1e9,       # both directions, copies overlapped with the kernel
+               "api": "rt_trace_host (pinned host buffers, 2-stream chunk pipeline)"}
         del x0h, k0h, hout
 
-    flops = FLOPS_PER_RAY_STEP[(cfg, prec)] * job.ray_steps
+    counts = {"flops": FLOPS_PER_RAY_STEP[(cfg, prec)], "instr": FP_INSTR_PER_RAY_STEP[(cfg, prec)],
+              "rf3": FP_RF3_PER_RAY_STEP[(cfg, prec)]}
+    fr = fractions(counts, job.ray_steps, kernel_ms, peak_after, prec)
     launch_residual = job.launch_residual
     peak = 2.0 * peak_after
-    achieved = flops / (kernel_ms * 1e-3)
-    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": NCU_DRAM_BYTES.get((cfg, prec)), "kernel": f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
-                "kernel_ms": kernel_ms, "flops_per_ray_step": FLOPS_PER_RAY_STEP[(cfg, prec)],
-                "fp_instr_per_ray_step": FP_INSTR_PER_RAY_STEP[(cfg, prec)],
-                "fp_rf3_per_ray_step": FP_RF3_PER_RAY_STEP[(cfg, prec)],
-                "pipe_frac": FP_INSTR_PER_RAY_STEP[(cfg, prec)] * job.ray_steps / (kernel_ms * 1e-3) / peak_after,
-                "pipe_model_frac": (FP_INSTR_PER_RAY_STEP[(cfg, prec)] + RF3_EXTRA[prec] * FP_RF3_PER_RAY_STEP[(cfg, prec)])
-                * job.ray_steps / (kernel_ms * 1e-3) / peak_after,
+    roofline = {"bound": "alu", "achieved": fr["roofline_frac"] * peak / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
+                "frac": fr["roofline_frac"], "traffic": NCU_DRAM_BYTES.get((cfg, prec)),
+                "kernel": f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
+                "kernel_ms": kernel_ms, "flops_per_ray_step": counts["flops"], "fp_instr_per_ray_step": counts["instr"],
+                "fp_rf3_per_ray_step": counts["rf3"], "pipe_frac": fr["pipe_frac"], "pipe_model_frac": fr["pipe_model_frac"],
                 "peak_source": f"rt_fma_peak({prec}) measured in this process after the timed region: "
                                f"{peak_after / 1e12:.3f} T{'D' if prec == 'f64' else 'F'}FMA/s at {peak_mhz:.0f} MHz "
                                f"(before: {peak_before / 1e12:.3f})"}
@@ -359,15 +435,25 @@ def run_ours(args) -> int:
                            (5, "f32", False), (4, "f64", True)):
             if (c, p) == (cfg, prec) and not scan:
                 continue
-            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 0, scan=scan)
+            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 1000 + c, scan=scan)
             _, kms = time_steps(torch, j, 3, 1, flush)
             pk, _ = rt.fma_peak(p, 100.0)
+            cn = {"flops": FLOPS_PER_RAY_STEP[(c, p)], "instr": FP_INSTR_PER_RAY_STEP[(c, p)], "rf3": FP_RF3_PER_RAY_STEP[(c, p)]}
             extra.append({"workload": f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else ""),
                           "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
-                          "roofline_frac": FLOPS_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / (2.0 * pk),
-                          "pipe_frac": FP_INSTR_PER_RAY_STEP[(c, p)] * j.ray_steps / (kms * 1e-3) / pk,
-                          "pipe_model_frac": (FP_INSTR_PER_RAY_STEP[(c, p)] + RF3_EXTRA[p] * FP_RF3_PER_RAY_STEP[(c, p)])
-                          * j.ray_steps / (kms * 1e-3) / pk})
+                          "traffic": NCU_DRAM_BYTES.get((c, p)) if not scan else None, **fractions(cn, j.ray_steps, kms, pk, p)})
+            j.close()
+            del j
+            torch.cuda.empty_cache()
+        for p in ("f64", "f32"):      # the second ensemble workload: full orbits, rt_orbit
+            j = OrbitJob(rt, torch, p)
+            _, kms = time_steps(torch, j, 3, 1, flush)
+            pk, _ = rt.fma_peak(p, 100.0)
+            extra.append({"workload": "orbits: 10 keV deuterons in config 4's tokamak, 2^20 particles x 1000 steps, trajectory "
+                                      "every 10 steps + energy drift (rt_orbit)", "dtype": p,
+                          "value": j.ray_steps / (kms * 1e-3), "unit": "particle-steps/s", "kernel_ms": kms,
+                          "kernel": "rt::orbit_kernel", "traffic": NCU_DRAM_BYTES.get(("orbit4", p)),
+                          **fractions(ORBIT_COUNTS[p], j.ray_steps, kms, pk, p)})
             j.close()
             del j
             torch.cuda.empty_cache()
@@ -378,11 +464,10 @@ def run_ours(args) -> int:
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": prec, "data": "synthetic",
-                "config": {"workload": WORKLOAD_NAMES[cfg], "n_rays_per_gpu": n_rays, "n_steps": inputs.FULL_SIZES[cfg][1],
-                           "l2": "flushed between steps (256 MiB memset)", "sharding": "independent ray batches per GPU, no collective",
-                           "launch_states": "rt_launch kernel, max |D0| = %.1e" % launch_residual},
+                "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
+                "dtype": prec, "data": "synthetic", "config": workload_config(cfg, args.scaling),
+                "run": {"launch_states": "rt_launch kernel, max |D0| = %.1e" % launch_residual,
+                        "rays_this_rank": n_rays if args.scaling == "weak" else list(sharding.ray_range(n_rays, rank, world))},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "checks": {"max_abs_D": red[0], "mean_abs_D": red[1] / max(red[2], 1.0), "status_counts": red[3:6]},
                 "cpu_baseline": cpu, "other_configs": extra}

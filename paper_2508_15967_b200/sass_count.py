@@ -1,4 +1,5 @@
-"""Count the floating-point work of one ray-step in the compiled ``trace_kernel`` instantiations (``cuobjdump -sass``).
+"""Count the floating-point work of one ray-step (particle-step) in the compiled ``trace_kernel`` and ``orbit_kernel``
+instantiations (``cuobjdump -sass``).
 
     python -m paper_2508_15967_b200.sass_count            # table for every trace kernel in librt_b200.so
 
@@ -92,7 +93,8 @@ def _rf3(ins, lo, hi, fp_ops):
 
 
 def count_kernels(lib: Path = LIB) -> dict:
-    """{(precision 'f64'|'f32', eq_kind, disp_kind): {'instr', 'executed', 'mufu', 'rsqrt', 'flops'}} per ray-step."""
+    """{(precision 'f64'|'f32', eq_kind, disp_kind | 'orbit'): {'instr', 'rf3', 'executed', 'mufu', 'rsqrt', 'flops',
+    'local'}} per ray-step (particle-step for the orbit kernels)."""
     exe = cuobjdump()
     if exe is None:
         raise RuntimeError("cuobjdump not found")
@@ -100,9 +102,13 @@ def count_kernels(lib: Path = LIB) -> dict:
     res = {}
     for fn in re.split(r"\n\s*Function : ", sass):
         m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)ELb0ELb0E", fn)      # the plain single-frequency kernels
-        if not m:
+        mo = re.match(r"_ZN2rt12orbit_kernelI([df])Li(\d)EE", fn)                   # the second workload (rt_orbit)
+        if not m and not mo:
             continue
-        prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
+        if m:
+            prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
+        else:
+            prec, eq, disp = mo.group(1), int(mo.group(2)), "orbit"
         ins = _parse(fn)
         fp_ops = _FP[prec]
         # Loop nest of the kernel = its backward branches.  The loops that hold FP-pipe instructions are nested:
@@ -146,6 +152,7 @@ if __name__ == "__main__":
     names = {0: "parabolic", 1: "linear", 2: "tokamak", 3: "grid", 4: "tokamak_pow"}
     disps = {0: "O", 1: "X", 2: "full"}
     print(f"{'kernel':34s} {'instr':>6s} {'rf3':>5s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s} {'local':>6s}")
-    for (prec, eq, disp), r in sorted(count_kernels().items()):
-        print(f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}> {r['instr']:6d} {r['rf3']:5d} {r['executed']:9d} {r['mufu']:5d} "
+    for (prec, eq, disp), r in sorted(count_kernels().items(), key=lambda kv: (kv[0][2] == "orbit", kv[0][0], kv[0][1], str(kv[0][2]))):
+        name = f"orbit_kernel<{prec}, {names[eq]:11s}>      " if disp == "orbit" else f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}>"
+        print(f"{name} {r['instr']:6d} {r['rf3']:5d} {r['executed']:9d} {r['mufu']:5d} "
               f"{r['rsqrt']:6d} {r['flops']:6d} {r['local']:6d}")

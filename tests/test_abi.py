@@ -130,6 +130,17 @@ def test_orbit_and_diagnostics_argument_checks_come_before_cuda(lib):
     assert kx(tol=0.0) == binding.RT_ERR_INVALID and kx(tol=float("nan")) == binding.RT_ERR_INVALID
     assert kx(n=0) == binding.RT_OK
     assert kx() in (binding.RT_ERR_INVALID, binding.RT_ERR_CUDA)            # host pointers: no CPU fallback
+    until = lambda eq=slab, disp=1, omega=1e11, n=8, chunk=10, chunks=5, tol=float("inf"), info=P(buf.ctypes.data): \
+        lib.rt_trace_until(eq.handle if eq else None, disp, 0, P(buf.ctypes.data), P(buf.ctypes.data), omega, n, chunk, chunks,
+                           1e-3, tol, P(buf.ctypes.data), P(buf.ctypes.data), P(buf.ctypes.data), info, None)
+    assert until(eq=None) == binding.RT_ERR_INVALID
+    assert until(eq=par) == binding.RT_ERR_UNSUPPORTED
+    assert until(omega=-1.0) == binding.RT_ERR_INVALID
+    assert until(chunk=0) == binding.RT_ERR_INVALID and until(chunks=-1) == binding.RT_ERR_INVALID
+    assert until(tol=0.0) == binding.RT_ERR_INVALID and until(tol=float("nan")) == binding.RT_ERR_INVALID
+    assert until(n=-1) == binding.RT_ERR_INVALID
+    assert until(info=None) == binding.RT_ERR_INVALID                      # out_info is required even for zero rays
+    assert until() in (binding.RT_ERR_INVALID, binding.RT_ERR_CUDA)         # host pointers: no CPU fallback
     slab.close()
     par.close()
 
@@ -181,6 +192,9 @@ def test_flop_tables_match_the_compiled_kernels(lib):
         assert got["flops"] == flops, (cfg, prec, got)
         assert got["instr"] == bench.FP_INSTR_PER_RAY_STEP[(cfg, prec)], (cfg, prec, got)
         assert got["rf3"] == bench.FP_RF3_PER_RAY_STEP[(cfg, prec)], (cfg, prec, got)
+    for prec, c in bench.ORBIT_COUNTS.items():
+        got = counted[(prec, *bench.ORBIT_KERNEL)]
+        assert (got["flops"], got["instr"], got["rf3"]) == (c["flops"], c["instr"], c["rf3"]), (prec, got)
     # spills would show up as local-memory traffic: no trace kernel may execute a local load / store inside a ray-step,
     # and what ptxas parks outside the step loop (store staging: once per ray) stays below 64 bytes
     assert all(r["local"] == 0 for r in counted.values()), {k: r["local"] for k, r in counted.items() if r["local"]}
