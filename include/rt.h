@@ -223,24 +223,8 @@ int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void
                    int64_t n_rays, int64_t chunk_steps, int64_t max_chunks, double dt, double tol, void* out_final,
                    void* out_residual, int32_t* out_status, int64_t* out_info, void* cuda_stream);
 
-/* Measured roofline denominator: run >= min_ms milliseconds of independent dependent-chain FMA accumulators (DFMA
- * for RT_F64, FFMA for RT_F32) on every SM and report the sustained rate.  Synchronous.
- *   fma_per_s     HOST out: fused multiply-adds per second (flop/s = 2x)
- *   sm_clock_mhz  HOST out: average SM clock over the run derived from clock64()/globaltimer; or NULL */
-int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz);
-
-/* The same microbenchmark with its instruction shape and occupancy exposed (evidence for DESIGN.md section 6's
- * "practical ceiling of the pipe"; rt_fma_peak is shape 0 with 4 blocks per SM).
- *   shape          0: acc = acc * a + acc (two distinct source registers);  1: acc = acc * a + b, a and b shared by all
- *                  chains (three distinct sources, two of them served by the operand-reuse cache);  2: acc_j = acc_j *
- *                  a_j + b_j with per-chain a_j, b_j (every instruction reads three registers from the register file);
- *                  3: shape 0 plus 4 independent MUFU reciprocal seeds per 16 FMAs (the seeds are not counted);
- *                  4: shape 0 with one chain per thread (rate = warps per scheduler / dependent-issue latency)
- *   blocks_per_sm  1..8 blocks of 256 threads per SM, i.e. 2..16 warps per scheduler
- * Errors: RT_ERR_INVALID for an unknown precision / shape / blocks_per_sm outside [1, 8] / min_ms outside (0, 10000]
- * / fma_per_s NULL (all checked before the first CUDA call); RT_ERR_CUDA when no device is usable. */
-int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
-                      double* sm_clock_mhz);
+/* The measurement entry points (the roofline denominator rt_fma_peak and its instruction-shape variants) are declared in
+ * include/rt_bench.h: they are part of the library, not of the ray-tracing interface. */
 
 /* Number of kernel launches this library has enqueued on the calling process so far (for bench.py's gpu_launches). */
 int64_t rt_launch_count(void);

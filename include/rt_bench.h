@@ -1,0 +1,39 @@
+/* rt_bench.h -- measurement entry points of librt_b200.so (NOT part of the ray-tracing interface of rt.h).
+ *
+ * bench.py reports the hot path against a roofline whose denominator is measured in the same process ("a
+ * microbenchmark of >= 8 independent dependent-chain DFMA (resp. FFMA) accumulators per thread ... reporting FMA/s and the
+ * SM clock observed").  rt_fma_peak is that microbenchmark; rt_fma_peak_shape runs it at other instruction shapes and
+ * occupancies, the evidence behind DESIGN.md section 6's operand-port model of the FP64 / FP32 pipe.  Both are
+ * synchronous, allocate and free their own scratch, and use the current device.  Return codes as in rt.h. */
+#ifndef RT_B200_RT_BENCH_H
+#define RT_B200_RT_BENCH_H
+
+#include "rt.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Measured roofline denominator: run >= min_ms milliseconds of independent dependent-chain FMA accumulators (DFMA
+ * for RT_F64, FFMA for RT_F32) on every SM and report the sustained rate.  Synchronous.
+ *   fma_per_s     HOST out: fused multiply-adds per second (flop/s = 2x)
+ *   sm_clock_mhz  HOST out: average SM clock over the run derived from clock64()/globaltimer; or NULL */
+int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz);
+
+/* The same microbenchmark with its instruction shape and occupancy exposed (evidence for DESIGN.md section 6's
+ * "practical ceiling of the pipe"; rt_fma_peak is shape 0 with 4 blocks per SM).
+ *   shape          0: acc = acc * a + acc (two distinct source registers);  1: acc = acc * a + b, a and b shared by all
+ *                  chains (three distinct sources, two of them served by the operand-reuse cache);  2: acc_j = acc_j *
+ *                  a_j + b_j with per-chain a_j, b_j (every instruction reads three registers from the register file);
+ *                  3: shape 0 plus 4 independent MUFU reciprocal seeds per 16 FMAs (the seeds are not counted);
+ *                  4: shape 0 with one chain per thread (rate = warps per scheduler / dependent-issue latency)
+ *   blocks_per_sm  1..8 blocks of 256 threads per SM, i.e. 2..16 warps per scheduler
+ * Errors: RT_ERR_INVALID for an unknown precision / shape / blocks_per_sm outside [1, 8] / min_ms outside (0, 10000]
+ * / fma_per_s NULL (all checked before the first CUDA call); RT_ERR_CUDA when no device is usable. */
+int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
+                      double* sm_clock_mhz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_B200_RT_BENCH_H */

@@ -60,7 +60,8 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        lib = ctypes.CDLL(str(build()))
+        # RT_ORACLE_LIB: load an alternative build of rt_oracle.cpp (tests/test_sanitizers.py: the ASan / UBSan build)
+        lib = ctypes.CDLL(os.environ.get("RT_ORACLE_LIB") or str(build()))
         P, D, I64, I32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_int
         lib.oracle_trace.argtypes = [ctypes.POINTER(_CEq), I32, P, P, D, I64, I64, D, I64, P, P, P, P, I32]
         lib.oracle_trace_w.argtypes = [ctypes.POINTER(_CEq), I32, P, P, P, I64, I64, D, I64, P, P, P, P, I32]

@@ -449,15 +449,3 @@ def fma_peak_shape(precision="f64", shape: int = 0, blocks_per_sm: int = 4, min_
     p = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
     _check(lib.rt_fma_peak_shape(p, int(shape), int(blocks_per_sm), float(min_ms), ctypes.byref(rate), ctypes.byref(mhz)))
     return rate.value, mhz.value
-
-
-if __name__ == "__main__":      # python -m paper_2508_15967_b200.binding : print the microbenchmark's shape table
-    print("| precision | shape | warps / scheduler | FMA per clock per SM | TFMA/s | SM MHz |\n|---|---|---|---|---|---|")
-    import torch
-    sms = torch.cuda.get_device_properties(0).multi_processor_count
-    for prec in ("f64", "f32"):
-        for shape in (0, 1, 2, 3, 4):
-            for bps in (1, 2, 4, 8):
-                r, mhz = fma_peak_shape(prec, shape, bps, 100.0)
-                print(f"| {prec} | {('acc*a+acc', 'acc*a+b', 'acc_j*a_j+b_j', 'acc*a+acc, + 4 MUFU per 16', 'acc*a+acc, one chain')[shape]} | {2 * bps} | {r / (mhz * 1e6) / sms:.1f} | "
-                      f"{r / 1e12:.2f} | {mhz:.0f} |")

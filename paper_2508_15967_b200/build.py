@@ -11,7 +11,7 @@ _HERE = Path(__file__).resolve().parent
 CSRC = _HERE / "csrc"
 LIB = _HERE / "librt_b200.so"
 SOURCES = ("rt_api.cu", "spline_fit.cpp")
-HEADERS = ("rt_math.cuh", "rt_kernels.cuh", "rt_params.h", "spline_fit.h", "../../include/rt.h")
+HEADERS = ("rt_math.cuh", "rt_kernels.cuh", "rt_params.h", "spline_fit.h", "../../include/rt.h", "../../include/rt_bench.h")
 NVCC_FLAGS = ("-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-shared", "-Xptxas", "-v")
 

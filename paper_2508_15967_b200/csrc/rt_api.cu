@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "../../include/rt.h"
+#include "../../include/rt_bench.h"
 #include "rt_kernels.cuh"
 #include "rt_params.h"
 #include "spline_fit.h"
@@ -66,12 +67,25 @@ rt::Params<T> make_params(const rt_equilibrium* eq, double omega) {
                             reinterpret_cast<const T*>(eq->prof_pp32));
 }
 
+// The grid kind's tables (and the host pipeline's workspace) live on the device that was current when they were created:
+// a call made with another device current would dereference foreign memory.
+int check_device(const rt_equilibrium* eq) {
+  if (!eq || !(eq->psi_pp64 || eq->slot[0])) return RT_OK;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cudaGetDevice"); }
+  if (dev != eq->device)
+    return fail(RT_ERR_INVALID, "this equilibrium handle was created on CUDA device " + std::to_string(eq->device) +
+                                    " but device " + std::to_string(dev) + " is current");
+  return RT_OK;
+}
+
 int check_combo(const rt_equilibrium* eq, int disp) {
   if (!eq) return fail(RT_ERR_INVALID, "equilibrium handle is NULL");
   if (disp < RT_DISP_OMODE || disp > RT_DISP_COLD_FULL) return fail(RT_ERR_INVALID, "unknown dispersion kind");
   if (eq->d.kind == RT_EQ_SLAB_PARABOLIC && disp != RT_DISP_OMODE)
     return fail(RT_ERR_UNSUPPORTED, "the parabolic slab has no magnetic field: only RT_DISP_OMODE is defined on it");
-  return RT_OK;
+  return check_device(eq);
 }
 
 int check_omega(double omega) {
@@ -242,11 +256,15 @@ int upload(const std::vector<double>& src, T** dst) {
 
 void free_handle(rt_equilibrium* eq) {
   if (!eq) return;
+  int cur = -1;
+  const bool owns = eq->psi_pp64 || eq->slot[0] || eq->streams[0];
+  if (owns && cudaGetDevice(&cur) == cudaSuccess && cur != eq->device) cudaSetDevice(eq->device); else cur = -1;
   cudaFree(eq->psi_pp64); cudaFree(eq->prof_pp64); cudaFree(eq->psi_pp32); cudaFree(eq->prof_pp32);
   for (int s = 0; s < 2; ++s) {
     if (eq->slot[s]) cudaFree(eq->slot[s]);
     if (eq->streams[s]) cudaStreamDestroy(eq->streams[s]);
   }
+  if (cur >= 0) cudaSetDevice(cur);
   delete eq;
 }
 
@@ -492,6 +510,7 @@ int rt_orbit(const rt_equilibrium* eq, int precision, const void* x0, const void
   if (!eq) return fail(RT_ERR_INVALID, "equilibrium handle is NULL");
   if (eq->d.kind == RT_EQ_SLAB_PARABOLIC)
     return fail(RT_ERR_UNSUPPORTED, "the parabolic slab has no magnetic field: orbits are not defined on it");
+  if (int rcd = check_device(eq)) return rcd;
   if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
   if (!std::isfinite(charge_over_mass)) return fail(RT_ERR_INVALID, "charge_over_mass must be finite");
   if (n < 0 || n_steps < 0) return fail(RT_ERR_INVALID, "n and n_steps must be >= 0");
@@ -531,10 +550,14 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
   if (C > n_rays) C = (n_rays + 1023) / 1024 * 1024;
   const size_t need = per_ray * (size_t)C + 256;
   if (!eq->streams[0]) {
+    if (!eq->psi_pp64) RT_CUDA(cudaGetDevice(&eq->device));      // analytic kinds: the workspace's device
     for (int s = 0; s < 2; ++s) RT_CUDA(cudaStreamCreateWithFlags(&eq->streams[s], cudaStreamNonBlocking));
   }
+  // nothing else runs on the handle's two streams: waiting for them (not for the device) is enough before the workspace
+  // is reallocated, and before returning on an error path while copies into the caller's buffers may still be in flight
+  auto drain = [&]() { cudaStreamSynchronize(eq->streams[0]); cudaStreamSynchronize(eq->streams[1]); };
   if (eq->slot_bytes < need) {
-    RT_CUDA(cudaDeviceSynchronize());
+    drain();
     for (int s = 0; s < 2; ++s) {
       if (eq->slot[s]) { cudaFree(eq->slot[s]); eq->slot[s] = nullptr; }
     }
@@ -542,6 +565,11 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
     for (int s = 0; s < 2; ++s) RT_CUDA(cudaMalloc(&eq->slot[s], need));
     eq->slot_bytes = need;
   }
+#define RT_CUDA_DRAIN(call)                                           \
+  do {                                                                \
+    cudaError_t e_ = (call);                                          \
+    if (e_ != cudaSuccess) { drain(); return cuda_fail(e_, #call); }  \
+  } while (0)
   const char* hx = static_cast<const char*>(x0);
   const char* hk = static_cast<const char*>(k0);
   int j = 0;
@@ -556,8 +584,8 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
     char* dres = base;               base += (size_t)n_res * (size_t)C * es;
     char* dstat = base;
     const size_t w = (size_t)c * es, hp = (size_t)n_rays * es;
-    RT_CUDA(cudaMemcpy2DAsync(dx, w, hx + (size_t)off * es, hp, w, 3, cudaMemcpyHostToDevice, st));
-    RT_CUDA(cudaMemcpy2DAsync(dk, w, hk + (size_t)off * es, hp, w, 3, cudaMemcpyHostToDevice, st));
+    RT_CUDA_DRAIN(cudaMemcpy2DAsync(dx, w, hx + (size_t)off * es, hp, w, 3, cudaMemcpyHostToDevice, st));
+    RT_CUDA_DRAIN(cudaMemcpy2DAsync(dk, w, hk + (size_t)off * es, hp, w, 3, cudaMemcpyHostToDevice, st));
     void* t = out_traj ? dtraj : nullptr;
     void* f = out_final ? dfin : nullptr;
     void* r = out_residual ? dres : nullptr;
@@ -566,16 +594,17 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
       rc = trace_device<double>(eq, disp, dx, dk, omega, nullptr, c, n_steps, dt, save_stride, t, f, r, s, st);
     else
       rc = trace_device<float>(eq, disp, dx, dk, omega, nullptr, c, n_steps, dt, save_stride, t, f, r, s, st);
-    if (rc) { cudaDeviceSynchronize(); return rc; }
+    if (rc) { drain(); return rc; }
     if (out_traj)
-      RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_traj) + (size_t)off * es, hp, dtraj, w, w, (size_t)n_saved * 6, cudaMemcpyDeviceToHost, st));
+      RT_CUDA_DRAIN(cudaMemcpy2DAsync(static_cast<char*>(out_traj) + (size_t)off * es, hp, dtraj, w, w, (size_t)n_saved * 6, cudaMemcpyDeviceToHost, st));
     if (out_final)
-      RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_final) + (size_t)off * es, hp, dfin, w, w, 6, cudaMemcpyDeviceToHost, st));
+      RT_CUDA_DRAIN(cudaMemcpy2DAsync(static_cast<char*>(out_final) + (size_t)off * es, hp, dfin, w, w, 6, cudaMemcpyDeviceToHost, st));
     if (out_residual)
-      RT_CUDA(cudaMemcpy2DAsync(static_cast<char*>(out_residual) + (size_t)off * es, hp, dres, w, w, (size_t)n_res, cudaMemcpyDeviceToHost, st));
+      RT_CUDA_DRAIN(cudaMemcpy2DAsync(static_cast<char*>(out_residual) + (size_t)off * es, hp, dres, w, w, (size_t)n_res, cudaMemcpyDeviceToHost, st));
     if (out_status)
-      RT_CUDA(cudaMemcpyAsync(out_status + off, dstat, (size_t)c * 4, cudaMemcpyDeviceToHost, st));
+      RT_CUDA_DRAIN(cudaMemcpyAsync(out_status + off, dstat, (size_t)c * 4, cudaMemcpyDeviceToHost, st));
   }
+#undef RT_CUDA_DRAIN
   RT_CUDA(cudaStreamSynchronize(eq->streams[0]));
   RT_CUDA(cudaStreamSynchronize(eq->streams[1]));
   return RT_OK;
@@ -724,6 +753,7 @@ int rt_diagnostics(const rt_equilibrium* eq, const double* x, const double* k, d
                    int64_t n, double* out, void* cuda_stream) {
   if (!eq) return fail(RT_ERR_INVALID, "equilibrium handle is NULL");
   int rc;
+  if ((rc = check_device(eq))) return rc;
   if (!omega_rays && (rc = check_omega(omega))) return rc;
   if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
   if (n == 0) return RT_OK;

@@ -23,22 +23,15 @@ namespace rt {
 // does not spill (profiles/r1_tuning.md).  So the register cap (`__maxnreg__`) is simply the smallest one without spills
 // inside the step, with 64-thread blocks so that the register file divides evenly:
 //   fp64, analytic equilibria   120 registers -> 8 blocks = 16 warps per SM
-//   fp64, grid equilibrium      112 registers -> 9 blocks = 18 warps per SM (96 spills inside the stage loop)
+//   fp64, grid equilibrium      112 registers -> 9 blocks = 18 warps per SM (no spills inside the rolled stage loop)
 //   fp32                         72 registers -> 14 blocks = 28 warps per SM (the grid kernel's LDS latency likes warps:
 //                                321 ms at 72 registers, 344 ms at 128)
-// The diagnostic kernels (rhs, launch, diag) use plain 128-thread blocks.
-#ifndef RT_GRID_ROLLED
-#define RT_GRID_ROLLED 1      // grid equilibrium: one copy of the stage code (stage loop not unrolled)
-#endif
+// The grid equilibrium keeps ONE copy of the stage code (stage loop not unrolled: unrolled it needs >= 168 registers and
+// is slower at every cap, profiles/r1_tuning.md).  The diagnostic kernels (rhs, launch, diag) use plain 128-thread blocks.
 constexpr int AUX_BLOCK = 128;
-template <class T, int EQ> struct TraceTune { static constexpr int BLOCK = 64, MAXNREG = 72; };
-template <int EQ> struct TraceTune<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
-template <> struct TraceTune<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 112; };
-#ifdef RT_TRACE_BLOCK       // experiments: one shape for every trace kernel
-template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = RT_TRACE_BLOCK, MAXNREG = RT_MAXNREG; };
-#else
-template <class T, int EQ> struct TraceShape : TraceTune<T, EQ> {};
-#endif
+template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = 64, MAXNREG = 72; };
+template <int EQ> struct TraceShape<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
+template <> struct TraceShape<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 112; };
 
 template <class T>
 struct TraceArgs {
@@ -75,7 +68,7 @@ RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
   T k[6], acc[6], ys[6], r;          // the slope of a stage is r k (ray_rhs): r is folded into the step-size factors
   bool ok = true;
-  if (EQ == EQ_GRID && RT_GRID_ROLLED) {
+  if (EQ == EQ_GRID) {
 #pragma unroll
     for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; }
     T ar = T(0);                     // a_st r_{st-1}
@@ -136,7 +129,7 @@ RT_DEV T abs_residual(const Params<T>& P, const T* y, Gather& gather) {
 // Shared-memory cell cache of the grid equilibrium.  A ray moves ~1 mm per RK4 step through 5.9 mm cells, so the 16
 // psi pieces (one 128-B line in fp64) and the 8 profile pieces it needs are the same for many consecutive stages.  Read
 // straight from global memory, every 128-bit load of a warp touches 32 different lines and the L1 data pipe saturates
-// (99.8 % `l1tex__data_pipe_lsu_wavefronts`, FP64 pipe 43 %: profiles/r1_cfg5_ncu.md).  Here each thread keeps its
+// (99.8 % `l1tex__data_pipe_lsu_wavefronts`, FP64 pipe 43 %: round-1 capture, profiles/README.md "history").  Here each thread keeps its
 // current cell's pieces in its own column of a [chunk][thread] shared array -- 16-byte chunks, consecutive threads in
 // consecutive chunks, so a warp's LDS.128 is 4 conflict-free wavefronts -- and refills the column from global memory
 // only when its cell index changes.  The column is private to the thread: no barrier is needed.
