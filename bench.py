@@ -49,17 +49,20 @@ UNIT = "ray-steps/s"
 # (its Newton refinement is NOT counted).  FP_INSTR_PER_RAY_STEP is what the FP64 / FP32 pipe actually issues per
 # ray-step (FMA, MUL, ADD, SETP instructions, refinements included).  Both tables are counted from the compiled kernels by
 # paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
-FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 259, (4, "f64"): 794, (5, "f64"): 1260,
-                      (1, "f32"): 115, (2, "f32"): 115, (3, "f32"): 262, (4, "f32"): 798, (5, "f32"): 1257}
-FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f64"): 624, (5, "f64"): 884,
-                         (1, "f32"): 69, (2, "f32"): 69, (3, "f32"): 178, (4, "f32"): 538, (5, "f32"): 819}
+FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 259, (4, "f64"): 767, (5, "f64"): 1252,
+                      (1, "f32"): 117, (2, "f32"): 117, (3, "f32"): 262, (4, "f32"): 771, (5, "f32"): 1252}
+FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f64"): 597, (5, "f64"): 876,
+                         (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 178, (4, "f32"): 512, (5, "f32"): 814}
 # FP_RF3_PER_RAY_STEP: how many of those instructions read THREE DISTINCT registers from the register file.  Such an instruction
-# occupies the FP64 pipe for 3 cycles instead of 2 (FP32: 1.56 instead of 1) -- measured by rt_fma_peak_shape, shape 2
-# (profiles/r1_fma_peak_shapes.md) -- so the pipe time of a ray-step is (instr + RF3_EXTRA * rf3) issue slots of the FMA
-# microbenchmark; `pipe_model_frac` is that time over the measured kernel time.
-FP_RF3_PER_RAY_STEP = {(1, "f64"): 26, (2, "f64"): 26, (3, "f64"): 39, (4, "f64"): 169, (5, "f64"): 328,
-                       (1, "f32"): 29, (2, "f32"): 29, (3, "f32"): 39, (4, "f32"): 157, (5, "f32"): 268}
-RF3_EXTRA = {"f64": 0.5, "f32": 0.563}      # shape 0 rate / shape 2 rate - 1:  63.9 / 42.7 = 1.50,  123.2 / 78.8 = 1.563
+# occupies the FP64 pipe for 3 cycles instead of 2 (scalar FP32: 1.56 slots instead of 1; packed f32x2: 3 cycles instead of 2) -- measured by
+# rt_fma_peak_shape, shapes 2 / 6 (profiles/r1_fma_peak_shapes.md, r2_fma_peak_shapes.md) -- so the pipe time of a ray-step is
+# (instr + RF3_EXTRA * rf3) issue slots of the FMA microbenchmark; `pipe_model_frac` is that time over the measured kernel
+# time.  The fp32 kernels of the analytic equilibria (configs 1-4) are the packed two-rays-per-thread
+# kernels (trace_kernel_x2); their counts are per ray (a packed instruction = one slot per ray).
+FP_RF3_PER_RAY_STEP = {(1, "f64"): 29, (2, "f64"): 29, (3, "f64"): 42, (4, "f64"): 160, (5, "f64"): 332,
+                       (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 48, (4, "f32"): 161, (5, "f32"): 260}
+RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1: 63.9 / 42.7, 123.2 / 78.8; packed 127.9 / 84.9
+PACKED = {(c, "f32") for c in (1, 2, 3, 4)}              # (config, precision) pairs that run trace_kernel_x2
 # The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from
 # sass_count.py's orbit_kernel rows (pinned by the same test).
 ORBIT_COUNTS = {"f64": dict(flops=248, instr=188, rf3=44), "f32": dict(flops=248, instr=166, rf3=32)}
@@ -342,11 +345,16 @@ def time_steps(torch, job: Job, steps: int, warmup: int, flush, barrier=None):
     return t0.elapsed_time(t1), statistics.fmean(a.elapsed_time(b) for a, b in ev)
 
 
-def fractions(counts: dict, units: float, kernel_ms: float, fma_rate: float, prec: str) -> dict:
-    """The three fractions of DESIGN.md section 6 for one kernel launch of `units` ray-steps (particle-steps)."""
+def fractions(counts: dict, units: float, kernel_ms: float, fma_rate: float, flavour: str) -> dict:
+    """The three fractions of DESIGN.md section 6 for one kernel launch of `units` ray-steps (particle-steps);
+    flavour = 'f64' | 'f32' | 'f32x2' selects the cost of a three-register instruction."""
     per_s = units / (kernel_ms * 1e-3)
     return {"roofline_frac": counts["flops"] * per_s / (2.0 * fma_rate), "pipe_frac": counts["instr"] * per_s / fma_rate,
-            "pipe_model_frac": (counts["instr"] + RF3_EXTRA[prec] * counts["rf3"]) * per_s / fma_rate}
+            "pipe_model_frac": (counts["instr"] + RF3_EXTRA[flavour] * counts["rf3"]) * per_s / fma_rate}
+
+
+def flavour(cfg: int, prec: str) -> str:
+    return "f32x2" if (cfg, prec) in PACKED else prec
 
 
 def run_ours(args) -> int:
@@ -414,12 +422,13 @@ def run_ours(args) -> int:
 
     counts = {"flops": FLOPS_PER_RAY_STEP[(cfg, prec)], "instr": FP_INSTR_PER_RAY_STEP[(cfg, prec)],
               "rf3": FP_RF3_PER_RAY_STEP[(cfg, prec)]}
-    fr = fractions(counts, job.ray_steps, kernel_ms, peak_after, prec)
+    fr = fractions(counts, job.ray_steps, kernel_ms, peak_after, flavour(cfg, prec))
     launch_residual = job.launch_residual
     peak = 2.0 * peak_after
     roofline = {"bound": "alu", "achieved": fr["roofline_frac"] * peak / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
                 "frac": fr["roofline_frac"], "traffic": NCU_DRAM_BYTES.get((cfg, prec)),
-                "kernel": f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
+                "kernel": "rt::trace_kernel_x2 (packed f32x2, two rays per thread)" if (cfg, prec) in PACKED
+                else f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
                 "kernel_ms": kernel_ms, "flops_per_ray_step": counts["flops"], "fp_instr_per_ray_step": counts["instr"],
                 "fp_rf3_per_ray_step": counts["rf3"], "pipe_frac": fr["pipe_frac"], "pipe_model_frac": fr["pipe_model_frac"],
                 "peak_source": f"rt_fma_peak({prec}) measured in this process after the timed region: "
@@ -441,7 +450,8 @@ def run_ours(args) -> int:
             cn = {"flops": FLOPS_PER_RAY_STEP[(c, p)], "instr": FP_INSTR_PER_RAY_STEP[(c, p)], "rf3": FP_RF3_PER_RAY_STEP[(c, p)]}
             extra.append({"workload": f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else ""),
                           "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
-                          "traffic": NCU_DRAM_BYTES.get((c, p)) if not scan else None, **fractions(cn, j.ray_steps, kms, pk, p)})
+                          "traffic": NCU_DRAM_BYTES.get((c, p)) if not scan else None,
+                          **fractions(cn, j.ray_steps, kms, pk, flavour(c, p) if not scan else p)})
             j.close()
             del j
             torch.cuda.empty_cache()

@@ -21,14 +21,17 @@ extern "C" {
 int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz);
 
 /* The same microbenchmark with its instruction shape and occupancy exposed (evidence for DESIGN.md section 6's
- * "practical ceiling of the pipe"; rt_fma_peak is shape 0 with 4 blocks per SM).
+ * "practical ceiling of the pipe"; rt_fma_peak is shape 0 -- for RT_F32 shape 5 -- with 4 blocks per SM).
  *   shape          0: acc = acc * a + acc (two distinct source registers);  1: acc = acc * a + b, a and b shared by all
  *                  chains (three distinct sources, two of them served by the operand-reuse cache);  2: acc_j = acc_j *
  *                  a_j + b_j with per-chain a_j, b_j (every instruction reads three registers from the register file);
  *                  3: shape 0 plus 4 independent MUFU reciprocal seeds per 16 FMAs (the seeds are not counted);
- *                  4: shape 0 with one chain per thread (rate = warps per scheduler / dependent-issue latency)
+ *                  4: shape 0 with one chain per thread (rate = warps per scheduler / dependent-issue latency);
+ *                  fp32 only: 5 / 6 = shapes 0 / 2 issued as packed f32x2 instructions (FFMA2: two fused multiply-adds per
+ *                  instruction and lane; rates are always reported in fused multiply-adds, not instructions).
+ *                  rt_fma_peak(RT_F32) is shape 5, the best the FP32 FMA pipe delivers
  *   blocks_per_sm  1..8 blocks of 256 threads per SM, i.e. 2..16 warps per scheduler
- * Errors: RT_ERR_INVALID for an unknown precision / shape / blocks_per_sm outside [1, 8] / min_ms outside (0, 10000]
+ * Errors: RT_ERR_INVALID for an unknown precision / shape (5 and 6 exist for RT_F32 only) / blocks_per_sm outside [1, 8] / min_ms outside (0, 10000]
  * / fma_per_s NULL (all checked before the first CUDA call); RT_ERR_CUDA when no device is usable. */
 int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
                       double* sm_clock_mhz);

@@ -109,9 +109,33 @@ unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / 
   M(rt::EQ_TOKAMAK_POW, rt::DISP_O) M(rt::EQ_TOKAMAK_POW, rt::DISP_X) M(rt::EQ_TOKAMAK_POW, rt::DISP_FULL)  \
   M(rt::EQ_GRID, rt::DISP_O) M(rt::EQ_GRID, rt::DISP_X) M(rt::EQ_GRID, rt::DISP_FULL)
 
+// fp32, analytic equilibria, one frequency, no resume: the packed two-rays-per-thread kernels (rt_kernels.cuh)
+#define RT_FOR_ANALYTIC_COMBOS(M)                          \
+  M(rt::EQ_PARABOLIC, rt::DISP_O)                          \
+  M(rt::EQ_LINEAR, rt::DISP_O) M(rt::EQ_LINEAR, rt::DISP_X) M(rt::EQ_LINEAR, rt::DISP_FULL)     \
+  M(rt::EQ_TOKAMAK, rt::DISP_O) M(rt::EQ_TOKAMAK, rt::DISP_X) M(rt::EQ_TOKAMAK, rt::DISP_FULL)  \
+  M(rt::EQ_TOKAMAK_POW, rt::DISP_O) M(rt::EQ_TOKAMAK_POW, rt::DISP_X) M(rt::EQ_TOKAMAK_POW, rt::DISP_FULL)
+int launch_trace_x2(const rt_equilibrium* eq, int disp, const rt::Params<float>& P, const rt::TraceArgs<float>& A, cudaStream_t st) {
+#define M(E, D)                                                                                        \
+  if (kernel_kind(eq) == (E) && disp == (D)) {                                                         \
+    constexpr int block = rt::TraceShape2<E>::BLOCK;                                                   \
+    rt::trace_kernel_x2<E, D><<<grid_for((A.n_rays + 1) / 2, block), block, 0, st>>>(P, A);            \
+    ++g_launches;                                                                                      \
+    RT_CUDA(cudaGetLastError());                                                                       \
+    return RT_OK;                                                                                      \
+  }
+  RT_FOR_ANALYTIC_COMBOS(M)
+#undef M
+  return fail(RT_ERR_UNSUPPORTED, "no packed kernel for this equilibrium / dispersion combination");
+}
+int launch_trace_x2(const rt_equilibrium*, int, const rt::Params<double>&, const rt::TraceArgs<double>&, cudaStream_t) {
+  return fail(RT_ERR_UNSUPPORTED, "packed kernels are fp32 only");
+}
+
 template <class T>
 int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const rt::TraceArgs<T>& A, cudaStream_t st) {
   if (A.n_rays == 0) return RT_OK;
+  if (sizeof(T) == 4 && !A.omega && !A.status_in && eq->d.kind != RT_EQ_GRID_RZ) return launch_trace_x2(eq, disp, P, A, st);
 #define M(E, D)                                                                            \
   if (kernel_kind(eq) == (E) && disp == (D)) {                                             \
     constexpr int block = rt::TraceShape<T, E>::BLOCK;                                     \
@@ -119,7 +143,7 @@ int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, con
       rt::trace_kernel<T, E, D, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A);  \
     else if (A.status_in)                                                                  \
       rt::trace_kernel<T, E, D, false, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
-    else                                                                                   \
+    else if constexpr (!(sizeof(T) == 4 && (E) != rt::EQ_GRID))   /* fp32 analytic: the packed kernels, above */ \
       rt::trace_kernel<T, E, D, false><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
     ++g_launches;                                                                          \
     RT_CUDA(cudaGetLastError());                                                           \
@@ -214,6 +238,7 @@ int trace_device(const rt_equilibrium* eq, int disp, const void* x0, const void*
   A.n_steps = n_steps;
   A.stride = save_stride;
   A.h = (T)dt;
+  A.hh = T(0.5) * A.h; A.h3 = A.h * T(1.0 / 3.0); A.h6 = A.h * T(1.0 / 6.0);    // the same roundings the kernel used to make
   return launch_trace<T>(eq, disp, P, A, st);
 }
 
@@ -813,14 +838,16 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
 }
 
 int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_clock_mhz) {
-  return rt_fma_peak_shape(precision, 0, 4, min_ms, fma_per_s, sm_clock_mhz);
+  // fp32: the packed shape -- the best the chip's FP32 FMA pipe delivers, so the denominator counts FMAs, not instructions
+  return rt_fma_peak_shape(precision, precision == RT_F32 ? 5 : 0, 4, min_ms, fma_per_s, sm_clock_mhz);
 }
 
 int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
                       double* sm_clock_mhz) {
   if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
-  if (shape < 0 || shape > 4)
-    return fail(RT_ERR_INVALID, "shape must be 0 (acc*a+acc), 1 (acc*a+b, shared a, b), 2 (acc_j*a_j+b_j), 3 (0 + MUFU) or 4 (one chain)");
+  if (shape < 0 || shape > 6 || (shape >= 5 && precision != RT_F32))
+    return fail(RT_ERR_INVALID, "shape must be 0 (acc*a+acc), 1 (acc*a+b, shared a, b), 2 (acc_j*a_j+b_j), 3 (0 + MUFU), "
+                                "4 (one chain), or for fp32 5 / 6 (shapes 0 / 2 with packed f32x2 accumulators)");
   if (blocks_per_sm < 1 || blocks_per_sm > 8) return fail(RT_ERR_INVALID, "blocks_per_sm must be in [1, 8]");
   if (!fma_per_s) return fail(RT_ERR_INVALID, "fma_per_s is NULL");
   if (!(min_ms > 0.0) || min_ms > 10000.0) return fail(RT_ERR_INVALID, "min_ms must be in (0, 10000]");
@@ -853,7 +880,9 @@ int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms
       else if (shape == 3) RT_PEAK(double, 3, 1e-9, 1e-3);
       else RT_PEAK(double, 4, 1e-9, 1e-3);
     } else {
-      if (shape == 0) RT_PEAK(float, 0, 1e-7f, 1e-3f);
+      if (shape == 5) rt::fma_peak_packed_kernel<5><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 1e-7f, 1e-3f, clk);
+      else if (shape == 6) rt::fma_peak_packed_kernel<6><<<grid, rt::FMA_BLOCK>>>(static_cast<float*>(sink), iters, 0.999f, 1e-3f, clk);
+      else if (shape == 0) RT_PEAK(float, 0, 1e-7f, 1e-3f);
       else if (shape == 1) RT_PEAK(float, 1, 0.999f, 1e-3f);
       else if (shape == 2) RT_PEAK(float, 2, 0.999f, 1e-3f);
       else if (shape == 3) RT_PEAK(float, 3, 1e-7f, 1e-3f);

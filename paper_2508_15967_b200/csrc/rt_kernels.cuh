@@ -45,6 +45,7 @@ struct TraceArgs {
   long long n_steps;
   long long stride;
   T h;                  // step in tau = c t
+  T hh, h3, h6;         // h/2, h/3, h/6: the tableau's step factors, folded on the host (constant bank operands)
   const double* omega;  // per-ray frequencies [n_rays] (PW kernels only), rad/s
   double omega_ref;     // the frequency the Params were folded at
   const int32_t* status_in;   // resume (rt_trace_until's chunks): each ray's status at entry, or NULL = every ray starts
@@ -63,11 +64,12 @@ RT_DEV constexpr bool rhs_component_active(int j) {
   return !((EQ == EQ_LINEAR && j >= 4) || (EQ == EQ_PARABOLIC && j == 5));
 }
 
+// rk4_stages: the four stages of one step from y; writes the candidate new state to ys and returns whether every stage
+// point was inside the domain (per lane for the packed fp32 kernels).  rk4_step applies the acceptance rule (A12).
 template <class T, int EQ, int DISP, class Gather>
-RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
-  const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
-  T k[6], acc[6], ys[6], r;          // the slope of a stage is r k (ray_rhs): r is folded into the step-size factors
-  bool ok = true;
+RT_DEV typename Lane<T>::mask rk4_stages(const Params<T>& P, T h, T hh, T h3, T h6, const T* y, T* ys, Gather& gather) {
+  T k[6], acc[6], r;                 // the slope of a stage is r k (ray_rhs): r is folded into the step-size factors
+  typename Lane<T>::mask ok = rt_true<T>();
   if (EQ == EQ_GRID) {
 #pragma unroll
     for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; }
@@ -76,7 +78,7 @@ RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
     for (int st = 0; st < 4; ++st) {
 #pragma unroll
       for (int j = 0; j < 6; ++j) ys[j] = rt_fma(ar, k[j], y[j]);
-      ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+      ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
       const T wr = ((st == 0 || st == 3) ? h6 : h3) * r;
       ar = ((st == 2) ? h : hh) * r;
 #pragma unroll
@@ -92,21 +94,28 @@ RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
 #pragma unroll
     for (int j = 0; j < 6; ++j)
       if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], y[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+    ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
     wr = h3 * r; ar = hh * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
       if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], acc[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+    ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
     wr = h3 * r; ar = h * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
       if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], acc[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
-    ok = ray_rhs<T, EQ, DISP>(P, ys, k, r, gather) && ok;
+    ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
     wr = h6 * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j) ys[j] = rhs_component_active<EQ>(j) ? rt_fma(wr, k[j], acc[j]) : y[j];
   }
+  return ok;
+}
+
+template <class T, int EQ, int DISP, class Gather>
+RT_DEV int rk4_step(const Params<T>& P, T h, T hh, T h3, T h6, T* y, Gather& gather) {
+  T ys[6];
+  const bool ok = rk4_stages<T, EQ, DISP>(P, h, hh, h3, h6, y, ys, gather);
   if (!ok) return 1;
   bool fin = true;
 #pragma unroll
@@ -119,9 +128,9 @@ RT_DEV int rk4_step(const Params<T>& P, T h, T* y, Gather& gather) {
 
 template <class T, int EQ, int DISP, class Gather>
 RT_DEV T abs_residual(const Params<T>& P, const T* y, Gather& gather) {
-  bool inside;
+  typename Lane<T>::mask inside;
   const T D = ray_D<T, EQ, DISP>(P, y, &inside, gather);
-  return inside ? rt_abs(D) : rt_nan<T>();
+  return rt_select(inside, rt_abs(D), rt_nan<T>());
 }
 
 #ifdef __CUDACC__
@@ -298,11 +307,110 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
   for (long long m = 1; m <= n_outer; ++m) {
 #pragma unroll 1
     for (long long s = 0; s < n_inner; ++s)
-      if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, y, gather);
+      if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, A.hh, A.h3, A.h6, y, gather);
     if (A.traj) save(A.traj + m * 6 * A.n_rays, A.res ? A.res + m * A.n_rays : nullptr);
   }
   if (A.fin || (!A.traj && A.res)) save(A.fin, A.traj ? nullptr : A.res);
   if (A.status && valid) A.status[i] = status;
+}
+
+// ---- fp32, two rays per thread: packed f32x2 arithmetic (rt_math.cuh: f32x2) ------------------------------------------
+// Thread t of a block traces rays 2 (block * BLOCK + t) and the next one, one in each half of every f32x2 value; a warp
+// owns 64 consecutive rays.  Same arithmetic per ray as trace_kernel<float, ...> (the IEEE fp32 operation on each half), so
+// the two kernels give bit-identical rays; what changes is the instruction stream: one FFMA2 / FMUL2 / FADD2 issue slot
+// serves two rays, and MUFU seeds, domain tests and table look-ups are done per half.  A lane whose ray is frozen keeps
+// computing on its frozen state and is masked out of every update.
+// The packed kernels exist for the analytic equilibria.  For the grid equilibrium the same approach was measured and
+// dropped (profiles/r2_tuning.md): with two rays per thread the per-ray shared-memory cell cache needs 128 registers
+// (16 warps per SM instead of 28) and the kernel, which is bound by the LDS data pipe and the latency of the look-up
+// chain rather than by issue slots, runs 2-3 % slower than trace_kernel<float, EQ_GRID, ...>.
+template <int EQ> struct TraceShape2 { static constexpr int BLOCK = 64, MAXNREG = 128; };
+
+template <int EQ, int DISP>
+__global__ void __maxnreg__((TraceShape2<EQ>::MAXNREG))
+trace_kernel_x2(const __grid_constant__ Params<float> P0, const __grid_constant__ TraceArgs<float> A) {
+  typedef f32x2 T;
+  constexpr int BLOCK = TraceShape2<EQ>::BLOCK, RAYS = 2 * BLOCK;
+  const Params<T>& P = static_cast<const Params<T>&>(reinterpret_cast<const Params<T>&>(P0));
+  const long long N = A.n_rays;
+  const long long ia = ((long long)blockIdx.x * BLOCK + threadIdx.x) * 2, ib = ia + 1;
+  const bool va = ia < N, vb = ib < N;
+  static_assert(EQ != EQ_GRID, "the packed kernels cover the analytic equilibria");
+  GatherDirect gather;
+  __shared__ __align__(16) float stage[7 * RAYS];
+  T y[6];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    y[c] = T(va ? A.x0[c * N + ia] : 0.0f, vb ? A.x0[c * N + ib] : 0.0f);
+    y[3 + c] = T(va ? A.k0[c * N + ia] : 0.0f, vb ? A.k0[c * N + ib] : 0.0f) * P.k2n;      // n = c k / w  (Eq. 6)
+  }
+  int sa = va ? 0 : 3, sb = vb ? 0 : 3;            // 3: padding lane, never stored
+  // store: each thread drops its two rays' 7 values into columns 2 lane, 2 lane + 1 of its warp's [7][64] slice; then the
+  // warp writes the rows with 128-bit stores (16 chunks of 16 bytes per row).  Nothing of this is live across the step loop.
+  auto save = [&](float* rows6, float* res_row) {
+    const int lane = threadIdx.x & 31;
+    float* st = stage + (threadIdx.x & ~31) * 2;                                   // this warp's slice: row r at st[r * RAYS]
+    const long long i0 = ((long long)blockIdx.x * BLOCK + (threadIdx.x & ~31)) * 2;  // first ray of this warp
+    const long long NN = A.n_rays;
+    T v[7];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { v[c] = y[c]; v[3 + c] = y[3 + c] * P.n2k; }
+    v[6] = res_row ? abs_residual<T, EQ, DISP>(P, y, gather) : T(0.0f);
+    if ((NN & 3) != 0) {                                                           // rows not 16-byte aligned: scalar stores
+      const long long ja = i0 + 2 * lane;
+#pragma unroll
+      for (int c = 0; c < 7; ++c) {
+        float* dst = (c < 6) ? (rows6 ? rows6 + c * NN : nullptr) : res_row;
+        if (!dst) continue;
+        if (ja < NN) dst[ja] = v[c].lo();
+        if (ja + 1 < NN) dst[ja + 1] = v[c].hi();
+      }
+      return;
+    }
+#pragma unroll
+    for (int c = 0; c < 7; ++c) *reinterpret_cast<float2*>(st + c * RAYS + 2 * lane) = make_float2(v[c].lo(), v[c].hi());
+    __syncwarp();
+    const int first = rows6 ? 0 : 6 * 16, last = res_row ? 7 * 16 : 6 * 16;
+    for (int q = first + lane; q < last; q += 32) {
+      const int row = q >> 4, col = (q & 15) * 4;
+      if (i0 + col < NN) {
+        const float4 val = *reinterpret_cast<const float4*>(st + row * RAYS + col);
+        float* dst = (row < 6) ? rows6 + row * NN : res_row;
+        *reinterpret_cast<float4*>(dst + i0 + col) = val;
+      }
+    }
+    __syncwarp();
+  };
+  const long long n_outer = A.traj ? A.n_steps / A.stride : 1, n_inner = A.traj ? A.stride : A.n_steps;
+  if (A.traj) save(A.traj, A.res);
+  for (long long m = 1; m <= n_outer; ++m) {
+#pragma unroll 1
+    for (long long s = 0; s < n_inner; ++s) {
+      if (sa != 0 && sb != 0) break;               // both rays frozen (or padding): nothing left to do in this stretch
+      T ys[6];
+      const mask2 ok = rk4_stages<T, EQ, DISP>(P, T(A.h), T(A.hh), T(A.h3), T(A.h6), y, ys, gather);
+      mask2 fin = {true, true};
+#pragma unroll
+      for (int j = 0; j < 6; ++j) fin = rt_and(fin, rt_finite(ys[j]));
+      // acceptance rule (reading A12), per ray: a stage point outside the domain -> status 1; a non-finite new state -> 2
+      const mask2 acc = {sa == 0 && ok.a && fin.a, sb == 0 && ok.b && fin.b};
+      if (acc.a && acc.b) {                        // the common case: both rays advance, no per-half selects
+#pragma unroll
+        for (int j = 0; j < 6; ++j) y[j] = ys[j];
+      } else {
+        if (sa == 0 && !acc.a) sa = ok.a ? 2 : 1;
+        if (sb == 0 && !acc.b) sb = ok.b ? 2 : 1;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) y[j] = rt_select(acc, ys[j], y[j]);
+      }
+    }
+    if (A.traj) save(A.traj + m * 6 * A.n_rays, A.res ? A.res + m * A.n_rays : nullptr);
+  }
+  if (A.fin || (!A.traj && A.res)) save(A.fin, A.traj ? nullptr : A.res);
+  if (A.status) {
+    if (va) A.status[ia] = sa;
+    if (vb) A.status[ib] = sb;
+  }
 }
 
 // ---- second ensemble workload: full-orbit charged particles in the same equilibria -----------------
@@ -655,8 +763,12 @@ __global__ void until_decide_kernel(long long* __restrict__ info, double tol, lo
 //            determinant has 1 per 22): the seeds run on the XU pipe BESIDE the FMA pipe and cost ~2 % of the FMA rate;
 //   SHAPE 4: shape 0 with ONE chain per thread: the rate is warps-per-scheduler / dependent-issue latency (8 cycles for
 //            a DFMA), i.e. 4 warps per scheduler saturate the FP64 pipe without any instruction-level parallelism.
+//   SHAPE 5 (fp32 only; the denominator rt_fma_peak reports for fp32): shape 0 with PACKED f32x2 accumulators -- 8 chains
+//            of FFMA2, each instruction two fused multiply-adds: what the chip's FP32 FMA pipe delivers at best;
+//   SHAPE 6 (fp32 only): shape 2 with packed accumulators (three distinct 64-bit register pairs per FFMA2).
 // On B200 the DFMA rate is 63.7 / 58 / 42.7 per clock per SM for shapes 0 / 1 / 2: an FP64 instruction that reads three
-// registers from the register file occupies the pipe for 3 cycles instead of 2 (profiles/r1_fma_peak_shapes.md).
+// registers from the register file occupies the pipe for 3 cycles instead of 2 (profiles/r1_fma_peak_shapes.md).  FP32:
+// 123.2 / 117 / 78.8 scalar, 127.9 / 84.9 packed (shapes 5 / 6): the same port limit, two FMAs per issue slot.
 constexpr int FMA_CHAINS = 16;
 constexpr int FMA_BLOCK = 256;
 RT_DEV double rcp_seed(double x) { double r; asm volatile("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x)); return r; }
@@ -698,6 +810,38 @@ fma_peak_kernel(T* __restrict__ sink, long long iters, T a, T b, unsigned long l
 #pragma unroll
   for (int j = 0; j < NC; ++j) s += acc[j];
   if (SHAPE == 3) s += seed[0] + seed[1] + seed[2] + seed[3];
+  sink[(long long)blockIdx.x * FMA_BLOCK + threadIdx.x] = s;
+  if (threadIdx.x == 0 && blockIdx.x == 0) { clk[0] = (unsigned long long)(c1 - c0); clk[1] = t1 - t0; }
+}
+
+// shapes 5 / 6: the same FMA count per iteration (FMA_CHAINS x 8) issued as FMA_CHAINS / 2 packed chains
+template <int SHAPE>
+__global__ void __launch_bounds__(FMA_BLOCK)
+fma_peak_packed_kernel(float* __restrict__ sink, long long iters, float a, float b, unsigned long long* __restrict__ clk) {
+  constexpr int NC = FMA_CHAINS / 2;
+  f32x2 acc[NC], aj[NC], bj[NC];
+#pragma unroll
+  for (int j = 0; j < NC; ++j) {
+    acc[j] = f32x2(float(threadIdx.x + j) * 1e-3f, float(threadIdx.x + j + 1) * 1e-3f);
+    aj[j] = f32x2(a + float(threadIdx.x + j) * 1e-9f, a - float(j) * 1e-9f);
+    bj[j] = f32x2(b + float(threadIdx.x + 2 * j) * 1e-9f, b);
+  }
+  const f32x2 pa(a);
+  unsigned long long t0, t1;
+  const long long c0 = clock64();
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t0));
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int j = 0; j < NC; ++j) acc[j] = (SHAPE == 5) ? rt_fma(acc[j], pa, acc[j]) : rt_fma(acc[j], aj[j], bj[j]);
+    }
+  }
+  const long long c1 = clock64();
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t1));
+  float s = 0.0f;
+#pragma unroll
+  for (int j = 0; j < NC; ++j) s += acc[j].lo() + acc[j].hi();
   sink[(long long)blockIdx.x * FMA_BLOCK + threadIdx.x] = s;
   if (threadIdx.x == 0 && blockIdx.x == 0) { clk[0] = (unsigned long long)(c1 - c0); clk[1] = t1 - t0; }
 }

@@ -68,6 +68,14 @@ struct Params {
   const T* prof_pp;             // [nPc][8]: F = sum f[m] ds^m (m = 0..3), then n_e/ne_scale likewise
 };
 
+#ifdef __CUDACC__
+struct f32x2;
+template <> struct Params<f32x2> : Params<float> {      // the packed kernels take the scalar constants (broadcast at use)
+  Params() = default;
+  RT_DEV Params(const Params<float>& p) : Params<float>(p) {}
+};
+#endif
+
 RT_DEV int rt_imin(int a, int b) { return a < b ? a : b; }
 RT_DEV double rt_sqrt(double a) { return sqrt(a); }
 RT_DEV float rt_sqrt(float a) { return sqrtf(a); }
@@ -144,6 +152,73 @@ template <class T> RT_DEV bool rt_less_nonneg(T a, T b) { return a < b; }
 template <class T> RT_DEV bool rt_positive(T a) { return a > T(0); }
 #endif
 
+// ---- two rays per thread in fp32: packed f32x2 arithmetic (sm_100a FFMA2 / FMUL2 / FADD2) ---------------------------
+// The fp32 trace kernels are issue-bound, not FMA-pipe-bound (every FFMA takes a whole issue slot, and every MUFU seed,
+// integer and LDS instruction displaces one), and an FFMA that reads three distinct registers occupies the pipe for 1.56
+// slots.  A packed FFMA2 does the same arithmetic for TWO rays in ONE issue slot and two pipe cycles (127.9 FMA per clock
+// per SM against 123.2 scalar; with three distinct register operands 84.9 against 78.8: profiles/r2_fma_peak_shapes.md),
+// which moves the kernels from issue-bound to FMA-pipe-bound.
+// f32x2 holds one value of ray A (low half) and of ray B (high half); every operation is the IEEE fp32 operation on
+// each half, so a ray's result does not depend on which thread half it rides in.  A scalar (per-call constant)
+// converts implicitly: ptxas turns the broadcast into a `.F32` operand of the packed instruction.  Negation and |x| are
+// written per half so that ptxas folds them into operand modifiers.  Per-half predicates and integers are mask2 / int2v.
+template <class T> struct Lane { typedef bool mask; typedef int index; typedef T scalar; static constexpr int N = 1; };
+#ifdef __CUDACC__
+struct f32x2 {
+  unsigned long long v;
+  f32x2() = default;
+  RT_DEV f32x2(float s) { asm("mov.b64 %0, {%1, %1};" : "=l"(v) : "f"(s)); }
+  RT_DEV explicit f32x2(double s) : f32x2((float)s) {}
+  RT_DEV explicit f32x2(int s) : f32x2((float)s) {}
+  RT_DEV f32x2(float lo, float hi) { asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi)); }
+  RT_DEV float lo() const { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return a; }
+  RT_DEV float hi() const { float a, b; asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); return b; }
+};
+struct mask2 { bool a, b; };
+struct int2v { int a, b; };
+template <> struct Lane<f32x2> { typedef mask2 mask; typedef int2v index; typedef float scalar; static constexpr int N = 2; };
+RT_DEV f32x2 operator+(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+RT_DEV f32x2 operator-(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+RT_DEV f32x2 operator*(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+RT_DEV f32x2 operator-(f32x2 a) { return f32x2(-a.lo(), -a.hi()); }
+RT_DEV f32x2& operator*=(f32x2& a, f32x2 b) { a = a * b; return a; }
+RT_DEV f32x2 rt_fma(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return d;
+}
+RT_DEV f32x2 rt_abs(f32x2 a) { return f32x2(fabsf(a.lo()), fabsf(a.hi())); }
+RT_DEV f32x2 rt_floor(f32x2 a) { return f32x2(floorf(a.lo()), floorf(a.hi())); }
+RT_DEV f32x2 rt_pow(f32x2 a, f32x2 b) { return f32x2(powf(a.lo(), b.lo()), powf(a.hi(), b.hi())); }
+RT_DEV f32x2 rt_sqrt(f32x2 a) { return f32x2(sqrtf(a.lo()), sqrtf(a.hi())); }
+template <> RT_DEV f32x2 rt_nan<f32x2>() { return f32x2(nanf("")); }
+RT_DEV f32x2 rt_rcp(f32x2 x) { return f32x2(rt_rcp(x.lo()), rt_rcp(x.hi())); }
+RT_DEV f32x2 rt_rsqrt(f32x2 x) { return f32x2(rt_rsqrt(x.lo()), rt_rsqrt(x.hi())); }
+RT_DEV f32x2 rt_sqrt_fast(f32x2 x) { return x * rt_rsqrt(x); }
+RT_DEV mask2 rt_finite(f32x2 a) { return {isfinite(a.lo()), isfinite(a.hi())}; }
+RT_DEV mask2 rt_less_nonneg(f32x2 a, f32x2 b) { return {a.lo() < b.lo(), a.hi() < b.hi()}; }
+RT_DEV mask2 rt_positive(f32x2 a) { return {a.lo() > 0.0f, a.hi() > 0.0f}; }
+RT_DEV mask2 operator>=(f32x2 a, f32x2 b) { return {a.lo() >= b.lo(), a.hi() >= b.hi()}; }
+RT_DEV mask2 operator<=(f32x2 a, f32x2 b) { return {a.lo() <= b.lo(), a.hi() <= b.hi()}; }
+RT_DEV mask2 rt_and(mask2 x, mask2 y) { return {x.a && y.a, x.b && y.b}; }
+RT_DEV mask2 rt_not(mask2 x) { return {!x.a, !x.b}; }
+RT_DEV f32x2 rt_select(mask2 m, f32x2 x, f32x2 y) { return f32x2(m.a ? x.lo() : y.lo(), m.b ? x.hi() : y.hi()); }
+RT_DEV int2v rt_select(mask2 m, int2v x, int y) { return {m.a ? x.a : y, m.b ? x.b : y}; }
+RT_DEV int2v rt_floor_int(f32x2 a) { return {(int)floorf(a.lo()), (int)floorf(a.hi())}; }
+RT_DEV int2v rt_imin(int2v a, int b) { return {rt_imin(a.a, b), rt_imin(a.b, b)}; }
+RT_DEV int2v operator*(int2v a, int b) { return {a.a * b, a.b * b}; }
+RT_DEV int2v operator+(int2v a, int2v b) { return {a.a + b.a, a.b + b.b}; }
+template <class T> RT_DEV T rt_from_index(int2v i) { return f32x2((float)i.a, (float)i.b); }
+#endif
+template <class T> RT_DEV typename Lane<T>::mask rt_true() { return true; }
+#ifdef __CUDACC__
+template <> RT_DEV mask2 rt_true<f32x2>() { return {true, true}; }
+#endif
+RT_DEV bool rt_and(bool x, bool y) { return x && y; }
+RT_DEV bool rt_not(bool x) { return !x; }
+template <class T> RT_DEV T rt_select(bool m, T x, T y) { return m ? x : y; }
+RT_DEV int rt_floor_int(double a) { return (int)rt_floor(a); }
+RT_DEV int rt_floor_int(float a) { return (int)rt_floor(a); }
+template <class T> RT_DEV T rt_from_index(int i) { return T(i); }
+
 #ifdef __CUDACC__
 RT_DEV void ld16(const double* p, double& a, double& b) {
   const double2 t = __ldg(reinterpret_cast<const double2*>(p));
@@ -161,10 +236,24 @@ template <class T> RT_DEV void ld4(const T* p, T* c) { for (int i = 0; i < 4; ++
 // How the grid equilibrium fetches a cell's spline pieces.  GatherDirect reads the global tables (diagnostic kernels,
 // launch solver, host builds); the trace kernel passes a shared-memory cell cache instead (rt_kernels.cuh: GatherCached).
 struct GatherDirect {
-  template <class T> RT_DEV void psi_select(const Params<T>&, int) {}
-  template <class T> RT_DEV void prof_select(const Params<T>&, int) {}
+  template <class T, class I> RT_DEV void psi_select(const Params<T>&, I) {}
+  template <class T, class I> RT_DEV void prof_select(const Params<T>&, I) {}
   template <class T> RT_DEV void psi_row(const Params<T>& P, int cell, int p, T* c) const { ld4(P.psi_pp + (size_t)cell * 16 + 4 * p, c); }
   template <class T> RT_DEV void prof_row(const Params<T>& P, int cell, int which, T* c) const { ld4(P.prof_pp + (size_t)cell * 8 + 4 * which, c); }
+#ifdef __CUDACC__
+  // per-half look-ups of the packed type (the grid branch of equilibrium<> has to compile for every T; the packed trace
+  // kernels themselves are instantiated for the analytic equilibria only)
+  RT_DEV void psi_row(const Params<f32x2>& P, int2v cell, int p, f32x2* c) const {
+    float a[4], b[4];
+    ld4(P.psi_pp + (size_t)cell.a * 16 + 4 * p, a); ld4(P.psi_pp + (size_t)cell.b * 16 + 4 * p, b);
+    for (int j = 0; j < 4; ++j) c[j] = f32x2(a[j], b[j]);
+  }
+  RT_DEV void prof_row(const Params<f32x2>& P, int2v cell, int which, f32x2* c) const {
+    float a[4], b[4];
+    ld4(P.prof_pp + (size_t)cell.a * 8 + 4 * which, a); ld4(P.prof_pp + (size_t)cell.b * 8 + 4 * which, b);
+    for (int j = 0; j < 4; ++j) c[j] = f32x2(a[j], b[j]);
+  }
+#endif
 };
 
 // Cubic c0 + c1 s + c2 s^2 + c3 s^3 with its first derivative and HALF its second derivative in 6 fused multiply-adds
@@ -366,15 +455,16 @@ RT_DEV void axisym_field(T iR, T psiR, T psiZ, T psiRRh, T psiRZ, T psiZZh, T F,
 }
 
 template <class T, int EQ, int DISP, bool SC = false, class Gather>
-RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L, Gather& gather) {
+RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L, Gather& gather) {
+  typedef typename Lane<T>::mask M;
   if (EQ == EQ_PARABOLIC) {
     // X = xs (1 + (x^2+y^2)/L^2)                                          (BASELINE.json config 1)
     L.X = rt_fma(P.par_g, rt_fma(x[0], x[0], x[1] * x[1]), P.xs);
-    return true;                                                           // grad X = 2 par_g (x, y, 0): see ray_rhs
+    return rt_true<T>();                                                   // everywhere; grad X = 2 par_g (x, y, 0): see ray_rhs
   }
   if (EQ == EQ_LINEAR) {
     // n_e = n_ref (x_foot - x)/L_ramp ;  B = (B0 R0 / x) z^                (config 3; Eq. 4 profile)
-    const bool inside = rt_positive(x[0]);
+    const M inside = rt_positive(x[0]);
     L.X = (x[0] - P.x_foot) * P.lin_gx;                                    // grad X = (lin_gx, 0, 0)
     if (DISP != DISP_O) {
       const T ix = rt_rcp(x[0]);
@@ -405,7 +495,7 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
     const T dR = R - P.R0;
     const T r2 = rt_fma(dR, dR, Z * Z);
     // r^2 < (rho_max a)^2 implies R > 0 because rt_create_equilibrium requires a < R0 and rho_max < 1
-    const bool inside = rt_less_nonneg(r2, P.rmax2);
+    const M inside = rt_less_nonneg(r2, T(P.rmax2));
     const T t = rt_fma(-P.inv_a2, r2, T(1));                               // 1 - rho^2
     T gx;                                                                  // (1/2) grad X = gx (dR, 0, Z)
     if (EQ == EQ_TOKAMAK) {
@@ -447,12 +537,13 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
   // R > 0 is implied by R >= Rmin: rt_create_equilibrium requires Rmin > 0.  Inside the rectangle R - Rmin >= +0 exactly,
   // so the cell index is >= 0 and only needs the upper clamp (R = Rmax belongs to the last cell); outside -- including NaN
   // positions, which convert to unspecified ints -- the index is forced to 0 to keep the gather in bounds.
-  bool inside = (R >= P.Rmin) && (R <= P.Rmax) && (Z >= P.Zmin) && (Z <= P.Zmax);
-  int iRc = rt_imin((int)rt_floor((R - P.Rmin) * P.inv_hR), P.nRc - 1);
-  int iZc = rt_imin((int)rt_floor((Z - P.Zmin) * P.inv_hZ), P.nZc - 1);
-  if (!inside) { iRc = 0; iZc = 0; }
-  const T dR = R - rt_fma(T(iRc), P.hR, P.Rmin), dZ = Z - rt_fma(T(iZc), P.hZ, P.Zmin);
-  const int cell = iRc * P.nZc + iZc;
+  typedef typename Lane<T>::index I;
+  M inside = rt_and(rt_and(R >= T(P.Rmin), R <= T(P.Rmax)), rt_and(Z >= T(P.Zmin), Z <= T(P.Zmax)));
+  I iRc = rt_imin(rt_floor_int((R - P.Rmin) * P.inv_hR), P.nRc - 1);
+  I iZc = rt_imin(rt_floor_int((Z - P.Zmin) * P.inv_hZ), P.nZc - 1);
+  iRc = rt_select(inside, iRc, 0); iZc = rt_select(inside, iZc, 0);
+  const T dR = R - rt_fma(rt_from_index<T>(iRc), T(P.hR), T(P.Rmin)), dZ = Z - rt_fma(rt_from_index<T>(iZc), T(P.hZ), T(P.Zmin));
+  const I cell = iRc * P.nZc + iZc;
   gather.psi_select(P, cell);
   T a[4], a1[4], a2h[4];   // a_p(dZ) = sum_q c[p][q] dZ^q, its first dZ-derivative and half its second
 #pragma unroll
@@ -471,10 +562,10 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
     cubic01(a1, dR, psiZ, psiRZ);
     psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
   }
-  inside = inside && (psi >= P.psi_min) && (psi <= P.psi_max);
-  int iP = rt_imin((int)rt_floor((psi - P.psi_min) * P.inv_hP), P.nPc - 1);      // same argument: psi >= psi_min when inside
-  if (!inside) iP = 0;
-  const T ds = psi - rt_fma(T(iP), P.hP, P.psi_min);
+  inside = rt_and(inside, rt_and(psi >= T(P.psi_min), psi <= T(P.psi_max)));
+  I iP = rt_imin(rt_floor_int((psi - P.psi_min) * P.inv_hP), P.nPc - 1);         // same argument: psi >= psi_min when inside
+  iP = rt_select(inside, iP, 0);
+  const T ds = psi - rt_fma(rt_from_index<T>(iP), T(P.hP), T(P.psi_min));
   T g[4], Ne, Nep;
   gather.prof_select(P, iP);
   gather.prof_row(P, iP, 1, g);
@@ -491,11 +582,76 @@ RT_DEV bool equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L,
   return inside;
 }
 
+// ---- the full determinant over the analytic tokamak (config 4, the headline kernel), written out ------------------
+// Same mathematics as equilibrium<EQ_TOKAMAK, DISP_FULL, SC> + disp_coefs + the generic assembly of ray_rhs, with the
+// products shared between the field, its gradients and the assembly formed once (6 FP64 instructions fewer per stage).
+// With h = sqrt(beta) B0/(q R), g = sqrt(beta) B0 R0/R, c = q'/q, e = 1/R + c dR, m = n_Z dR - n_R Z (header of
+// equilibrium<>):  B' = (-h Z, g, h dR),  (1/2) grad Y2 = (h^2 (dR - r^2 e) - g^2/R, 0, h^2 Z (1 - c r^2)),
+// grad_x(n.B') = (h (n_Z - e m) - n_phi g/R, (n_phi B'_R - n_R g)/R, -h (n_R + c Z m)),  (1/2) grad X = gx (dR, 0, Z).  Then
+//   f_R = Ax gx dR + Ab h^2 (dR - r^2 e) + (g/R)(C n_phi - Ab g) - C h (n_Z - e m)
+//   f_Z = Z (Ax gx + Ab h^2 (1 - c r^2)) + C h (n_R + c Z m)
+//   f_phi = (n_phi (C h Z) + n_R (C g)) / R
+//   f_x = A n + C B':  C B'_R = -(C h) Z,  C B'_phi = C g,  C B'_Z = (C h) dR.
+template <class T, int EQ>
+RT_DEV typename Lane<T>::mask tokamak_full_rhs(const Params<T>& P, const T* y, T* f, T& r) {
+  const T* n = y + 3;
+  const T R2 = rt_fma(y[0], y[0], y[1] * y[1]);
+  const T iR = rt_rsqrt(R2);
+  const T R = R2 * iR;
+  const T Z = y[2];
+  const T cph = y[0] * iR, sph = y[1] * iR;
+  const T nR = rt_fma(n[0], cph, n[1] * sph);
+  const T nP = rt_fma(n[1], cph, -n[0] * sph);
+  const T nZ = n[2];
+  const T dR = R - P.R0;
+  const T r2 = rt_fma(dR, dR, Z * Z);
+  const typename Lane<T>::mask inside = rt_less_nonneg(r2, T(P.rmax2));   // implies R > 0 (a < R0, rho_max < 1)
+  const T t = rt_fma(-P.inv_a2, r2, T(1));                       // 1 - rho^2
+  T X, gx;
+  if (EQ == EQ_TOKAMAK) {
+    const T sq = rt_sqrt_fast(t);
+    X = (P.xs * sq) * t;
+    gx = P.tok_gxh * sq;
+  } else {
+    const T pw = rt_pow(t, P.p_exp - T(1));
+    X = (P.xs * pw) * t;
+    gx = P.tok_gxh * pw;
+  }
+  const T iq = rt_rcp(rt_fma(P.q1_a2, r2, P.q0));
+  const T h = (P.sB0 * iq) * iR;
+  const T g = P.sB0R0 * iR;
+  const T c = P.two_q1_a2 * iq;
+  const T e = rt_fma(c, dR, iR);
+  const T h2 = h * h;
+  const T giR = g * iR;
+  const T Y2 = rt_fma(h2, r2, g * g);
+  const T m = rt_fma(nZ, dR, -nR * Z);
+  const T G = rt_fma(h, m, g * nP);
+  const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
+  const Coef<T> k = disp_coefs<T, DISP_FULL, true>(P, X, Y2, G, v);
+  r = k.r;
+  const T Axg = k.Ax * gx, Abh2 = k.Ab * h2, Ch = k.C * h, Cg = k.C * g, ChZ = Ch * Z;
+  const T al = rt_fma(-r2, e, dR);                               // dR - r^2 e
+  const T be = rt_fma(-e, m, nZ);                                // n_Z - e m
+  const T ga = rt_fma(k.C, nP, -k.Ab * g);                       // C n_phi - Ab g
+  const T fR = rt_fma(Axg, dR, rt_fma(Abh2, al, rt_fma(giR, ga, -Ch * be)));
+  const T ze = rt_fma(-c, r2, T(1));                             // 1 - c r^2
+  const T de = rt_fma(c * Z, m, nR);                             // n_R + c Z m
+  f[5] = rt_fma(Z, rt_fma(Abh2, ze, Axg), Ch * de);
+  const T fP = rt_fma(nP, ChZ, nR * Cg) * iR;
+  f[3] = rt_fma(fR, cph, -fP * sph);
+  f[4] = rt_fma(fR, sph, fP * cph);
+  f[0] = rt_fma(-ChZ, cph, rt_fma(-Cg, sph, k.A * n[0]));
+  f[1] = rt_fma(-ChZ, sph, rt_fma(Cg, cph, k.A * n[1]));
+  f[2] = rt_fma(Ch, dR, k.A * n[2]);
+  return inside;
+}
+
 // ---- one evaluation of the ray right-hand side, y = (x, n) --------------------------------------------------------
 // Returns the right-hand side as (f, r): dy/dtau = r f, r = 1/s the reciprocal of the header comment.  Returns false
 // (and f, r unspecified) if x is outside the equilibrium's domain.
 template <class T, int EQ, int DISP, class Gather>
-RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) {
+RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) {
   Local<T> L;
   const T* n = y + 3;
   if (EQ == EQ_PARABOLIC) {
@@ -507,10 +663,11 @@ RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) 
     r = rt_rcp(rt_fma(n[0], n[0], rt_fma(n[1], n[1], rt_fma(gx, y[0], rt_fma(gy, y[1], base)))));
     f[0] = n[0]; f[1] = n[1]; f[2] = n[2];
     f[3] = -gx; f[4] = -gy; f[5] = T(0);
-    return true;
+    return rt_true<T>();
   }
+  if ((EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) && DISP == DISP_FULL) return tokamak_full_rhs<T, EQ>(P, y, f, r);
   constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
-  const bool inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
+  const typename Lane<T>::mask inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
   if (DISP == DISP_O) {
     // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)   =>   dx/dtau = n r, dn/dtau = -grad X r/2, r = 1/(v+X)
@@ -558,9 +715,9 @@ RT_DEV bool ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) 
 
 // dy/dtau itself (diagnostics: rt_rhs)
 template <class T, int EQ, int DISP, class Gather>
-RT_DEV bool ray_rhs_scaled(const Params<T>& P, const T* y, T* f, Gather& gather) {
+RT_DEV typename Lane<T>::mask ray_rhs_scaled(const Params<T>& P, const T* y, T* f, Gather& gather) {
   T r;
-  const bool inside = ray_rhs<T, EQ, DISP>(P, y, f, r, gather);
+  const typename Lane<T>::mask inside = ray_rhs<T, EQ, DISP>(P, y, f, r, gather);
 #pragma unroll
   for (int j = 0; j < 6; ++j) f[j] *= r;
   return inside;
@@ -568,7 +725,7 @@ RT_DEV bool ray_rhs_scaled(const Params<T>& P, const T* y, T* f, Gather& gather)
 
 // signed D at y = (x, n); *inside reports the domain test
 template <class T, int EQ, int DISP, class Gather>
-RT_DEV T ray_D(const Params<T>& P, const T* y, bool* inside, Gather& gather) {
+RT_DEV T ray_D(const Params<T>& P, const T* y, typename Lane<T>::mask* inside, Gather& gather) {
   Local<T> L;
   *inside = equilibrium<T, EQ, DISP>(P, y, y + 3, L, gather);
   const T v = y[3] * y[3] + y[4] * y[4] + y[5] * y[5];

@@ -16,6 +16,11 @@ Reported per kernel:
                 ray-step is 2 instr + rf3 cycles per warp and scheduler;
 * ``executed``  flops as executed, a fused multiply-add counted as 2;
 * ``mufu``      MUFU seeds (reciprocals and reciprocal square roots), ``rsqrt`` of them square roots;
+* f32, analytic equilibria: the kernels that run are ``trace_kernel_x2`` (two rays per thread, packed f32x2 arithmetic).
+                Their loop body advances two rays; the counts are reported PER RAY: a packed FFMA2 / FMUL2 / FADD2 is one
+                pipe slot per ray (it occupies the FMA pipe for two cycles and does the operation for both rays), a scalar
+                FP instruction or MUFU seed half a slot.  ``rf3`` counts packed instructions with three distinct register
+                operands: 3 pipe cycles instead of 2 (84.9 against 127.9 FMA per clock per SM, ``rt_fma_peak_shape`` shapes 6 / 5);
 * ``local``     local-memory (spill) instructions executed per ray-step: must be 0.  ptxas may still report a few bytes
                 of spill for values parked once before the step loop and reloaded after it (the store staging);
 * ``flops``     the ALGORITHMIC flops bench.py uses for ``roofline.achieved``: every division and square root counted as
@@ -37,6 +42,7 @@ from pathlib import Path
 LIB = Path(__file__).resolve().parent / "librt_b200.so"
 _INS = re.compile(r"\s+/\*([0-9a-f]+)\*/\s+(?:@!?U?P\w+\s+)?([A-Z0-9_.]+)(.*?);")
 _FP = {"d": ("DFMA", "DMUL", "DADD", "DSETP"), "f": ("FFMA", "FMUL", "FADD", "FSETP")}
+_FP2 = ("FFMA2", "FMUL2", "FADD2")       # packed f32x2: one instruction serves both rays of a thread
 
 
 def cuobjdump() -> str | None:
@@ -103,14 +109,18 @@ def count_kernels(lib: Path = LIB) -> dict:
     for fn in re.split(r"\n\s*Function : ", sass):
         m = re.match(r"_ZN2rt12trace_kernelI([df])Li(\d)ELi(\d)ELb0ELb0E", fn)      # the plain single-frequency kernels
         mo = re.match(r"_ZN2rt12orbit_kernelI([df])Li(\d)EE", fn)                   # the second workload (rt_orbit)
-        if not m and not mo:
+        m2 = re.match(r"_ZN2rt15trace_kernel_x2ILi(\d)ELi(\d)EE", fn)              # fp32, two rays per thread (packed)
+        if not m and not mo and not m2:
             continue
+        packed = bool(m2)
         if m:
             prec, eq, disp = m.group(1), int(m.group(2)), int(m.group(3))
-        else:
+        elif mo:
             prec, eq, disp = mo.group(1), int(mo.group(2)), "orbit"
+        else:
+            prec, eq, disp = "f", int(m2.group(1)), int(m2.group(2))
         ins = _parse(fn)
-        fp_ops = _FP[prec]
+        fp_ops = _FP[prec] + (_FP2 if packed else ())
         # Loop nest of the kernel = its backward branches.  The loops that hold FP-pipe instructions are nested:
         # sample loop > step loop (> stage loop, when the stages are rolled: grid equilibrium).  The small loops of the
         # store staging and of the cooperative cell-cache refill hold no FP instruction and are ignored.
@@ -138,19 +148,30 @@ def count_kernels(lib: Path = LIB) -> dict:
             rsq += 3 * rsqi
             rf3 += 3 * _rf3(ins, *chain[0], fp_ops)
         fma, mul, add, setp = _FP[prec]
+        local = tot["STL"] + tot["LDL"]                     # spill traffic executed per ray-step (must be 0)
+        if packed:
+            # the loop body advances TWO rays: a packed instruction is one pipe slot per ray; a scalar FP instruction
+            # (per-half domain tests, |x|) and a MUFU seed serve one ray each, i.e. half a slot per ray
+            n2 = tot["FFMA2"] + tot["FMUL2"] + tot["FADD2"]
+            n1 = tot[fma] + tot[mul] + tot[add] + tot[setp]
+            executed = 2 * tot["FFMA2"] + tot["FMUL2"] + tot["FADD2"] + (2 * tot[fma] + tot[mul] + tot[add] + 1) // 2
+            mufu, rsq = tot["MUFU"] // 2, rsq // 2
+            res[("f32", eq, disp)] = dict(instr=n2 + (n1 + 1) // 2, executed=executed, mufu=mufu, rsqrt=rsq,
+                                          flops=executed + mufu, local=local, rf3=rf3, packed=True)
+            continue
         executed = 2 * tot[fma] + tot[mul] + tot[add]
         mufu = tot["MUFU"]
         flops = executed - 5 * (mufu - rsq) - 7 * rsq if prec == "d" else executed + mufu
-        local = tot["STL"] + tot["LDL"]                     # spill traffic executed per ray-step (must be 0)
         res[("f64" if prec == "d" else "f32", eq, disp)] = dict(instr=tot[fma] + tot[mul] + tot[add] + tot[setp],
                                                                 executed=executed, mufu=mufu, rsqrt=rsq, flops=flops,
-                                                                local=local, rf3=rf3)
+                                                                local=local, rf3=rf3, packed=False)
     return res
 
 
 if __name__ == "__main__":
     names = {0: "parabolic", 1: "linear", 2: "tokamak", 3: "grid", 4: "tokamak_pow"}
     disps = {0: "O", 1: "X", 2: "full"}
+    print("(f32 analytic rows: trace_kernel_x2, two rays per thread, packed FFMA2 / FMUL2 / FADD2; counts are per ray)")
     print(f"{'kernel':34s} {'instr':>6s} {'rf3':>5s} {'executed':>9s} {'mufu':>5s} {'rsqrt':>6s} {'flops':>6s} {'local':>6s}")
     for (prec, eq, disp), r in sorted(count_kernels().items(), key=lambda kv: (kv[0][2] == "orbit", kv[0][0], kv[0][1], str(kv[0][2]))):
         name = f"orbit_kernel<{prec}, {names[eq]:11s}>      " if disp == "orbit" else f"trace_kernel<{prec}, {names[eq]:11s}, {disps[disp]:4s}>"

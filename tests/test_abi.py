@@ -162,7 +162,8 @@ def test_no_cpu_fallback_without_a_device(lib):
     rate = ctypes.c_double()
     assert lib.rt_fma_peak(0, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
     assert lib.rt_fma_peak_shape(0, 1, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_CUDA
-    assert lib.rt_fma_peak_shape(0, 5, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
+    assert lib.rt_fma_peak_shape(0, 5, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID     # packed: fp32 only
+    assert lib.rt_fma_peak_shape(1, 7, 2, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
     assert lib.rt_fma_peak_shape(0, 0, 9, 10.0, ctypes.byref(rate), None) == binding.RT_ERR_INVALID
     with pytest.raises(binding.RtError):
         binding.create_equilibrium(inputs.synth_grid(seed=3, nR=9, nZ=9, nPsi=9))   # grid tables live on the device
@@ -207,8 +208,11 @@ def test_flop_tables_match_the_compiled_kernels(lib):
     report = report_path.read_text()
     blocks = report.split("Compiling entry function")
     traces = [b for b in blocks if "trace_kernel" in b.split("\n")[0]]
-    assert len(traces) == 78                  # 13 (equilibrium, dispersion) pairs x 2 precisions x {one w, per-ray w,
-                                              # one w resuming from a status array (rt_trace_until's chunk kernel)}
+    # 13 (equilibrium, dispersion) pairs x 2 precisions x {one w, per-ray w, one w resuming from a status array
+    # (rt_trace_until's chunk kernel)}, where the 10 plain fp32 kernels of the analytic equilibria are the packed
+    # trace_kernel_x2 instead of trace_kernel<float, ...>
+    assert len(traces) == 78
+    assert sum("trace_kernel_x2" in b.split("\n")[0] for b in traces) == 10
     import re
     spilled = [max(int(x) for x in re.findall(r"(\d+) bytes spill stores", b)) for b in traces]
     assert max(spilled) <= 64, spilled

@@ -556,6 +556,44 @@ def test_fma_peak_shapes_order_as_documented(rt):
     assert rt.fma_peak("f64", 50.0)[0] == pytest.approx(r0, rel=0.03)
 
 
+def test_fp32_peak_is_the_packed_shape(rt):
+    """The fp32 roofline denominator counts fused multiply-adds, not instructions: rt_fma_peak('f32') is the packed f32x2
+    shape (5), which is at least as fast as scalar FFMAs (shape 0); with three distinct register operands (6) a packed
+    instruction takes 3 pipe cycles instead of 2, like a DFMA."""
+    r0, _ = rt.fma_peak_shape("f32", 0, 4, 50.0)
+    r5, _ = rt.fma_peak_shape("f32", 5, 4, 50.0)
+    r6, _ = rt.fma_peak_shape("f32", 6, 4, 50.0)
+    assert r5 >= 0.99 * r0 and 0.6 < r6 / r5 < 0.72, (r0, r5, r6)
+    assert rt.fma_peak("f32", 50.0)[0] == pytest.approx(r5, rel=0.03)
+    with pytest.raises(rt.RtError):
+        rt.fma_peak_shape("f64", 5, 4, 10.0)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 63, 64, 65, 127, 129, 1000, 1002])
+def test_packed_fp32_kernels_at_ragged_sizes(rt, oracle, n):
+    """The packed fp32 kernels trace two rays per thread: odd counts, a lone last ray, counts that are not a multiple of 4
+    (scalar store path) and of the 128 rays of a block, with guard rows around the outputs."""
+    import torch
+    w, oeq, k0 = _workload(oracle, 4, n, 60)
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, w.omega, 60, w.dt, 30, traj=True)
+    eq = rt.create_equilibrium(w.eq)
+    guard, G = 7.0, 64                       # 64 guard floats (256 bytes: the outputs stay 16-byte aligned) on either side
+    buf = torch.full((G + 3 * 6 * n + G,), guard, dtype=torch.float32, device="cuda")
+    res = torch.full((G + 3 * n + G,), guard, dtype=torch.float32, device="cuda")
+    out = {"traj": buf[G:G + 18 * n].view(3, 6, n), "residual": res[G:G + 3 * n].view(3, n)}
+    rt.trace(eq, w.disp, _dev(w.x0, "f32"), _dev(k0, "f32"), w.omega, 60, w.dt, 30, traj=True, out=out)
+    torch.cuda.synchronize()
+    assert bool((buf[:G] == guard).all()) and bool((buf[G + 18 * n:] == guard).all())
+    assert bool((res[:G] == guard).all()) and bool((res[G + 3 * n:] == guard).all())
+    tr = _host(out["traj"])
+    for m in range(3):
+        ex, ek = rel_err_xk(tr[m], ref["traj"][m])
+        assert ex < 1e-4 and ek < 1e-4, (n, m, ex, ek)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    np.testing.assert_array_equal(_host(out["final"]), tr[-1])
+    eq.close()
+
+
 def test_calls_are_enqueued_on_the_callers_stream(rt, oracle):
     """The ABI enqueues on the stream it is given and returns without synchronising (include/rt.h): two traces issued
     back to back on two side streams give the results of the same calls on the default stream, bit for bit."""

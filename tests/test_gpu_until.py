@@ -116,6 +116,14 @@ def test_degenerate_calls_and_argument_errors(rt, oracle):
     plain = rt.trace(eq, w.disp, x0d, k0d, w.omega, 40, w.dt)
     assert torch.equal(one["final"], plain["final"]) and torch.equal(one["status"], plain["status"])
     assert torch.equal(one["residual"], plain["residual"])
+    # fp32: the chunk kernel is the scalar trace_kernel<float> (resuming), the plain call the packed trace_kernel_x2 -- the same
+    # IEEE operations on each ray, so one chunk must reproduce the plain call (to rounding: the compiler may contract a
+    # multiply-add pair of the scalar code that stays two packed instructions)
+    x32, k32 = x0d.float().contiguous(), k0d.float().contiguous()
+    one32 = rt.trace_until(eq, w.disp, x32, k32, w.omega, 40, 1, w.dt)
+    plain32 = rt.trace(eq, w.disp, x32, k32, w.omega, 40, w.dt)
+    assert torch.equal(one32["status"], plain32["status"])
+    assert float(((one32["final"] - plain32["final"]).abs() / plain32["final"].abs().amax(dim=1, keepdim=True)).max()) < 2e-6
     e = torch.empty((3, 0), dtype=torch.float64, device="cuda")                          # zero rays
     z = rt.until_info(rt.trace_until(eq, w.disp, e, e.clone(), w.omega, 10, 5, w.dt)["info"])
     assert (z["chunks"], z["n_active"], z["reason"]) == (0, 0, 1)
