@@ -23,7 +23,7 @@ namespace rt {
 // does not spill (profiles/r1_tuning.md).  So the register cap (`__maxnreg__`) is simply the smallest one without spills
 // inside the step, with 64-thread blocks so that the register file divides evenly:
 //   fp64, analytic equilibria   120 registers -> 8 blocks = 16 warps per SM
-//   fp64, grid equilibrium      112 registers -> 9 blocks = 18 warps per SM (no spills inside the rolled stage loop)
+//   fp64, grid equilibrium      128 registers -> 8 blocks = 16 warps per SM (the profile pieces live in 16 of them)
 //   fp32                         72 registers -> 14 blocks = 28 warps per SM (the grid kernel's LDS latency likes warps:
 //                                321 ms at 72 registers, 344 ms at 128)
 // The grid equilibrium keeps ONE copy of the stage code (stage loop not unrolled: unrolled it needs >= 168 registers and
@@ -31,7 +31,7 @@ namespace rt {
 constexpr int AUX_BLOCK = 128;
 template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = 64, MAXNREG = 72; };
 template <int EQ> struct TraceShape<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
-template <> struct TraceShape<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 112; };
+template <> struct TraceShape<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 128; };
 
 template <class T>
 struct TraceArgs {
@@ -157,10 +157,16 @@ RT_DEV void unpack4(const float4* s, int row, int pitch, float* c) {
 template <class T, int BLOCK>
 struct GatherCached {
   typedef typename Vec16<T>::type V;
-  static constexpr int PSI_CHUNKS = 16 * sizeof(T) / 16, PROF_CHUNKS = 8 * sizeof(T) / 16;
+  // fp64: the 8 pieces of the two 1-D profiles stay in REGISTERS while the psi-cell is unchanged (about ten stages), so a
+  // stage reads only the 16 psi pieces from shared memory (8 instead of 12 LDS.128: config 5 fp64 543 -> 535 ms).  fp32:
+  // they stay in shared memory -- the fp32 kernel is issue-bound and the register copies cost more than the two LDS.128
+  // they replace (289 -> 301 ms, profiles/r2_tuning.md).
+  static constexpr bool PROF_REGS = sizeof(T) == 8;
+  static constexpr int PSI_CHUNKS = 16 * sizeof(T) / 16, PROF_CHUNKS = PROF_REGS ? 0 : 8 * sizeof(T) / 16;
   static constexpr int CHUNKS = PSI_CHUNKS + PROF_CHUNKS;
   V* col;                  // this thread's column: chunk j at col[j * BLOCK]
   int cell, pcell;         // cached cell indices (-1: nothing cached)
+  T prof[PROF_REGS ? 8 : 1];
   RT_DEV void psi_select(const Params<T>& P, int c) {
     if (c != cell) {
       const V* g = reinterpret_cast<const V*>(P.psi_pp + (size_t)c * 16);
@@ -171,14 +177,26 @@ struct GatherCached {
   }
   RT_DEV void prof_select(const Params<T>& P, int c) {
     if (c != pcell) {
-      const V* g = reinterpret_cast<const V*>(P.prof_pp + (size_t)c * 8);
+      if (PROF_REGS) {
+        ld4(P.prof_pp + (size_t)c * 8, prof);
+        ld4(P.prof_pp + (size_t)c * 8 + 4, prof + 4);
+      } else {
+        const V* g = reinterpret_cast<const V*>(P.prof_pp + (size_t)c * 8);
 #pragma unroll
-      for (int j = 0; j < PROF_CHUNKS; ++j) col[(PSI_CHUNKS + j) * BLOCK] = __ldg(g + j);
+        for (int j = 0; j < PROF_CHUNKS; ++j) col[(PSI_CHUNKS + j) * BLOCK] = __ldg(g + j);
+      }
       pcell = c;
     }
   }
   RT_DEV void psi_row(const Params<T>&, int, int p, T* c) const { unpack4(col, p, BLOCK, c); }
-  RT_DEV void prof_row(const Params<T>&, int, int which, T* c) const { unpack4(col + PSI_CHUNKS * BLOCK, which, BLOCK, c); }
+  RT_DEV void prof_row(const Params<T>&, int, int which, T* c) const {
+    if (PROF_REGS) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) c[j] = prof[4 * which + j];
+    } else {
+      unpack4(col + PSI_CHUNKS * BLOCK, which, BLOCK, c);
+    }
+  }
 };
 
 template <class T, int EQ> struct TraceGather { typedef GatherDirect type; };

@@ -275,6 +275,43 @@ RT_DEV void cubic01(const T* c, T s, T& f, T& f1) {
   f1 = rt_fma(rt_fma(c[3], s, b1), s, b0);
 }
 
+// Horner steps that share their multiplier, issued back to back.  An FP64 instruction that reads three distinct registers
+// from the register file occupies the FP64 pipe for 3 cycles instead of 2; an operand found in the
+// operand-reuse cache (the same register in the same slot of the preceding instruction) does not count.  The spline
+// evaluation is made of Horner steps x * s + y with the SAME s (the offset inside the cell) for four rows at a time:
+// written as volatile asm in row-interleaved order, ptxas keeps them adjacent with s in one slot and flags it `.reuse`,
+// so every step after the first reads two registers.  (Plain C++ leaves the order to the scheduler, which spreads them.)
+#ifdef __CUDACC__
+RT_DEV double rt_fma_s(double x, double s, double y) {
+  double d;
+  asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(x), "d"(s), "d"(y));
+  return d;
+}
+template <class T> RT_DEV T rt_fma_s(T x, T s, T y) { return rt_fma(x, s, y); }
+#else
+template <class T> RT_DEV T rt_fma_s(T x, T s, T y) { return rt_fma(x, s, y); }
+#endif
+// N cubics c[p][0..3] at the same argument s: value, first derivative and (D2) half the second derivative, level by level
+// across the N polynomials (same arithmetic as cubic012 / cubic01 on each).
+template <class T, int N, bool D2>
+RT_DEV void cubics_at(const T (*c)[4], T s, T* f, T* f1, T* f2h) {
+  T b1[N], b0[N], d1[N];
+#pragma unroll
+  for (int p = 0; p < N; ++p) b1[p] = rt_fma_s(c[p][3], s, c[p][2]);
+#pragma unroll
+  for (int p = 0; p < N; ++p) b0[p] = rt_fma_s(b1[p], s, c[p][1]);
+#pragma unroll
+  for (int p = 0; p < N; ++p) d1[p] = rt_fma_s(c[p][3], s, b1[p]);         // 2 c3 s + c2
+#pragma unroll
+  for (int p = 0; p < N; ++p) f[p] = rt_fma_s(b0[p], s, c[p][0]);
+#pragma unroll
+  for (int p = 0; p < N; ++p) f1[p] = rt_fma_s(d1[p], s, b0[p]);           // 3 c3 s^2 + 2 c2 s + c1
+  if (D2) {
+#pragma unroll
+    for (int p = 0; p < N; ++p) f2h[p] = rt_fma_s(c[p][3], s, d1[p]);      // 3 c3 s + c2
+  }
+}
+
 // ---- Stix elements (Eq. 8-10) as functions of X, Y2 ------------------------------------------
 //   S = 1 - X sig,  sig = 1/(1-Y2) + mu/(1-mu^2 Y2)
 //   Dx^2 = X^2 Y2 del^2,  del = mu^2/(1-mu^2 Y2) - 1/(1-Y2)      (eps12 = -i Dx; only Dx^2 enters D)
@@ -546,39 +583,62 @@ RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const 
   const I cell = iRc * P.nZc + iZc;
   gather.psi_select(P, cell);
   T a[4], a1[4], a2h[4];   // a_p(dZ) = sum_q c[p][q] dZ^q, its first dZ-derivative and half its second
-#pragma unroll
-  for (int p = 0; p < 4; ++p) {
-    T c[4];
-    gather.psi_row(P, cell, p, c);
-    if (DISP == DISP_O) cubic01(c, dZ, a[p], a1[p]);
-    else cubic012(c, dZ, a[p], a1[p], a2h[p]);
-  }
   T psi, psiR, psiRRh = T(0), psiZ, psiRZ = T(0), psiZZh = T(0);
-  if (DISP == DISP_O) {
-    cubic01(a, dR, psi, psiR);
-    psiZ = rt_fma(rt_fma(rt_fma(a1[3], dR, a1[2]), dR, a1[1]), dR, a1[0]);
+  if (sizeof(T) == 8 && DISP != DISP_O) {
+    // fp64: the 24 + 13 Horner steps grouped by their multiplier (dZ, then dR), see rt_fma_s
+    T c[4][4];
+#pragma unroll
+    for (int p = 0; p < 4; ++p) gather.psi_row(P, cell, p, c[p]);
+    cubics_at<T, 4, true>(c, dZ, a, a1, a2h);
+    const T b1 = rt_fma_s(a[3], dR, a[2]), e1 = rt_fma_s(a1[3], dR, a1[2]), g1 = rt_fma_s(a2h[3], dR, a2h[2]);
+    const T b0 = rt_fma_s(b1, dR, a[1]), e0 = rt_fma_s(e1, dR, a1[1]), g0 = rt_fma_s(g1, dR, a2h[1]);
+    const T d1 = rt_fma_s(a[3], dR, b1), h1 = rt_fma_s(a1[3], dR, e1);
+    psi = rt_fma_s(b0, dR, a[0]); psiZ = rt_fma_s(e0, dR, a1[0]); psiZZh = rt_fma_s(g0, dR, a2h[0]);
+    psiR = rt_fma_s(d1, dR, b0); psiRZ = rt_fma_s(h1, dR, e0);
+    psiRRh = rt_fma_s(a[3], dR, d1);
   } else {
-    cubic012(a, dR, psi, psiR, psiRRh);
-    cubic01(a1, dR, psiZ, psiRZ);
-    psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      T c[4];
+      gather.psi_row(P, cell, p, c);
+      if (DISP == DISP_O) cubic01(c, dZ, a[p], a1[p]);
+      else cubic012(c, dZ, a[p], a1[p], a2h[p]);
+    }
+    if (DISP == DISP_O) {
+      cubic01(a, dR, psi, psiR);
+      psiZ = rt_fma(rt_fma(rt_fma(a1[3], dR, a1[2]), dR, a1[1]), dR, a1[0]);
+    } else {
+      cubic012(a, dR, psi, psiR, psiRRh);
+      cubic01(a1, dR, psiZ, psiRZ);
+      psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
+    }
   }
   inside = rt_and(inside, rt_and(psi >= T(P.psi_min), psi <= T(P.psi_max)));
   I iP = rt_imin(rt_floor_int((psi - P.psi_min) * P.inv_hP), P.nPc - 1);         // same argument: psi >= psi_min when inside
   iP = rt_select(inside, iP, 0);
   const T ds = psi - rt_fma(rt_from_index<T>(iP), T(P.hP), T(P.psi_min));
-  T g[4], Ne, Nep;
+  T Ne, Nep, F = T(0), Fp = T(0);
   gather.prof_select(P, iP);
-  gather.prof_row(P, iP, 1, g);
-  cubic01(g, ds, Ne, Nep);
+  if (sizeof(T) == 8 && DISP != DISP_O) {
+    T pq[2][4], v[2], v1[2];
+    gather.prof_row(P, iP, 1, pq[0]);
+    gather.prof_row(P, iP, 0, pq[1]);
+    cubics_at<T, 2, false>(pq, ds, v, v1, v);
+    Ne = v[0]; Nep = v1[0]; F = v[1]; Fp = v1[1];
+  } else {
+    T g[4];
+    gather.prof_row(P, iP, 1, g);
+    cubic01(g, ds, Ne, Nep);
+    if (DISP != DISP_O) {
+      T f[4];
+      gather.prof_row(P, iP, 0, f);
+      cubic01(f, ds, F, Fp);
+    }
+  }
   L.X = P.xs * Ne;
   const T gx = P.xsh * Nep;
   L.hgX[0] = gx * psiR; L.hgX[2] = gx * psiZ;
-  if (DISP != DISP_O) {
-    T f[4], F, Fp;
-    gather.prof_row(P, iP, 0, f);
-    cubic01(f, ds, F, Fp);
-    axisym_field<T, DISP>(iR, psiR, psiZ, psiRRh, psiRZ, psiZZh, F, Fp, L);
-  }
+  if (DISP != DISP_O) axisym_field<T, DISP>(iR, psiR, psiZ, psiRRh, psiRZ, psiZZh, F, Fp, L);
   return inside;
 }
 
