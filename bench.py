@@ -69,8 +69,10 @@ ORBIT_COUNTS = {"f64": dict(flops=248, instr=188, rf3=44), "f32": dict(flops=248
 ORBIT_KERNEL = (2, "orbit")
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
-# DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (profiles/), or None
-NCU_DRAM_BYTES = {(4, "f64"): 5.99e9}     # profiles/r1_cfg4_f64_ncu_e.md: dram__bytes_read.sum + dram__bytes_write.sum
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed `ncu --set full`
+# captures of this build: profiles/r2_cfg4_f64_ncu_f.md (headline), profiles/r2_other_configs_ncu_f.md (the others)
+NCU_DRAM_BYTES = {(4, "f64"): 5.988e9, (2, "f64"): 6.99e7, (2, "f32"): 2.53e7, (3, "f64"): 1.26e7, (4, "f32"): 2.963e9,
+                  (5, "f64"): 1.826e9, (5, "f32"): 9.24e8, ("orbit4", "f64"): 5.98e9}
 
 WORKLOAD_NAMES = {
     1: "cfg1: O-mode, parabolic slab, 1024 rays x 1000 steps, full trajectory",
