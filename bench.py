@@ -59,7 +59,7 @@ FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 213, (4, "f
 # (instr + RF3_EXTRA * rf3) issue slots of the FMA microbenchmark; `pipe_model_frac` is that time over the measured kernel
 # time.  The fp32 kernels of the analytic equilibria (configs 1-4) are the packed two-rays-per-thread
 # kernels (trace_kernel_x2); their counts are per ray (a packed instruction = one slot per ray).
-FP_RF3_PER_RAY_STEP = {(1, "f64"): 29, (2, "f64"): 29, (3, "f64"): 42, (4, "f64"): 160, (5, "f64"): 332,
+FP_RF3_PER_RAY_STEP = {(1, "f64"): 29, (2, "f64"): 29, (3, "f64"): 42, (4, "f64"): 160, (5, "f64"): 312,
                        (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 48, (4, "f32"): 161, (5, "f32"): 260}
 RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1: 63.9 / 42.7, 123.2 / 78.8; packed 127.9 / 84.9
 PACKED = {(c, "f32") for c in (1, 2, 3, 4)}              # (config, precision) pairs that run trace_kernel_x2
