@@ -65,7 +65,7 @@ RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1
 PACKED = {(c, "f32") for c in (1, 2, 3, 4)}              # (config, precision) pairs that run trace_kernel_x2
 # The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from
 # sass_count.py's orbit_kernel rows (pinned by the same test).
-ORBIT_COUNTS = {"f64": dict(flops=248, instr=188, rf3=44), "f32": dict(flops=248, instr=166, rf3=32)}
+ORBIT_COUNTS = {"f64": dict(flops=238, instr=184, rf3=49), "f32": dict(flops=238, instr=162, rf3=43)}
 ORBIT_KERNEL = (2, "orbit")
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}

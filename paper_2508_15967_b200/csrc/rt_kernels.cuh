@@ -465,8 +465,7 @@ RT_DEV int orbit_step(const Params<T>& P, T qm, T h, T* y, Gather& gather) {
 #pragma unroll
   for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; ys[j] = y[j]; }
   bool ok = true;
-#pragma unroll 1
-  for (int st = 0; st < 4; ++st) {
+  auto stage = [&](int st) {
     const T a = (st == 0) ? T(0) : ((st == 3) ? h : hh);
     const T w = (st == 0 || st == 3) ? h6 : h3;
 #pragma unroll
@@ -474,6 +473,13 @@ RT_DEV int orbit_step(const Params<T>& P, T qm, T h, T* y, Gather& gather) {
     ok = orbit_rhs<T, EQ>(P, qm, ys, k, gather) && ok;
 #pragma unroll
     for (int j = 0; j < NA; ++j) acc[j] = rt_fma(w, k[j], acc[j]);
+  };
+  if (EQ == EQ_GRID) {               // one copy of the stage code, as in rk4_stages
+#pragma unroll 1
+    for (int st = 0; st < 4; ++st) stage(st);
+  } else {                           // analytic fields: the four stages unrolled (the compiler schedules across them)
+#pragma unroll
+    for (int st = 0; st < 4; ++st) stage(st);
   }
   if (!ok) return 1;
   bool fin = true;
