@@ -359,6 +359,15 @@ def flavour(cfg: int, prec: str) -> str:
     return "f32x2" if (cfg, prec) in PACKED else prec
 
 
+def rank_plan(scaling: str, cfg: int, n_rays: int, rank: int, world: int):
+    """What rank `rank` of `world` traces: (seed of the ensemble it draws, (begin, end) ray range of it, or None = all).
+    strong: ONE seeded ensemble, contiguous ranges; weak: every rank its own full-size batch."""
+    from paper_2508_15967_b200 import sharding
+    if scaling == "strong":
+        return 1000 + cfg, sharding.ray_range(n_rays, rank, world)
+    return sharding.rank_seed(1000 + cfg, rank), None
+
+
 def run_ours(args) -> int:
     import torch
     if not torch.cuda.is_available():
@@ -382,10 +391,8 @@ def run_ours(args) -> int:
     cfg, prec = args.config, args.precision
     n_rays = args.n_rays if args.n_rays else inputs.FULL_SIZES[cfg][0]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB of L2
-    if args.scaling == "strong":      # ONE seeded ensemble, rank r traces its contiguous range
-        job = Job(rt, torch, cfg, prec, n_rays, 1000 + cfg, ray_range=sharding.ray_range(n_rays, rank, world))
-    else:                             # every rank traces its own full-size batch
-        job = Job(rt, torch, cfg, prec, n_rays, sharding.rank_seed(1000 + cfg, rank))
+    seed, span = rank_plan(args.scaling, cfg, n_rays, rank, world)
+    job = Job(rt, torch, cfg, prec, n_rays, seed, ray_range=span)
 
     peak_before, _ = rt.fma_peak(prec, 200.0)
     sampler = ClockSampler(local)

@@ -370,16 +370,27 @@ def test_rays_leaving_the_domain_freeze_identically(rt, oracle, cfg):
     fin = _host(out["final"])
     ex, ek = rel_err_xk(fin[:, 1::2], ref["final"][:, 1::2])
     assert ex < 1e-10 and ek < 1e-10, (ex, ek)
-    # The frozen rays stopped on the same step (a one-step difference would be ~1e-3).  Their last stretch runs where
-    # n_e -> 0 (X ~ 1e-6 at rho -> 1 on the grid) and the two roots of the full determinant merge (hard
-    # part 6): the right-hand side is ill-conditioned there.  The tolerance is therefore derived from the oracle's own
-    # sensitivity: re-run it with the launch positions perturbed by 1e-15 relative and allow 50x that spread.
-    x1 = w.x0 * (1.0 + 1e-15 * np.random.default_rng(0).normal(size=w.x0.shape))
-    ref1 = oracle.trace(oeq, w.disp, x1, k0, w.omega, 300, w.dt)
-    sx, sk = rel_err_xk(ref1["final"][:, ::2], ref["final"][:, ::2])
+    # The frozen rays stopped on the same step (a one-step difference would be ~1e-3).  On the analytic tokamak they are
+    # held to the same 1e-10 as every other ray (measured 3e-15).  On the grid their last stretch runs where n_e -> 0 at
+    # psi -> psi_edge (X ~ 1e-6) and the two roots of the full determinant merge (hard part 6): the
+    # right-hand side is ill-conditioned there and the ORACLE's own result moves by up to 2e-7 under a 1e-15 perturbation
+    # of the launch positions.  The tolerance there is that measured sensitivity (largest of three perturbations) x 50,
+    # capped at 1e-5; for all but the few worst rays it is 1e-10 (asserted on the median).
     ex, ek = rel_err_xk(fin[:, ::2], ref["final"][:, ::2])
-    assert ex < max(1e-10, 50 * sx) and ek < max(1e-10, 50 * sk), (ex, ek, sx, sk)
-    assert ex < 1e-4 and ek < 1e-4
+    if cfg == 4:
+        assert ex < 1e-10 and ek < 1e-10, (ex, ek)
+    else:
+        sx = sk = 0.0
+        for seed in (0, 1, 2):
+            x1 = w.x0 * (1.0 + 1e-15 * np.random.default_rng(seed).normal(size=w.x0.shape))
+            ref1 = oracle.trace(oeq, w.disp, x1, k0, w.omega, 300, w.dt)
+            a, b = rel_err_xk(ref1["final"][:, ::2], ref["final"][:, ::2])
+            sx, sk = max(sx, a), max(sk, b)
+        assert ex < max(1e-10, 50 * sx) and ek < max(1e-10, 50 * sk), (ex, ek, sx, sk)
+        assert ex < 1e-5 and ek < 1e-5
+        d = fin[:, ::2] - ref["final"][:, ::2]
+        per_ray = np.linalg.norm(d[3:], axis=0) / np.linalg.norm(ref["final"][3:, ::2], axis=0)
+        assert np.median(per_ray) < 1e-10
     inward = np.zeros_like(ref["residual"], dtype=bool)
     inward[:, 1::2] = True            # the magnitude check against the oracle's own states: well-conditioned rays only
     _check_residual(oracle, oeq, w, _host(out["traj"]), _host(out["residual"]), ref["residual"], "f64", inward)

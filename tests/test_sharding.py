@@ -42,6 +42,12 @@ def _worker(rank, world, port, q):
         t_max = sharding.max_over_ranks(0.1 * (rank + 1), dist)
         total = sharding.sum_over_ranks(float(mine[1].sum()), dist)
         seeds = sharding.rank_seed(1004, rank)
+        import bench                                          # bench.py's own per-rank plan, both scaling modes
+        strong, weak = bench.rank_plan("strong", 4, 1001, rank, world), bench.rank_plan("weak", 4, 1001, rank, world)
+        covered = torch.tensor([strong[1][1] - strong[1][0]], dtype=torch.int64)
+        dist.all_reduce(covered)
+        assert int(covered.item()) == 1001 and strong[0] == 1004 and strong[1] == (b, e)
+        assert weak == (seeds, None)
         dist.barrier()
         q.put((rank, int(counts.item()), t_max, total, seeds, float(w.x0[1].sum())))
     finally:
