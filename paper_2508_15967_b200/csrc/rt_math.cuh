@@ -491,6 +491,89 @@ RT_DEV void axisym_field(T iR, T psiR, T psiZ, T psiRRh, T psiRZ, T psiZZh, T F,
   }
 }
 
+// ---- grid equilibrium: the spline look-ups at one point (config 5) -------------------------------------
+// psi(R, Z) bicubic with its first and second derivatives, then F(psi), n_e(psi) cubic with their first derivatives
+// (n_e in units of Params::xs / alpha, i.e. X = xs Ne).  psiRRh / psiZZh are HALF the second derivatives.
+template <class T>
+struct GridVals { T psiR, psiZ, psiRRh, psiRZ, psiZZh, F, Fp, Ne, Nep; };
+
+template <class T, int DISP, class Gather>
+RT_DEV typename Lane<T>::mask grid_splines(const Params<T>& P, T R, T Z, Gather& gather, GridVals<T>& V) {
+  typedef typename Lane<T>::mask M;
+  // R > 0 is implied by R >= Rmin: rt_create_equilibrium requires Rmin > 0.  Inside the rectangle R - Rmin >= +0 exactly,
+  // so the cell index is >= 0 and only needs the upper clamp (R = Rmax belongs to the last cell); outside -- including NaN
+  // positions, which convert to unspecified ints -- the index is forced to 0 to keep the gather in bounds.
+  typedef typename Lane<T>::index I;
+  M inside = rt_and(rt_and(R >= T(P.Rmin), R <= T(P.Rmax)), rt_and(Z >= T(P.Zmin), Z <= T(P.Zmax)));
+  const T Ro = R - P.Rmin, Zo = Z - P.Zmin;                       // offsets from the grid's corner
+  I iRc = rt_imin(rt_floor_int(Ro * P.inv_hR), P.nRc - 1);
+  I iZc = rt_imin(rt_floor_int(Zo * P.inv_hZ), P.nZc - 1);
+  iRc = rt_select(inside, iRc, 0); iZc = rt_select(inside, iZc, 0);
+  // offset inside the cell: (R - Rmin) - i hR in one fused step (i hR is exact in the fma; the oracle's R - (Rmin + i hR)
+  // differs by a rounding of R)
+  const T dR = rt_fma(-rt_from_index<T>(iRc), T(P.hR), Ro), dZ = rt_fma(-rt_from_index<T>(iZc), T(P.hZ), Zo);
+  const I cell = iRc * P.nZc + iZc;
+  gather.psi_select(P, cell);
+  T a[4], a1[4], a2h[4];   // a_p(dZ) = sum_q c[p][q] dZ^q, its first dZ-derivative and half its second
+  T psi, psiR, psiRRh = T(0), psiZ, psiRZ = T(0), psiZZh = T(0);
+  if (sizeof(T) == 8 && DISP != DISP_O) {
+    // fp64: the 24 + 13 Horner steps grouped by their multiplier (dZ, then dR), see rt_fma_s
+    T c[4][4];
+#pragma unroll
+    for (int p = 0; p < 4; ++p) gather.psi_row(P, cell, p, c[p]);
+    cubics_at<T, 4, true>(c, dZ, a, a1, a2h);
+    const T b1 = rt_fma_s(a[3], dR, a[2]), e1 = rt_fma_s(a1[3], dR, a1[2]), g1 = rt_fma_s(a2h[3], dR, a2h[2]);
+    const T b0 = rt_fma_s(b1, dR, a[1]), e0 = rt_fma_s(e1, dR, a1[1]), g0 = rt_fma_s(g1, dR, a2h[1]);
+    const T d1 = rt_fma_s(a[3], dR, b1), h1 = rt_fma_s(a1[3], dR, e1);
+    psi = rt_fma_s(b0, dR, a[0]); psiZ = rt_fma_s(e0, dR, a1[0]); psiZZh = rt_fma_s(g0, dR, a2h[0]);
+    psiR = rt_fma_s(d1, dR, b0); psiRZ = rt_fma_s(h1, dR, e0);
+    psiRRh = rt_fma_s(a[3], dR, d1);
+  } else {
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      T c[4];
+      gather.psi_row(P, cell, p, c);
+      if (DISP == DISP_O) cubic01(c, dZ, a[p], a1[p]);
+      else cubic012(c, dZ, a[p], a1[p], a2h[p]);
+    }
+    if (DISP == DISP_O) {
+      cubic01(a, dR, psi, psiR);
+      psiZ = rt_fma(rt_fma(rt_fma(a1[3], dR, a1[2]), dR, a1[1]), dR, a1[0]);
+    } else {
+      cubic012(a, dR, psi, psiR, psiRRh);
+      cubic01(a1, dR, psiZ, psiRZ);
+      psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
+    }
+  }
+  inside = rt_and(inside, rt_and(psi >= T(P.psi_min), psi <= T(P.psi_max)));
+  const T po = psi - P.psi_min;
+  I iP = rt_imin(rt_floor_int(po * P.inv_hP), P.nPc - 1);                        // same argument: psi >= psi_min when inside
+  iP = rt_select(inside, iP, 0);
+  const T ds = rt_fma(-rt_from_index<T>(iP), T(P.hP), po);
+  T Ne, Nep, F = T(0), Fp = T(0);
+  gather.prof_select(P, iP);
+  if (sizeof(T) == 8 && DISP != DISP_O) {
+    T pq[2][4], v[2], v1[2];
+    gather.prof_row(P, iP, 1, pq[0]);
+    gather.prof_row(P, iP, 0, pq[1]);
+    cubics_at<T, 2, false>(pq, ds, v, v1, v);
+    Ne = v[0]; Nep = v1[0]; F = v[1]; Fp = v1[1];
+  } else {
+    T g[4];
+    gather.prof_row(P, iP, 1, g);
+    cubic01(g, ds, Ne, Nep);
+    if (DISP != DISP_O) {
+      T f[4];
+      gather.prof_row(P, iP, 0, f);
+      cubic01(f, ds, F, Fp);
+    }
+  }
+  V.psiR = psiR; V.psiZ = psiZ; V.psiRRh = psiRRh; V.psiRZ = psiRZ; V.psiZZh = psiZZh;
+  V.F = F; V.Fp = Fp; V.Ne = Ne; V.Nep = Nep;
+  return inside;
+}
+
+
 template <class T, int EQ, int DISP, bool SC = false, class Gather>
 RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L, Gather& gather) {
   typedef typename Lane<T>::mask M;
@@ -571,74 +654,12 @@ RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const 
     return inside;
   }
   // EQ_GRID: bicubic psi(R,Z), cubic F(psi), n_e(psi)                                    (config 5)
-  // R > 0 is implied by R >= Rmin: rt_create_equilibrium requires Rmin > 0.  Inside the rectangle R - Rmin >= +0 exactly,
-  // so the cell index is >= 0 and only needs the upper clamp (R = Rmax belongs to the last cell); outside -- including NaN
-  // positions, which convert to unspecified ints -- the index is forced to 0 to keep the gather in bounds.
-  typedef typename Lane<T>::index I;
-  M inside = rt_and(rt_and(R >= T(P.Rmin), R <= T(P.Rmax)), rt_and(Z >= T(P.Zmin), Z <= T(P.Zmax)));
-  I iRc = rt_imin(rt_floor_int((R - P.Rmin) * P.inv_hR), P.nRc - 1);
-  I iZc = rt_imin(rt_floor_int((Z - P.Zmin) * P.inv_hZ), P.nZc - 1);
-  iRc = rt_select(inside, iRc, 0); iZc = rt_select(inside, iZc, 0);
-  const T dR = R - rt_fma(rt_from_index<T>(iRc), T(P.hR), T(P.Rmin)), dZ = Z - rt_fma(rt_from_index<T>(iZc), T(P.hZ), T(P.Zmin));
-  const I cell = iRc * P.nZc + iZc;
-  gather.psi_select(P, cell);
-  T a[4], a1[4], a2h[4];   // a_p(dZ) = sum_q c[p][q] dZ^q, its first dZ-derivative and half its second
-  T psi, psiR, psiRRh = T(0), psiZ, psiRZ = T(0), psiZZh = T(0);
-  if (sizeof(T) == 8 && DISP != DISP_O) {
-    // fp64: the 24 + 13 Horner steps grouped by their multiplier (dZ, then dR), see rt_fma_s
-    T c[4][4];
-#pragma unroll
-    for (int p = 0; p < 4; ++p) gather.psi_row(P, cell, p, c[p]);
-    cubics_at<T, 4, true>(c, dZ, a, a1, a2h);
-    const T b1 = rt_fma_s(a[3], dR, a[2]), e1 = rt_fma_s(a1[3], dR, a1[2]), g1 = rt_fma_s(a2h[3], dR, a2h[2]);
-    const T b0 = rt_fma_s(b1, dR, a[1]), e0 = rt_fma_s(e1, dR, a1[1]), g0 = rt_fma_s(g1, dR, a2h[1]);
-    const T d1 = rt_fma_s(a[3], dR, b1), h1 = rt_fma_s(a1[3], dR, e1);
-    psi = rt_fma_s(b0, dR, a[0]); psiZ = rt_fma_s(e0, dR, a1[0]); psiZZh = rt_fma_s(g0, dR, a2h[0]);
-    psiR = rt_fma_s(d1, dR, b0); psiRZ = rt_fma_s(h1, dR, e0);
-    psiRRh = rt_fma_s(a[3], dR, d1);
-  } else {
-#pragma unroll
-    for (int p = 0; p < 4; ++p) {
-      T c[4];
-      gather.psi_row(P, cell, p, c);
-      if (DISP == DISP_O) cubic01(c, dZ, a[p], a1[p]);
-      else cubic012(c, dZ, a[p], a1[p], a2h[p]);
-    }
-    if (DISP == DISP_O) {
-      cubic01(a, dR, psi, psiR);
-      psiZ = rt_fma(rt_fma(rt_fma(a1[3], dR, a1[2]), dR, a1[1]), dR, a1[0]);
-    } else {
-      cubic012(a, dR, psi, psiR, psiRRh);
-      cubic01(a1, dR, psiZ, psiRZ);
-      psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
-    }
-  }
-  inside = rt_and(inside, rt_and(psi >= T(P.psi_min), psi <= T(P.psi_max)));
-  I iP = rt_imin(rt_floor_int((psi - P.psi_min) * P.inv_hP), P.nPc - 1);         // same argument: psi >= psi_min when inside
-  iP = rt_select(inside, iP, 0);
-  const T ds = psi - rt_fma(rt_from_index<T>(iP), T(P.hP), T(P.psi_min));
-  T Ne, Nep, F = T(0), Fp = T(0);
-  gather.prof_select(P, iP);
-  if (sizeof(T) == 8 && DISP != DISP_O) {
-    T pq[2][4], v[2], v1[2];
-    gather.prof_row(P, iP, 1, pq[0]);
-    gather.prof_row(P, iP, 0, pq[1]);
-    cubics_at<T, 2, false>(pq, ds, v, v1, v);
-    Ne = v[0]; Nep = v1[0]; F = v[1]; Fp = v1[1];
-  } else {
-    T g[4];
-    gather.prof_row(P, iP, 1, g);
-    cubic01(g, ds, Ne, Nep);
-    if (DISP != DISP_O) {
-      T f[4];
-      gather.prof_row(P, iP, 0, f);
-      cubic01(f, ds, F, Fp);
-    }
-  }
-  L.X = P.xs * Ne;
-  const T gx = P.xsh * Nep;
-  L.hgX[0] = gx * psiR; L.hgX[2] = gx * psiZ;
-  if (DISP != DISP_O) axisym_field<T, DISP>(iR, psiR, psiZ, psiRRh, psiRZ, psiZZh, F, Fp, L);
+  GridVals<T> V;
+  const M inside = grid_splines<T, DISP>(P, R, Z, gather, V);
+  L.X = P.xs * V.Ne;
+  const T gx = P.xsh * V.Nep;
+  L.hgX[0] = gx * V.psiR; L.hgX[2] = gx * V.psiZ;
+  if (DISP != DISP_O) axisym_field<T, DISP>(iR, V.psiR, V.psiZ, V.psiRRh, V.psiRZ, V.psiZZh, V.F, V.Fp, L);
   return inside;
 }
 
@@ -707,6 +728,55 @@ RT_DEV typename Lane<T>::mask tokamak_full_rhs(const Params<T>& P, const T* y, T
   return inside;
 }
 
+// ---- the full determinant over the grid equilibrium (config 5), assembly written out ------------------------------------
+// Same mathematics as equilibrium<EQ_GRID, DISP_FULL> + axisym_field + disp_coefs + the generic assembly of ray_rhs; the
+// products C/R, Ab/R^2 and Ax gx that the field, its gradients and the assembly share are formed once (5 FP instructions
+// per stage fewer).  With Q = psi_R^2 + psi_Z^2 + F^2 = R^2 |B|^2, g = n_Z psi_R + n_phi F - n_R psi_Z = R (n.B),
+// hQ_R = F F' psi_R + psi_R psi_RR + psi_Z psi_RZ = (1/2) dQ/dR (hQ_Z likewise), g_R, g_Z the derivatives of g at fixed n:
+//   f_R = Ax gx psi_R + (Ab/R^2) hQ_R - (Ab |B|^2 + C (g_R - n.B))/R ,   f_Z = Ax gx psi_Z + (Ab/R^2) hQ_Z - (C/R) g_Z ,
+//   f_phi = (C/R) (n_phi psi_Z + n_R F)/R ,   C B = (C/R)(-psi_Z, F, psi_R).
+template <class T, class Gather>
+RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) {
+  const T* n = y + 3;
+  const T R2 = rt_fma(y[0], y[0], y[1] * y[1]);
+  const T iR = rt_rsqrt(R2);
+  const T R = R2 * iR;
+  const T cph = y[0] * iR, sph = y[1] * iR;
+  const T nR = rt_fma(n[0], cph, n[1] * sph);
+  const T nP = rt_fma(n[1], cph, -n[0] * sph);
+  const T nZ = n[2];
+  GridVals<T> V;
+  const typename Lane<T>::mask inside = grid_splines<T, DISP_FULL>(P, R, y[2], gather, V);
+  const T X = P.xs * V.Ne, gx = P.xsh * V.Nep;
+  const T iR2 = iR * iR;
+  const T Q = rt_fma(V.F, V.F, rt_fma(V.psiR, V.psiR, V.psiZ * V.psiZ));
+  const T b2 = Q * iR2;
+  const T psiRR = V.psiRRh + V.psiRRh, psiZZ = V.psiZZh + V.psiZZh;
+  const T FFp = V.F * V.Fp;
+  const T hQR = rt_fma(FFp, V.psiR, rt_fma(V.psiR, psiRR, V.psiZ * V.psiRZ));
+  const T hQZ = rt_fma(FFp, V.psiZ, rt_fma(V.psiR, V.psiRZ, V.psiZ * psiZZ));
+  const T g = rt_fma(nZ, V.psiR, rt_fma(nP, V.F, -nR * V.psiZ));
+  const T G = g * iR;
+  const T nPFp = nP * V.Fp;
+  const T gR = rt_fma(nZ, psiRR, rt_fma(nPFp, V.psiR, -nR * V.psiRZ));
+  const T gZ = rt_fma(nZ, V.psiRZ, rt_fma(nPFp, V.psiZ, -nR * psiZZ));
+  const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
+  const Coef<T> k = disp_coefs<T, DISP_FULL, false>(P, X, b2, G, v);
+  r = k.r;
+  const T Ci = k.C * iR, Ai2 = k.Ab * iR2, Axg = k.Ax * gx;
+  const T t2 = rt_fma(k.C, gR - G, k.Ab * b2);
+  const T fR = rt_fma(Axg, V.psiR, rt_fma(Ai2, hQR, -iR * t2));
+  f[5] = rt_fma(Axg, V.psiZ, rt_fma(Ai2, hQZ, -Ci * gZ));
+  const T fP = (Ci * iR) * rt_fma(nP, V.psiZ, nR * V.F);
+  f[3] = rt_fma(fR, cph, -fP * sph);
+  f[4] = rt_fma(fR, sph, fP * cph);
+  const T xR = -Ci * V.psiZ, xP = Ci * V.F;
+  f[0] = rt_fma(xR, cph, rt_fma(-xP, sph, k.A * n[0]));
+  f[1] = rt_fma(xR, sph, rt_fma(xP, cph, k.A * n[1]));
+  f[2] = rt_fma(Ci, V.psiR, k.A * n[2]);
+  return inside;
+}
+
 // ---- one evaluation of the ray right-hand side, y = (x, n) --------------------------------------------------------
 // Returns the right-hand side as (f, r): dy/dtau = r f, r = 1/s the reciprocal of the header comment.  Returns false
 // (and f, r unspecified) if x is outside the equilibrium's domain.
@@ -726,6 +796,7 @@ RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r
     return rt_true<T>();
   }
   if ((EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) && DISP == DISP_FULL) return tokamak_full_rhs<T, EQ>(P, y, f, r);
+  if (EQ == EQ_GRID && DISP == DISP_FULL) return grid_full_rhs<T>(P, y, f, r, gather);
   constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
   const typename Lane<T>::mask inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
