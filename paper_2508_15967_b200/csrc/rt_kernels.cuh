@@ -13,6 +13,8 @@
 
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "rt_math.cuh"
 
 namespace rt {
@@ -66,8 +68,11 @@ RT_DEV constexpr bool rhs_component_active(int j) {
 
 // rk4_stages: the four stages of one step from y; writes the candidate new state to ys and returns whether every stage
 // point was inside the domain (per lane for the packed fp32 kernels).  rk4_step applies the acceptance rule (A12).
-template <class T, int EQ, int DISP, class Gather>
-RT_DEV typename Lane<T>::mask rk4_stages(const Params<T>& P, T h, T hh, T h3, T h6, const T* y, T* ys, Gather& gather) {
+// SERIES: the ion terms by their series (rt_math.cuh: disp_coefs); `fast` is cleared if a stage point lies outside the
+// series' range (Y2 >= Params::y2cap), and the step then has to be repeated with SERIES = false.
+template <class T, int EQ, int DISP, bool SERIES, class Gather>
+RT_DEV typename Lane<T>::mask rk4_stages(const Params<T>& P, T h, T hh, T h3, T h6, const T* y, T* ys, Gather& gather,
+                                         typename Lane<T>::mask& fast) {
   T k[6], acc[6], r;                 // the slope of a stage is r k (ray_rhs): r is folded into the step-size factors
   typename Lane<T>::mask ok = rt_true<T>();
   if (EQ == EQ_GRID) {
@@ -78,7 +83,7 @@ RT_DEV typename Lane<T>::mask rk4_stages(const Params<T>& P, T h, T hh, T h3, T 
     for (int st = 0; st < 4; ++st) {
 #pragma unroll
       for (int j = 0; j < 6; ++j) ys[j] = rt_fma(ar, k[j], y[j]);
-      ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
+      ok = rt_and(ray_rhs<T, EQ, DISP, SERIES>(P, ys, k, r, gather, fast), ok);
       const T wr = ((st == 0 || st == 3) ? h6 : h3) * r;
       ar = ((st == 2) ? h : hh) * r;
 #pragma unroll
@@ -89,22 +94,22 @@ RT_DEV typename Lane<T>::mask rk4_stages(const Params<T>& P, T h, T hh, T h3, T 
   } else {
 #pragma unroll
     for (int j = 0; j < 6; ++j) { ys[j] = y[j]; acc[j] = y[j]; }
-    ok = ray_rhs<T, EQ, DISP>(P, y, k, r, gather);
+    ok = ray_rhs<T, EQ, DISP, SERIES>(P, y, k, r, gather, fast);
     T wr = h6 * r, ar = hh * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
       if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], y[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
-    ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
+    ok = rt_and(ray_rhs<T, EQ, DISP, SERIES>(P, ys, k, r, gather, fast), ok);
     wr = h3 * r; ar = hh * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
       if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], acc[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
-    ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
+    ok = rt_and(ray_rhs<T, EQ, DISP, SERIES>(P, ys, k, r, gather, fast), ok);
     wr = h3 * r; ar = h * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j)
       if (rhs_component_active<EQ>(j)) { acc[j] = rt_fma(wr, k[j], acc[j]); ys[j] = rt_fma(ar, k[j], y[j]); }
-    ok = rt_and(ray_rhs<T, EQ, DISP>(P, ys, k, r, gather), ok);
+    ok = rt_and(ray_rhs<T, EQ, DISP, SERIES>(P, ys, k, r, gather, fast), ok);
     wr = h6 * r;
 #pragma unroll
     for (int j = 0; j < 6; ++j) ys[j] = rhs_component_active<EQ>(j) ? rt_fma(wr, k[j], acc[j]) : y[j];
@@ -112,10 +117,14 @@ RT_DEV typename Lane<T>::mask rk4_stages(const Params<T>& P, T h, T hh, T h3, T 
   return ok;
 }
 
-template <class T, int EQ, int DISP, class Gather>
+// One step with the acceptance rule.  SERIES: returns -1, with y untouched, if a stage point lay outside the range of the ion
+// terms' series; the caller then repeats this step (and finishes its stretch of steps) with SERIES = false.
+template <class T, int EQ, int DISP, bool SERIES, class Gather>
 RT_DEV int rk4_step(const Params<T>& P, T h, T hh, T h3, T h6, T* y, Gather& gather) {
   T ys[6];
-  const bool ok = rk4_stages<T, EQ, DISP>(P, h, hh, h3, h6, y, ys, gather);
+  bool fast = true;
+  const bool ok = rk4_stages<T, EQ, DISP, SERIES>(P, h, hh, h3, h6, y, ys, gather, fast);
+  if (SERIES && DISP != DISP_O && !fast) return -1;
   if (!ok) return 1;
   bool fin = true;
 #pragma unroll
@@ -328,9 +337,19 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
   const long long n_outer = A.traj ? A.n_steps / A.stride : 1, n_inner = A.traj ? A.stride : A.n_steps;
   if (A.traj) save(A.traj, A.res);
   for (long long m = 1; m <= n_outer; ++m) {
+    long long s = 0;
 #pragma unroll 1
-    for (long long s = 0; s < n_inner; ++s)
-      if (status == 0) status = rk4_step<T, EQ, DISP>(P, A.h, A.hh, A.h3, A.h6, y, gather);
+    for (; s < n_inner; ++s)                        // the hot loop: ion terms by their series
+      if (status == 0) {
+        const int st = rk4_step<T, EQ, DISP, true>(P, A.h, A.hh, A.h3, A.h6, y, gather);
+        if (st < 0) break;                         // a stage point outside the series' range (Y2 >= Params::y2cap)
+        status = st;
+      }
+    if (DISP != DISP_O) {
+#pragma unroll 1
+      for (; s < n_inner; ++s)                      // the rest of this stretch exactly (rare: nothing in BASELINE's configs)
+        if (status == 0) status = rk4_step<T, EQ, DISP, false>(P, A.h, A.hh, A.h3, A.h6, y, gather);
+    }
     if (A.traj) save(A.traj + m * 6 * A.n_rays, A.res ? A.res + m * A.n_rays : nullptr);
   }
   if (A.fin || (!A.traj && A.res)) save(A.fin, A.traj ? nullptr : A.res);
@@ -407,15 +426,18 @@ trace_kernel_x2(const __grid_constant__ Params<float> P0, const __grid_constant_
   const long long n_outer = A.traj ? A.n_steps / A.stride : 1, n_inner = A.traj ? A.stride : A.n_steps;
   if (A.traj) save(A.traj, A.res);
   for (long long m = 1; m <= n_outer; ++m) {
-#pragma unroll 1
-    for (long long s = 0; s < n_inner; ++s) {
-      if (sa != 0 && sb != 0) break;               // both rays frozen (or padding): nothing left to do in this stretch
+    // one step of both rays with the acceptance rule (reading A12) per ray: a stage point outside the domain -> status 1,
+    // a non-finite new state -> 2.  SERIES: returns false, with nothing changed, if a stage point of either ray lay outside
+    // the range of the ion terms' series.
+    auto step = [&](auto series) -> bool {
+      constexpr bool SERIES = decltype(series)::value;
       T ys[6];
-      const mask2 ok = rk4_stages<T, EQ, DISP>(P, T(A.h), T(A.hh), T(A.h3), T(A.h6), y, ys, gather);
+      mask2 fast = {true, true};
+      const mask2 ok = rk4_stages<T, EQ, DISP, SERIES>(P, T(A.h), T(A.hh), T(A.h3), T(A.h6), y, ys, gather, fast);
+      if (SERIES && DISP != DISP_O && !rt_all(fast)) return false;
       mask2 fin = {true, true};
 #pragma unroll
       for (int j = 0; j < 6; ++j) fin = rt_and(fin, rt_finite(ys[j]));
-      // acceptance rule (reading A12), per ray: a stage point outside the domain -> status 1; a non-finite new state -> 2
       const mask2 acc = {sa == 0 && ok.a && fin.a, sb == 0 && ok.b && fin.b};
       if (acc.a && acc.b) {                        // the common case: both rays advance, no per-half selects
 #pragma unroll
@@ -425,6 +447,20 @@ trace_kernel_x2(const __grid_constant__ Params<float> P0, const __grid_constant_
         if (sb == 0 && !acc.b) sb = ok.b ? 2 : 1;
 #pragma unroll
         for (int j = 0; j < 6; ++j) y[j] = rt_select(acc, ys[j], y[j]);
+      }
+      return true;
+    };
+    long long s = 0;
+#pragma unroll 1
+    for (; s < n_inner; ++s) {                     // the hot loop: ion terms by their series
+      if (sa != 0 && sb != 0) break;               // both rays frozen (or padding): nothing left to do in this stretch
+      if (!step(std::true_type())) break;
+    }
+    if (DISP != DISP_O) {
+#pragma unroll 1
+      for (; s < n_inner; ++s) {                   // the rest of this stretch exactly (rare)
+        if (sa != 0 && sb != 0) break;
+        step(std::false_type());
       }
     }
     if (A.traj) save(A.traj + m * 6 * A.n_rays, A.res ? A.res + m * A.n_rays : nullptr);

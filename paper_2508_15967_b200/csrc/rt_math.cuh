@@ -48,6 +48,7 @@ struct Params {
   T beta2;      // 2 beta
   T mu;         // Z m_e / m_i; 0 = electrons only
   T mu2, mu3, mu4, one_plus_mu;
+  T y2cap;      // the ion terms' series (disp_coefs, SERIES) is exact to rounding for Y2 < y2cap (rt_params.h: series_cap)
   T k2n, n2k;   // c/w and w/c
   // slab_parabolic:  X = xs + par_g (x^2 + y^2)
   T par_g;      // xs / L^2
@@ -109,7 +110,7 @@ RT_DEV double rt_rsqrt(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   const double e = fma(-x * y, y, 1.0);      // e = 1 - x y^2
-  return fma(y * e, fma(0.375, e, 0.5), y);  // y (1 + e/2 + 3 e^2/8)
+  return y * fma(e, fma(0.375, e, 0.5), 1.0);  // y (1 + e/2 + 3 e^2/8)
 }
 RT_DEV float rt_rcp(float x) {
   float r;
@@ -128,7 +129,7 @@ RT_DEV double rt_sqrt_fast(double x) {
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   const double g = x * y;
   const double e = fma(-g, y, 1.0);
-  return fma(g * e, fma(0.375, e, 0.5), g);
+  return g * fma(e, fma(0.375, e, 0.5), 1.0);
 }
 RT_DEV float rt_sqrt_fast(float x) { return x * rt_rsqrt(x); }
 // Domain tests of the fp64 hot loop as INTEGER comparisons of the bit patterns (a DSETP occupies the FP64 pipe, which is
@@ -200,6 +201,7 @@ RT_DEV mask2 operator>=(f32x2 a, f32x2 b) { return {a.lo() >= b.lo(), a.hi() >= 
 RT_DEV mask2 operator<=(f32x2 a, f32x2 b) { return {a.lo() <= b.lo(), a.hi() <= b.hi()}; }
 RT_DEV mask2 rt_and(mask2 x, mask2 y) { return {x.a && y.a, x.b && y.b}; }
 RT_DEV mask2 rt_not(mask2 x) { return {!x.a, !x.b}; }
+RT_DEV bool rt_all(mask2 x) { return x.a && x.b; }
 RT_DEV f32x2 rt_select(mask2 m, f32x2 x, f32x2 y) { return f32x2(m.a ? x.lo() : y.lo(), m.b ? x.hi() : y.hi()); }
 RT_DEV int2v rt_select(mask2 m, int2v x, int y) { return {m.a ? x.a : y, m.b ? x.b : y}; }
 RT_DEV int2v rt_floor_int(f32x2 a) { return {(int)floorf(a.lo()), (int)floorf(a.hi())}; }
@@ -213,6 +215,7 @@ template <class T> RT_DEV typename Lane<T>::mask rt_true() { return true; }
 template <> RT_DEV mask2 rt_true<f32x2>() { return {true, true}; }
 #endif
 RT_DEV bool rt_and(bool x, bool y) { return x && y; }
+RT_DEV bool rt_all(bool x) { return x; }
 RT_DEV bool rt_not(bool x) { return !x; }
 template <class T> RT_DEV T rt_select(bool m, T x, T y) { return m ? x : y; }
 RT_DEV int rt_floor_int(double a) { return (int)rt_floor(a); }
@@ -388,27 +391,48 @@ RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2
 // The coefficients are returned WITHOUT the common factor r = 1/s (Coef::r): rk4_step folds r into the step-size
 // factors (two multiplications per stage instead of one per coefficient), ray_rhs_scaled applies it for the diagnostics.
 template <class T>
-struct Coef { T A, C, Ax, Ab, r; };
+struct Coef {
+  T A, C, Ax, Ab, r;
+  T YD;                              // Y2 DYn (full determinant only)
+  typename Lane<T>::mask fast;       // SERIES: Y2 < Params::y2cap, i.e. the series of the ion terms is exact to rounding here
+};
 
 // SC: the caller's field is already in units of sqrt(beta) (Params::sB0), i.e. b2 IS Y2 and Ab multiplies (1/2) grad Y2.
 // Ax multiplies HALF the gradient of X (Local::hgX), which is where the 1/2 of the header comment has gone.
-template <class T, int DISP, bool SC>
+template <class T, int DISP, bool SC, bool SERIES>
 RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
   const T Y2 = SC ? b2 : P.beta * b2, Y22 = SC ? b2 + b2 : P.beta2 * b2;
   const T e1 = rt_rcp(T(1) - Y2);
-  const T e2 = rt_rcp(rt_fma(-P.mu2, Y2, T(1)));
-  const T e1s = e1 * e1, e2s = e2 * e2;
-  const T sig = rt_fma(P.mu, e2, e1);
-  const T sigp = rt_fma(P.mu3, e2s, e1s);
-  const T del = rt_fma(P.mu2, e2, -e1);
-  const T delp = rt_fma(P.mu4, e2s, -e1s);
+  const T e1s = e1 * e1;
+  T sig, sigp, del, delp;
+  Coef<T> c;
+  if (SERIES) {
+    // Ion terms by their series in z = mu^2 Y2 (mu = Z m_e/m_i <= 5.4e-4): e2 = 1/(1 - z) = 1 + z + z^2 + ..., so
+    //   mu e2 = mu + mu^3 Y2 + O(mu z^2),  mu^3 e2^2 = mu^3 + O(mu^3 z),  mu^2 e2 = mu^2 + mu^4 Y2 + O(mu^2 z^2),
+    //   mu^4 e2^2 = mu^4 + O(mu^4 z);
+    // for Y2 < y2cap (folded on the host so that every dropped term is below a quarter ulp of the sum it enters) this is
+    // the rounded exact value: one reciprocal and three FP instructions per stage fewer.  A stage with Y2 >= y2cap clears
+    // c.fast and the caller repeats the step with SERIES = false.
+    c.fast = rt_less_nonneg(Y2, T(P.y2cap));
+    sig = e1 + rt_fma(P.mu3, Y2, P.mu);
+    sigp = e1s + P.mu3;
+    del = rt_fma(P.mu4, Y2, P.mu2) - e1;
+    delp = P.mu4 - e1s;
+  } else {
+    c.fast = rt_true<T>();
+    const T e2 = rt_rcp(rt_fma(-P.mu2, Y2, T(1)));
+    const T e2s = e2 * e2;
+    sig = rt_fma(P.mu, e2, e1);
+    sigp = rt_fma(P.mu3, e2s, e1s);
+    del = rt_fma(P.mu2, e2, -e1);
+    delp = rt_fma(P.mu4, e2s, -e1s);
+  }
   const T S = rt_fma(-X, sig, T(1));
   const T Xd = X * del;
   const T XdY22 = Xd * Y22;                          // 2 X Y2 del
   const T q1 = XdY22 * del;
   const T q2 = (Xd * X) * rt_fma(Y22, delp, del);
   const T Xsp = X * sigp;
-  Coef<T> c;
   if (DISP == DISP_X) {
     const T DS = rt_fma(T(-2), S, v);
     const T DXn = rt_fma(sig, DS, -q1);
@@ -434,7 +458,8 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
     const T Dv = Dw - pat;
     const T DXn = rt_fma(q1, pw, rt_fma(P.one_plus_mu, ab, sig * DS));
     const T DYn = rt_fma(q2, pw, Xsp * DS);
-    const T s = rt_fma(v, Dv, rt_fma(u, Du, -rt_fma(Y2, DYn, X * DXn)));
+    c.YD = Y2 * DYn;
+    const T s = rt_fma(v, Dv, rt_fma(u, Du, -rt_fma(X, DXn, c.YD)));
     c.r = rt_rcp(s);
     c.A = Dv;
     c.C = Bc * Du;
@@ -673,8 +698,8 @@ RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const 
 //   f_Z = Z (Ax gx + Ab h^2 (1 - c r^2)) + C h (n_R + c Z m)
 //   f_phi = (n_phi (C h Z) + n_R (C g)) / R
 //   f_x = A n + C B':  C B'_R = -(C h) Z,  C B'_phi = C g,  C B'_Z = (C h) dR.
-template <class T, int EQ>
-RT_DEV typename Lane<T>::mask tokamak_full_rhs(const Params<T>& P, const T* y, T* f, T& r) {
+template <class T, int EQ, bool SERIES>
+RT_DEV typename Lane<T>::mask tokamak_full_rhs(const Params<T>& P, const T* y, T* f, T& r, typename Lane<T>::mask& fast) {
   const T* n = y + 3;
   const T R2 = rt_fma(y[0], y[0], y[1] * y[1]);
   const T iR = rt_rsqrt(R2);
@@ -702,23 +727,19 @@ RT_DEV typename Lane<T>::mask tokamak_full_rhs(const Params<T>& P, const T* y, T
   const T h = (P.sB0 * iq) * iR;
   const T g = P.sB0R0 * iR;
   const T c = P.two_q1_a2 * iq;
-  const T e = rt_fma(c, dR, iR);
   const T h2 = h * h;
-  const T giR = g * iR;
   const T Y2 = rt_fma(h2, r2, g * g);
   const T m = rt_fma(nZ, dR, -nR * Z);
   const T G = rt_fma(h, m, g * nP);
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
-  const Coef<T> k = disp_coefs<T, DISP_FULL, true>(P, X, Y2, G, v);
+  const Coef<T> k = disp_coefs<T, DISP_FULL, true, SERIES>(P, X, Y2, G, v);
   r = k.r;
+  fast = rt_and(fast, k.fast);
   const T Axg = k.Ax * gx, Abh2 = k.Ab * h2, Ch = k.C * h, Cg = k.C * g, ChZ = Ch * Z;
-  const T al = rt_fma(-r2, e, dR);                               // dR - r^2 e
-  const T be = rt_fma(-e, m, nZ);                                // n_Z - e m
-  const T ga = rt_fma(k.C, nP, -k.Ab * g);                       // C n_phi - Ab g
-  const T fR = rt_fma(Axg, dR, rt_fma(Abh2, al, rt_fma(giR, ga, -Ch * be)));
   const T ze = rt_fma(-c, r2, T(1));                             // 1 - c r^2
-  const T de = rt_fma(c * Z, m, nR);                             // n_R + c Z m
-  f[5] = rt_fma(Z, rt_fma(Abh2, ze, Axg), Ch * de);
+  const T K = rt_fma(Ch, c * m, rt_fma(Abh2, ze, Axg));          // Ax gx + Ab h^2 (1 - c r^2) + C h c m
+  const T fR = rt_fma(dR, K, rt_fma(-iR, k.YD, -Ch * nZ));
+  f[5] = rt_fma(Z, K, Ch * nR);
   const T fP = rt_fma(nP, ChZ, nR * Cg) * iR;
   f[3] = rt_fma(fR, cph, -fP * sph);
   f[4] = rt_fma(fR, sph, fP * cph);
@@ -735,8 +756,8 @@ RT_DEV typename Lane<T>::mask tokamak_full_rhs(const Params<T>& P, const T* y, T
 // hQ_R = F F' psi_R + psi_R psi_RR + psi_Z psi_RZ = (1/2) dQ/dR (hQ_Z likewise), g_R, g_Z the derivatives of g at fixed n:
 //   f_R = Ax gx psi_R + (Ab/R^2) hQ_R - (Ab |B|^2 + C (g_R - n.B))/R ,   f_Z = Ax gx psi_Z + (Ab/R^2) hQ_Z - (C/R) g_Z ,
 //   f_phi = (C/R) (n_phi psi_Z + n_R F)/R ,   C B = (C/R)(-psi_Z, F, psi_R).
-template <class T, class Gather>
-RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) {
+template <class T, bool SERIES, class Gather>
+RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather, typename Lane<T>::mask& fast) {
   const T* n = y + 3;
   const T R2 = rt_fma(y[0], y[0], y[1] * y[1]);
   const T iR = rt_rsqrt(R2);
@@ -761,10 +782,11 @@ RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f
   const T gR = rt_fma(nZ, psiRR, rt_fma(nPFp, V.psiR, -nR * V.psiRZ));
   const T gZ = rt_fma(nZ, V.psiRZ, rt_fma(nPFp, V.psiZ, -nR * psiZZ));
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
-  const Coef<T> k = disp_coefs<T, DISP_FULL, false>(P, X, b2, G, v);
+  const Coef<T> k = disp_coefs<T, DISP_FULL, false, SERIES>(P, X, b2, G, v);
   r = k.r;
+  fast = rt_and(fast, k.fast);
   const T Ci = k.C * iR, Ai2 = k.Ab * iR2, Axg = k.Ax * gx;
-  const T t2 = rt_fma(k.C, gR - G, k.Ab * b2);
+  const T t2 = rt_fma(k.C, gR, k.YD);                            // C (g_R - n.B) + Ab |B|^2 = C g_R + Y2 DYn (Ab = beta DYn + C (n.B)/|B|^2)
   const T fR = rt_fma(Axg, V.psiR, rt_fma(Ai2, hQR, -iR * t2));
   f[5] = rt_fma(Axg, V.psiZ, rt_fma(Ai2, hQZ, -Ci * gZ));
   const T fP = (Ci * iR) * rt_fma(nP, V.psiZ, nR * V.F);
@@ -780,8 +802,10 @@ RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f
 // ---- one evaluation of the ray right-hand side, y = (x, n) --------------------------------------------------------
 // Returns the right-hand side as (f, r): dy/dtau = r f, r = 1/s the reciprocal of the header comment.  Returns false
 // (and f, r unspecified) if x is outside the equilibrium's domain.
-template <class T, int EQ, int DISP, class Gather>
-RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather) {
+// SERIES: the ion terms of the Stix elements by their series (disp_coefs); `fast` is cleared (never set) if a point lies
+// outside the series' range, in which case the caller has to repeat the evaluation with SERIES = false.
+template <class T, int EQ, int DISP, bool SERIES, class Gather>
+RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r, Gather& gather, typename Lane<T>::mask& fast) {
   Local<T> L;
   const T* n = y + 3;
   if (EQ == EQ_PARABOLIC) {
@@ -795,8 +819,8 @@ RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r
     f[3] = -gx; f[4] = -gy; f[5] = T(0);
     return rt_true<T>();
   }
-  if ((EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) && DISP == DISP_FULL) return tokamak_full_rhs<T, EQ>(P, y, f, r);
-  if (EQ == EQ_GRID && DISP == DISP_FULL) return grid_full_rhs<T>(P, y, f, r, gather);
+  if ((EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) && DISP == DISP_FULL) return tokamak_full_rhs<T, EQ, SERIES>(P, y, f, r, fast);
+  if (EQ == EQ_GRID && DISP == DISP_FULL) return grid_full_rhs<T, SERIES>(P, y, f, r, gather, fast);
   constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
   const typename Lane<T>::mask inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
   const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
@@ -812,8 +836,9 @@ RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r
     }
     return inside;
   }
-  const Coef<T> c = disp_coefs<T, DISP, SC>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
+  const Coef<T> c = disp_coefs<T, DISP, SC, SERIES>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
   r = c.r;
+  fast = rt_and(fast, c.fast);
   f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
   if (EQ == EQ_LINEAR) {
     T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gxh);
@@ -844,11 +869,14 @@ RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r
   return inside;
 }
 
-// dy/dtau itself (diagnostics: rt_rhs)
+// dy/dtau itself (diagnostics: rt_rhs), evaluated the way the trace kernels do it: with the ion series first, exactly if the
+// point is outside the series' range
 template <class T, int EQ, int DISP, class Gather>
 RT_DEV typename Lane<T>::mask ray_rhs_scaled(const Params<T>& P, const T* y, T* f, Gather& gather) {
   T r;
-  const typename Lane<T>::mask inside = ray_rhs<T, EQ, DISP>(P, y, f, r, gather);
+  typename Lane<T>::mask fast = rt_true<T>();
+  typename Lane<T>::mask inside = ray_rhs<T, EQ, DISP, true>(P, y, f, r, gather, fast);
+  if (!rt_all(fast)) inside = ray_rhs<T, EQ, DISP, false>(P, y, f, r, gather, fast);
 #pragma unroll
   for (int j = 0; j < 6; ++j) f[j] *= r;
   return inside;

@@ -16,6 +16,30 @@ constexpr double kQe = 1.602176634e-19;     // C
 constexpr double kMe = 9.1093837139e-31;    // kg
 constexpr double kEps0 = 8.8541878188e-12;  // F/m
 
+// Range of the series the hot loop uses for the ion terms of the Stix elements (rt_math.cuh: disp_coefs, SERIES): the
+// largest Y2 = (W_ce/w)^2 up to which every term dropped from
+//   sig  = e1   + mu   e2   -> e1   + (mu + mu^3 Y2)        dropped: mu z^2/(1-z)              z = mu^2 Y2, e2 = 1/(1-z)
+//   sig' = e1^2 + mu^3 e2^2 -> e1^2 + mu^3                  dropped: mu^3 (2z - z^2)/(1-z)^2
+//   del  = mu^2 e2   - e1   -> (mu^2 + mu^4 Y2) - e1        dropped: mu^2 z^2/(1-z)
+//   del' = mu^4 e2^2 - e1^2 -> mu^4 - e1^2                  dropped: mu^4 (2z - z^2)/(1-z)^2
+// stays below `tol` (a quarter ulp of the working precision) relative to the smallest magnitude the electron term
+// e1 = 1/(1 - Y2) (resp. e1^2) takes on [0, Y2]: 1/max(1, Y2 - 1).  The bounds grow with Y2, so bisection finds the cap.
+// Deuterium, fp64: Y2 < 3.6 (w > 0.53 W_ce); electrons only (mu = 0): no limit.
+inline double series_cap(double mu, double tol) {
+  if (!(mu > 0.0)) return 1.7e308;
+  auto ok = [&](double Y2) {
+    const double z = mu * mu * Y2;
+    if (!(z < 0.5)) return false;
+    const double m = Y2 > 2.0 ? Y2 - 1.0 : 1.0;                          // 1 / min |e1| on [0, Y2] (ignoring the pole)
+    const double d1 = z * z / (1.0 - z), d2 = (2.0 * z - z * z) / ((1.0 - z) * (1.0 - z));
+    return mu * d1 * m <= tol && mu * mu * mu * d2 * m * m <= tol;        // the del / del' bounds are these times mu
+  };
+  double lo = 0.0, hi = 1.0;
+  while (ok(hi) && hi < 1e300) { lo = hi; hi *= 2.0; }
+  for (int it = 0; it < 100; ++it) { const double mid = 0.5 * (lo + hi); (ok(mid) ? lo : hi) = mid; }
+  return lo;
+}
+
 // d: the equilibrium's scalars; rho_max: resolved domain radius (tokamak); ne_scale: what the grid's n_e table was
 // divided by; psi_pp / prof_pp: device tables of element type T (grid kind), else NULL.
 template <class T>
@@ -34,6 +58,7 @@ Params<T> fold_params(const rt_equilibrium_desc& d, double rho_max, double ne_sc
   const double mu = (d.ion_mass > 0.0) ? d.ion_charge * kMe / d.ion_mass : 0.0;
   P.mu = (T)mu; P.mu2 = (T)(mu * mu); P.mu3 = (T)(mu * mu * mu); P.mu4 = (T)(mu * mu * mu * mu);
   P.one_plus_mu = (T)(1.0 + mu);
+  P.y2cap = (T)series_cap(mu, sizeof(T) == 8 ? 0x1p-54 : 0x1p-25);
   P.k2n = (T)(kC / omega);
   P.n2k = (T)(omega / kC);
   P.par_g = (T)(d.L != 0.0 ? xs / (d.L * d.L) : 0.0);

@@ -98,6 +98,38 @@ def _rf3(ins, lo, hi, fp_ops):
     return n3
 
 
+def _step_region(ins, fp_ops):
+    """(step loop, stage loop or None) of a trace / orbit kernel as address ranges [lo, hi).
+
+    Loop nest of the kernel = its backward branches.  The loops that hold FP-pipe instructions: the sample loop, inside it
+    the step loop -- for the magnetised dispersion functions TWO step loops side by side, the hot one (ion terms by their
+    series, rt_math.cuh: disp_coefs) and the rarely entered exact one, which holds more FP instructions -- and, when the
+    stages are rolled (grid equilibrium), a stage loop inside each step loop.  The small loops of the store staging and of
+    the cell-cache refill hold no FP instruction and are ignored.  Returned: the step loop with the fewest FP instructions
+    (the hot one)."""
+    loops = set()
+    for a, op, rest in ins:
+        if op.startswith("BRA"):
+            t = _target(rest)
+            if t is not None and t < a:
+                loops.add((t, a + 16))
+    nfp = {l: sum(1 for b, o, _ in ins if l[0] <= b < l[1] and o.split(".")[0] in fp_ops) for l in loops}
+    fpl = sorted((l for l in loops if nfp[l] > 0), key=lambda l: l[0] - l[1])            # largest first
+    if not fpl:
+        return None
+    inside = lambda a, b: b[0] <= a[0] and a[1] <= b[1] and a != b
+    outer = fpl[0]
+    if len(fpl) == 1:
+        return outer, None                                   # no sample loop distinguishable: the one loop is the step loop
+    assert all(inside(l, outer) for l in fpl[1:]), "FP loops outside the sample loop"
+    steps = [l for l in fpl[1:] if not any(inside(l, m) for m in fpl[1:])]               # maximal loops inside the sample loop
+    nmufu = lambda l: sum(1 for b, o, _ in ins if l[0] <= b < l[1] and o.startswith("MUFU"))
+    step = min(steps, key=lambda l: (nfp[l] + nmufu(l), l[0]))        # fp32: the series saves a MUFU seed, not an FP instruction
+    stages = [l for l in fpl[1:] if inside(l, step)]
+    assert len(stages) <= 1, "more than one FP loop inside the step loop"
+    return step, (stages[0] if stages else None)
+
+
 def count_kernels(lib: Path = LIB) -> dict:
     """{(precision 'f64'|'f32', eq_kind, disp_kind | 'orbit'): {'instr', 'rf3', 'executed', 'mufu', 'rsqrt', 'flops',
     'local'}} per ray-step (particle-step for the orbit kernels)."""
@@ -121,32 +153,20 @@ def count_kernels(lib: Path = LIB) -> dict:
             prec, eq, disp = "f", int(m2.group(1)), int(m2.group(2))
         ins = _parse(fn)
         fp_ops = _FP[prec] + (_FP2 if packed else ())
-        # Loop nest of the kernel = its backward branches.  The loops that hold FP-pipe instructions are nested:
-        # sample loop > step loop (> stage loop, when the stages are rolled: grid equilibrium).  The small loops of the
-        # store staging and of the cooperative cell-cache refill hold no FP instruction and are ignored.
-        loops = []
-        for a, op, rest in ins:
-            if op.startswith("BRA"):
-                t = _target(rest)
-                if t is not None and t < a:
-                    loops.append((t, a + 16))
-        nfp = {l: sum(1 for b, o, _ in ins if l[0] <= b < l[1] and o.split(".")[0] in fp_ops) for l in loops}
-        chain = sorted((l for l in loops if nfp[l] > 0), key=lambda l: l[1] - l[0])
-        if not chain:
+        sel = _step_region(ins, fp_ops)
+        if sel is None:
             continue
-        for small, big in zip(chain, chain[1:]):
-            assert big[0] <= small[0] and small[1] <= big[1], "FP loops are not nested"
-        rolled = len(chain) >= 3
-        region = chain[1] if rolled else chain[0]          # the step loop's body = one ray-step
+        region, stage = sel
+        rolled = stage is not None
         c, rsq = _count(ins, *region)
         tot = Counter(c)
         rf3 = _rf3(ins, *region, fp_ops)
         if rolled:                                          # the stage loop runs 4 times per step
-            ci, rsqi = _count(ins, *chain[0])
+            ci, rsqi = _count(ins, *stage)
             for k, v in ci.items():
                 tot[k] += 3 * v
             rsq += 3 * rsqi
-            rf3 += 3 * _rf3(ins, *chain[0], fp_ops)
+            rf3 += 3 * _rf3(ins, *stage, fp_ops)
         fma, mul, add, setp = _FP[prec]
         local = tot["STL"] + tot["LDL"]                     # spill traffic executed per ray-step (must be 0)
         if packed:
