@@ -52,7 +52,7 @@ UNIT = "ray-steps/s"
 FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 247, (4, "f64"): 707, (5, "f64"): 1200,
                       (1, "f32"): 117, (2, "f32"): 117, (3, "f32"): 250, (4, "f32"): 711, (5, "f32"): 1200}
 FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 197, (4, "f64"): 553, (5, "f64"): 820,
-                         (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 178, (4, "f32"): 484, (5, "f32"): 774}
+                         (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 178, (4, "f32"): 484, (5, "f32"): 775}
 # FP_RF3_PER_RAY_STEP: how many of those instructions read THREE DISTINCT registers from the register file.  Such an instruction
 # occupies the FP64 pipe for 3 cycles instead of 2 (scalar FP32: 1.56 slots instead of 1; packed f32x2: 3 cycles instead of 2) -- measured by
 # rt_fma_peak_shape, shapes 2 / 6 (profiles/r1_fma_peak_shapes.md, r2_fma_peak_shapes.md) -- so the pipe time of a ray-step is
@@ -60,9 +60,9 @@ FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 197, (4, "f
 # time.  The fp32 kernels of the analytic equilibria (configs 1-4) are the packed two-rays-per-thread
 # kernels (trace_kernel_x2); their counts are per ray (a packed instruction = one slot per ray).
 FP_RF3_PER_RAY_STEP = {(1, "f64"): 27, (2, "f64"): 27, (3, "f64"): 42, (4, "f64"): 134, (5, "f64"): 312,
-                       (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 45, (4, "f32"): 143, (5, "f32"): 240}
+                       (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 45, (4, "f32"): 143, (5, "f32"): 276}
 RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1: 63.9 / 42.7, 123.2 / 78.8; packed 127.9 / 84.9
-PACKED = {(c, "f32") for c in (1, 2, 3, 4)}              # (config, precision) pairs that run trace_kernel_x2
+PACKED = {(c, "f32") for c in (1, 2, 3, 4, 5)}           # (config, precision) pairs that run trace_kernel_x2
 # The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from
 # sass_count.py's orbit_kernel rows (pinned by the same test).
 ORBIT_COUNTS = {"f64": dict(flops=238, instr=184, rf3=50), "f32": dict(flops=238, instr=162, rf3=50)}

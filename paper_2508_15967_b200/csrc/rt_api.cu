@@ -109,12 +109,15 @@ unsigned grid_for(long long n, int block) { return (unsigned)((n + block - 1) / 
   M(rt::EQ_TOKAMAK_POW, rt::DISP_O) M(rt::EQ_TOKAMAK_POW, rt::DISP_X) M(rt::EQ_TOKAMAK_POW, rt::DISP_FULL)  \
   M(rt::EQ_GRID, rt::DISP_O) M(rt::EQ_GRID, rt::DISP_X) M(rt::EQ_GRID, rt::DISP_FULL)
 
-// fp32, analytic equilibria, one frequency, no resume: the packed two-rays-per-thread kernels (rt_kernels.cuh)
-#define RT_FOR_ANALYTIC_COMBOS(M)                          \
+// fp32, one frequency, no resume: the packed two-rays-per-thread kernels (rt_kernels.cuh) -- every analytic equilibrium, and
+// the grid equilibrium with the full determinant (spline look-ups per ray in scalar arithmetic, the rest packed)
+#define RT_FOR_PACKED_COMBOS(M)                            \
   M(rt::EQ_PARABOLIC, rt::DISP_O)                          \
   M(rt::EQ_LINEAR, rt::DISP_O) M(rt::EQ_LINEAR, rt::DISP_X) M(rt::EQ_LINEAR, rt::DISP_FULL)     \
   M(rt::EQ_TOKAMAK, rt::DISP_O) M(rt::EQ_TOKAMAK, rt::DISP_X) M(rt::EQ_TOKAMAK, rt::DISP_FULL)  \
-  M(rt::EQ_TOKAMAK_POW, rt::DISP_O) M(rt::EQ_TOKAMAK_POW, rt::DISP_X) M(rt::EQ_TOKAMAK_POW, rt::DISP_FULL)
+  M(rt::EQ_TOKAMAK_POW, rt::DISP_O) M(rt::EQ_TOKAMAK_POW, rt::DISP_X) M(rt::EQ_TOKAMAK_POW, rt::DISP_FULL)  \
+  M(rt::EQ_GRID, rt::DISP_FULL)
+constexpr bool has_packed_kernel(int eq_kind, int disp) { return eq_kind != rt::EQ_GRID || disp == rt::DISP_FULL; }
 int launch_trace_x2(const rt_equilibrium* eq, int disp, const rt::Params<float>& P, const rt::TraceArgs<float>& A, cudaStream_t st) {
 #define M(E, D)                                                                                        \
   if (kernel_kind(eq) == (E) && disp == (D)) {                                                         \
@@ -124,7 +127,7 @@ int launch_trace_x2(const rt_equilibrium* eq, int disp, const rt::Params<float>&
     RT_CUDA(cudaGetLastError());                                                                       \
     return RT_OK;                                                                                      \
   }
-  RT_FOR_ANALYTIC_COMBOS(M)
+  RT_FOR_PACKED_COMBOS(M)
 #undef M
   return fail(RT_ERR_UNSUPPORTED, "no packed kernel for this equilibrium / dispersion combination");
 }
@@ -135,7 +138,7 @@ int launch_trace_x2(const rt_equilibrium*, int, const rt::Params<double>&, const
 template <class T>
 int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, const rt::TraceArgs<T>& A, cudaStream_t st) {
   if (A.n_rays == 0) return RT_OK;
-  if (sizeof(T) == 4 && !A.omega && !A.status_in && eq->d.kind != RT_EQ_GRID_RZ) return launch_trace_x2(eq, disp, P, A, st);
+  if (sizeof(T) == 4 && !A.omega && !A.status_in && has_packed_kernel(kernel_kind(eq), disp)) return launch_trace_x2(eq, disp, P, A, st);
 #define M(E, D)                                                                            \
   if (kernel_kind(eq) == (E) && disp == (D)) {                                             \
     constexpr int block = rt::TraceShape<T, E>::BLOCK;                                     \
@@ -143,7 +146,7 @@ int launch_trace(const rt_equilibrium* eq, int disp, const rt::Params<T>& P, con
       rt::trace_kernel<T, E, D, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A);  \
     else if (A.status_in)                                                                  \
       rt::trace_kernel<T, E, D, false, true><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
-    else if constexpr (!(sizeof(T) == 4 && (E) != rt::EQ_GRID))   /* fp32 analytic: the packed kernels, above */ \
+    else if constexpr (!(sizeof(T) == 4 && has_packed_kernel((E), (D))))   /* fp32: the packed kernels, above */ \
       rt::trace_kernel<T, E, D, false><<<grid_for(A.n_rays, block), block, 0, st>>>(P, A); \
     ++g_launches;                                                                          \
     RT_CUDA(cudaGetLastError());                                                           \

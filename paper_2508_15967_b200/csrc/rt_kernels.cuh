@@ -213,6 +213,10 @@ struct GatherCached {
   }
 };
 
+// the packed fp32 kernel of the grid equilibrium: one scalar cell cache per ray of the thread (rt_math.cuh: grid_values_per_ray)
+template <int BLOCK> struct GatherPair { GatherCached<float, BLOCK> a, b; };
+template <int BLOCK> struct gather_is_pair<GatherPair<BLOCK>> { static constexpr bool value = true; };
+
 template <class T, int EQ> struct TraceGather { typedef GatherDirect type; };
 template <class T> struct TraceGather<T, EQ_GRID> { typedef GatherCached<T, TraceShape<T, EQ_GRID>::BLOCK> type; };
 
@@ -377,8 +381,14 @@ trace_kernel_x2(const __grid_constant__ Params<float> P0, const __grid_constant_
   const long long N = A.n_rays;
   const long long ia = ((long long)blockIdx.x * BLOCK + threadIdx.x) * 2, ib = ia + 1;
   const bool va = ia < N, vb = ib < N;
-  static_assert(EQ != EQ_GRID, "the packed kernels cover the analytic equilibria");
-  GatherDirect gather;
+  static_assert(EQ != EQ_GRID || DISP == DISP_FULL, "grid equilibrium: the packed kernel exists for the full determinant");
+  typename std::conditional<EQ == EQ_GRID, GatherPair<BLOCK>, GatherDirect>::type gather;
+  if constexpr (EQ == EQ_GRID) {
+    typedef GatherCached<float, BLOCK> GC;
+    __shared__ typename GC::V cache[2 * GC::CHUNKS * BLOCK];
+    gather.a.col = cache + threadIdx.x;              gather.a.cell = -1; gather.a.pcell = -1;
+    gather.b.col = cache + GC::CHUNKS * BLOCK + threadIdx.x; gather.b.cell = -1; gather.b.pcell = -1;
+  }
   __shared__ __align__(16) float stage[7 * RAYS];
   T y[6];
 #pragma unroll
@@ -397,7 +407,8 @@ trace_kernel_x2(const __grid_constant__ Params<float> P0, const __grid_constant_
     T v[7];
 #pragma unroll
     for (int c = 0; c < 3; ++c) { v[c] = y[c]; v[3 + c] = y[3 + c] * P.n2k; }
-    v[6] = res_row ? abs_residual<T, EQ, DISP>(P, y, gather) : T(0.0f);
+    GatherDirect direct;                                                           // once per sample: straight from the tables
+    v[6] = res_row ? abs_residual<T, EQ, DISP>(P, y, direct) : T(0.0f);
     if ((NN & 3) != 0) {                                                           // rows not 16-byte aligned: scalar stores
       const long long ja = i0 + 2 * lane;
 #pragma unroll

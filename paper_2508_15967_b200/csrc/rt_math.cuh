@@ -599,6 +599,31 @@ RT_DEV typename Lane<T>::mask grid_splines(const Params<T>& P, T R, T Z, Gather&
 }
 
 
+// How grid_full_rhs reaches the spline look-ups.  Normally the look-ups run in the caller's lane type.  The packed fp32 trace
+// kernel of the grid equilibrium (rt_kernels.cuh: trace_kernel_x2<EQ_GRID>) instead does them PER RAY in scalar arithmetic,
+// each ray with its own shared-memory cell cache, and packs the nine results: the pieces of a cell come out of shared
+// memory as four consecutive registers per row, which suits scalar Horner steps as they are, whereas packed Horner steps
+// would need every piece paired with the other ray's first (measured: ~100 register moves per stage, profiles/r2_tuning.md).
+template <class G> struct gather_is_pair { static constexpr bool value = false; };
+template <class T, int DISP, class Gather>
+RT_DEV typename Lane<T>::mask grid_values(const Params<T>& P, T R, T Z, Gather& gather, GridVals<T>& V) {
+  return grid_splines<T, DISP>(P, R, Z, gather, V);
+}
+#ifdef __CUDACC__
+template <int DISP, class Pair>
+RT_DEV mask2 grid_values_per_ray(const Params<f32x2>& P, f32x2 R, f32x2 Z, Pair& gather, GridVals<f32x2>& V) {
+  const Params<float>& Pf = P;
+  GridVals<float> a, b;
+  mask2 in;
+  in.a = grid_splines<float, DISP>(Pf, R.lo(), Z.lo(), gather.a, a);
+  in.b = grid_splines<float, DISP>(Pf, R.hi(), Z.hi(), gather.b, b);
+  V.psiR = f32x2(a.psiR, b.psiR); V.psiZ = f32x2(a.psiZ, b.psiZ); V.psiRRh = f32x2(a.psiRRh, b.psiRRh);
+  V.psiRZ = f32x2(a.psiRZ, b.psiRZ); V.psiZZh = f32x2(a.psiZZh, b.psiZZh);
+  V.F = f32x2(a.F, b.F); V.Fp = f32x2(a.Fp, b.Fp); V.Ne = f32x2(a.Ne, b.Ne); V.Nep = f32x2(a.Nep, b.Nep);
+  return in;
+}
+#endif
+
 template <class T, int EQ, int DISP, bool SC = false, class Gather>
 RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const T* n, Local<T>& L, Gather& gather) {
   typedef typename Lane<T>::mask M;
@@ -767,7 +792,9 @@ RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f
   const T nP = rt_fma(n[1], cph, -n[0] * sph);
   const T nZ = n[2];
   GridVals<T> V;
-  const typename Lane<T>::mask inside = grid_splines<T, DISP_FULL>(P, R, y[2], gather, V);
+  typename Lane<T>::mask inside;
+  if constexpr (gather_is_pair<Gather>::value) inside = grid_values_per_ray<DISP_FULL>(P, R, y[2], gather, V);
+  else inside = grid_values<T, DISP_FULL>(P, R, y[2], gather, V);
   const T X = P.xs * V.Ne, gx = P.xsh * V.Nep;
   const T iR2 = iR * iR;
   const T Q = rt_fma(V.F, V.F, rt_fma(V.psiR, V.psiR, V.psiZ * V.psiZ));
@@ -819,54 +846,58 @@ RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r
     f[3] = -gx; f[4] = -gy; f[5] = T(0);
     return rt_true<T>();
   }
-  if ((EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) && DISP == DISP_FULL) return tokamak_full_rhs<T, EQ, SERIES>(P, y, f, r, fast);
-  if (EQ == EQ_GRID && DISP == DISP_FULL) return grid_full_rhs<T, SERIES>(P, y, f, r, gather, fast);
-  constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
-  const typename Lane<T>::mask inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
-  const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
-  if (DISP == DISP_O) {
-    // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)   =>   dx/dtau = n r, dn/dtau = -grad X r/2, r = 1/(v+X)
-    r = rt_rcp(v + L.X);
-    f[0] = n[0]; f[1] = n[1]; f[2] = n[2];
-    if (EQ == EQ_LINEAR) {
-      f[3] = -P.lin_gxh; f[4] = T(0); f[5] = T(0);
-    } else {
-      const T fR = -L.hgX[0];
-      f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = -L.hgX[2];
-    }
-    return inside;
-  }
-  const Coef<T> c = disp_coefs<T, DISP, SC, SERIES>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
-  r = c.r;
-  fast = rt_and(fast, c.fast);
-  f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
-  if (EQ == EQ_LINEAR) {
-    T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gxh);
-    if (DISP == DISP_FULL) {
-      f[2] = rt_fma(c.C, L.B[2], f[2]);
-      fn = rt_fma(-c.C, L.gG[0], fn);
-    }
-    f[3] = fn; f[4] = T(0); f[5] = T(0);
-    return inside;
-  }
-  // axisymmetric kinds: assemble in (R^, phi^, Z^), rotate to Cartesian
-  T fR = rt_fma(c.Ab, L.hgb2[0], c.Ax * L.hgX[0]);
-  T fZ = rt_fma(c.Ab, L.hgb2[2], c.Ax * L.hgX[2]);
-  if (DISP == DISP_FULL) {
-    const T xR = c.C * L.B[0], xP = c.C * L.B[1];
-    f[0] = rt_fma(xR, L.cph, rt_fma(-xP, L.sph, f[0]));
-    f[1] = rt_fma(xR, L.sph, rt_fma(xP, L.cph, f[1]));
-    f[2] = rt_fma(c.C, L.B[2], f[2]);
-    fR = rt_fma(-c.C, L.gG[0], fR);
-    fZ = rt_fma(-c.C, L.gG[2], fZ);
-    const T fP = -c.C * L.gG[1];
-    f[3] = rt_fma(fR, L.cph, -fP * L.sph);
-    f[4] = rt_fma(fR, L.sph, fP * L.cph);
+  if constexpr ((EQ == EQ_TOKAMAK || EQ == EQ_TOKAMAK_POW) && DISP == DISP_FULL) {
+    return tokamak_full_rhs<T, EQ, SERIES>(P, y, f, r, fast);
+  } else if constexpr (EQ == EQ_GRID && DISP == DISP_FULL) {
+    return grid_full_rhs<T, SERIES>(P, y, f, r, gather, fast);
   } else {
-    f[3] = fR * L.cph; f[4] = fR * L.sph;
+    constexpr bool SC = (EQ != EQ_GRID);      // analytic fields come in units of 1/sqrt(beta); the grid's table is in tesla
+    const typename Lane<T>::mask inside = equilibrium<T, EQ, DISP, SC>(P, y, n, L, gather);
+    const T v = rt_fma(n[0], n[0], rt_fma(n[1], n[1], n[2] * n[2]));
+    if (DISP == DISP_O) {
+      // D = v - 1 + X:  dD/dn = 2 n, dD/dx = grad X, W = -2 (v + X)   =>   dx/dtau = n r, dn/dtau = -grad X r/2, r = 1/(v+X)
+      r = rt_rcp(v + L.X);
+      f[0] = n[0]; f[1] = n[1]; f[2] = n[2];
+      if (EQ == EQ_LINEAR) {
+        f[3] = -P.lin_gxh; f[4] = T(0); f[5] = T(0);
+      } else {
+        const T fR = -L.hgX[0];
+        f[3] = fR * L.cph; f[4] = fR * L.sph; f[5] = -L.hgX[2];
+      }
+      return inside;
+    }
+    const Coef<T> c = disp_coefs<T, DISP, SC, SERIES>(P, L.X, L.b2, (DISP == DISP_FULL) ? L.G : T(0), v);
+    r = c.r;
+    fast = rt_and(fast, c.fast);
+    f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
+    if (EQ == EQ_LINEAR) {
+      T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gxh);
+      if (DISP == DISP_FULL) {
+        f[2] = rt_fma(c.C, L.B[2], f[2]);
+        fn = rt_fma(-c.C, L.gG[0], fn);
+      }
+      f[3] = fn; f[4] = T(0); f[5] = T(0);
+      return inside;
+    }
+    // axisymmetric kinds: assemble in (R^, phi^, Z^), rotate to Cartesian
+    T fR = rt_fma(c.Ab, L.hgb2[0], c.Ax * L.hgX[0]);
+    T fZ = rt_fma(c.Ab, L.hgb2[2], c.Ax * L.hgX[2]);
+    if (DISP == DISP_FULL) {
+      const T xR = c.C * L.B[0], xP = c.C * L.B[1];
+      f[0] = rt_fma(xR, L.cph, rt_fma(-xP, L.sph, f[0]));
+      f[1] = rt_fma(xR, L.sph, rt_fma(xP, L.cph, f[1]));
+      f[2] = rt_fma(c.C, L.B[2], f[2]);
+      fR = rt_fma(-c.C, L.gG[0], fR);
+      fZ = rt_fma(-c.C, L.gG[2], fZ);
+      const T fP = -c.C * L.gG[1];
+      f[3] = rt_fma(fR, L.cph, -fP * L.sph);
+      f[4] = rt_fma(fR, L.sph, fP * L.cph);
+    } else {
+      f[3] = fR * L.cph; f[4] = fR * L.sph;
+    }
+    f[5] = fZ;
+    return inside;
   }
-  f[5] = fZ;
-  return inside;
 }
 
 // dy/dtau itself (diagnostics: rt_rhs), evaluated the way the trace kernels do it: with the ion series first, exactly if the

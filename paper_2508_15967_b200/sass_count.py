@@ -19,7 +19,8 @@ Reported per kernel:
 * f32, analytic equilibria: the kernels that run are ``trace_kernel_x2`` (two rays per thread, packed f32x2 arithmetic).
                 Their loop body advances two rays; the counts are reported PER RAY: a packed FFMA2 / FMUL2 / FADD2 is one
                 pipe slot per ray (it occupies the FMA pipe for two cycles and does the operation for both rays), a scalar
-                FP instruction or MUFU seed half a slot.  ``rf3`` counts packed instructions with three distinct register
+                FP instruction or MUFU seed (they serve ONE of the two rays: per-half domain tests, and the per-ray spline
+                look-ups of the grid equilibrium's packed kernel) half a slot; likewise for ``rf3``.  ``rf3`` counts packed instructions with three distinct register
                 operands: 3 pipe cycles instead of 2 (84.9 against 127.9 FMA per clock per SM, ``rt_fma_peak_shape`` shapes 6 / 5);
 * ``local``     local-memory (spill) instructions executed per ray-step: must be 0.  ptxas may still report a few bytes
                 of spill for values parked once before the step loop and reloaded after it (the store staging);
@@ -160,13 +161,15 @@ def count_kernels(lib: Path = LIB) -> dict:
         rolled = stage is not None
         c, rsq = _count(ins, *region)
         tot = Counter(c)
-        rf3 = _rf3(ins, *region, fp_ops)
-        if rolled:                                          # the stage loop runs 4 times per step
+
+        def rf3_of(ops):                                    # the stage loop (rolled stages) runs 4 times per step
+            return _rf3(ins, *region, ops) + (3 * _rf3(ins, *stage, ops) if rolled else 0)
+        rf3 = rf3_of(fp_ops)
+        if rolled:
             ci, rsqi = _count(ins, *stage)
             for k, v in ci.items():
                 tot[k] += 3 * v
             rsq += 3 * rsqi
-            rf3 += 3 * _rf3(ins, *stage, fp_ops)
         fma, mul, add, setp = _FP[prec]
         local = tot["STL"] + tot["LDL"]                     # spill traffic executed per ray-step (must be 0)
         if packed:
@@ -177,7 +180,8 @@ def count_kernels(lib: Path = LIB) -> dict:
             executed = 2 * tot["FFMA2"] + tot["FMUL2"] + tot["FADD2"] + (2 * tot[fma] + tot[mul] + tot[add] + 1) // 2
             mufu, rsq = tot["MUFU"] // 2, rsq // 2
             res[("f32", eq, disp)] = dict(instr=n2 + (n1 + 1) // 2, executed=executed, mufu=mufu, rsqrt=rsq,
-                                          flops=executed + mufu, local=local, rf3=rf3, packed=True)
+                                          flops=executed + mufu, local=local,
+                                          rf3=rf3_of(_FP2) + (rf3_of(_FP[prec]) + 1) // 2, packed=True)
             continue
         executed = 2 * tot[fma] + tot[mul] + tot[add]
         mufu = tot["MUFU"]

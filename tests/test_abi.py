@@ -212,7 +212,7 @@ def test_flop_tables_match_the_compiled_kernels(lib):
     # (rt_trace_until's chunk kernel)}, where the 10 plain fp32 kernels of the analytic equilibria are the packed
     # trace_kernel_x2 instead of trace_kernel<float, ...>
     assert len(traces) == 78
-    assert sum("trace_kernel_x2" in b.split("\n")[0] for b in traces) == 10
+    assert sum("trace_kernel_x2" in b.split("\n")[0] for b in traces) == 11
     import re
     spilled = [max(int(x) for x in re.findall(r"(\d+) bytes spill stores", b)) for b in traces]
     assert max(spilled) <= 64, spilled
