@@ -163,7 +163,8 @@ RT_DEV void unpack4(const float4* s, int row, int pitch, float* c) {
   c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w;
 }
 
-template <class T, int BLOCK>
+// ASYNC_PROF: the profile pieces' refill as cp.async too (worth it only where other work separates request and wait)
+template <class T, int BLOCK, bool ASYNC_PROF = false>
 struct GatherCached {
   typedef typename Vec16<T>::type V;
   // fp64: the 8 pieces of the two 1-D profiles stay in REGISTERS while the psi-cell is unchanged (about ten stages), so a
@@ -176,32 +177,43 @@ struct GatherCached {
   V* col;                  // this thread's column: chunk j at col[j * BLOCK]
   int cell, pcell;         // cached cell indices (-1: nothing cached)
   T prof[PROF_REGS ? 8 : 1];
-  RT_DEV void psi_select(const Params<T>& P, int c) {
+  // refill: global -> shared directly (cp.async, 16 bytes per chunk), no staging through registers and no separate STS;
+  // wait() before the column is read.  A thread's copies all land in its own column: no barrier is needed.
+  // (both requests return whether a copy was issued that wait() has to cover)
+  RT_DEV bool psi_request(const Params<T>& P, int c) {
     if (c != cell) {
-      // refill: global -> shared directly (cp.async, 16 bytes per chunk), no staging through registers and no separate
-      // STS; the thread waits for its own copies before it reads its column
       const V* g = reinterpret_cast<const V*>(P.psi_pp + (size_t)c * 16);
       const unsigned dst = (unsigned)__cvta_generic_to_shared(col);
 #pragma unroll
       for (int j = 0; j < PSI_CHUNKS; ++j)
         asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + (unsigned)(j * BLOCK * sizeof(V))), "l"(g + j) : "memory");
-      asm volatile("cp.async.wait_all;" ::: "memory");
       cell = c;
+      return true;
     }
+    return false;
   }
-  RT_DEV void prof_select(const Params<T>& P, int c) {
+  RT_DEV bool prof_request(const Params<T>& P, int c) {
     if (c != pcell) {
       if (PROF_REGS) {
         ld4(P.prof_pp + (size_t)c * 8, prof);
         ld4(P.prof_pp + (size_t)c * 8 + 4, prof + 4);
-      } else {
+      } else if (ASYNC_PROF) {
+        const V* g = reinterpret_cast<const V*>(P.prof_pp + (size_t)c * 8);
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(col + PSI_CHUNKS * BLOCK);
+#pragma unroll
+        for (int j = 0; j < PROF_CHUNKS; ++j)
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + (unsigned)(j * BLOCK * sizeof(V))), "l"(g + j) : "memory");
+      } else {           // scalar fp32 kernels: load + store (the wait follows at once; cp.async here: 282 -> 305 ms)
         const V* g = reinterpret_cast<const V*>(P.prof_pp + (size_t)c * 8);
 #pragma unroll
-        for (int j = 0; j < PROF_CHUNKS; ++j) col[(PSI_CHUNKS + j) * BLOCK] = __ldg(g + j);   // (cp.async here: 282 -> 305 ms)
+        for (int j = 0; j < PROF_CHUNKS; ++j) col[(PSI_CHUNKS + j) * BLOCK] = __ldg(g + j);
       }
       pcell = c;
+      return !PROF_REGS && ASYNC_PROF;
     }
+    return false;
   }
+  RT_DEV void wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
   RT_DEV void psi_row(const Params<T>&, int, int p, T* c) const { unpack4(col, p, BLOCK, c); }
   RT_DEV void prof_row(const Params<T>&, int, int which, T* c) const {
     if (PROF_REGS) {
@@ -214,7 +226,7 @@ struct GatherCached {
 };
 
 // the packed fp32 kernel of the grid equilibrium: one scalar cell cache per ray of the thread (rt_math.cuh: grid_values_per_ray)
-template <int BLOCK> struct GatherPair { GatherCached<float, BLOCK> a, b; };
+template <int BLOCK> struct GatherPair { GatherCached<float, BLOCK, true> a, b; };
 template <int BLOCK> struct gather_is_pair<GatherPair<BLOCK>> { static constexpr bool value = true; };
 
 template <class T, int EQ> struct TraceGather { typedef GatherDirect type; };
@@ -384,7 +396,7 @@ trace_kernel_x2(const __grid_constant__ Params<float> P0, const __grid_constant_
   static_assert(EQ != EQ_GRID || DISP == DISP_FULL, "grid equilibrium: the packed kernel exists for the full determinant");
   typename std::conditional<EQ == EQ_GRID, GatherPair<BLOCK>, GatherDirect>::type gather;
   if constexpr (EQ == EQ_GRID) {
-    typedef GatherCached<float, BLOCK> GC;
+    typedef GatherCached<float, BLOCK, true> GC;
     __shared__ typename GC::V cache[2 * GC::CHUNKS * BLOCK];
     gather.a.col = cache + threadIdx.x;              gather.a.cell = -1; gather.a.pcell = -1;
     gather.b.col = cache + GC::CHUNKS * BLOCK + threadIdx.x; gather.b.cell = -1; gather.b.pcell = -1;

@@ -239,8 +239,9 @@ template <class T> RT_DEV void ld4(const T* p, T* c) { for (int i = 0; i < 4; ++
 // How the grid equilibrium fetches a cell's spline pieces.  GatherDirect reads the global tables (diagnostic kernels,
 // launch solver, host builds); the trace kernel passes a shared-memory cell cache instead (rt_kernels.cuh: GatherCached).
 struct GatherDirect {
-  template <class T, class I> RT_DEV void psi_select(const Params<T>&, I) {}
-  template <class T, class I> RT_DEV void prof_select(const Params<T>&, I) {}
+  template <class T, class I> RT_DEV bool psi_request(const Params<T>&, I) { return false; }
+  template <class T, class I> RT_DEV bool prof_request(const Params<T>&, I) { return false; }
+  RT_DEV void wait() {}
   template <class T> RT_DEV void psi_row(const Params<T>& P, int cell, int p, T* c) const { ld4(P.psi_pp + (size_t)cell * 16 + 4 * p, c); }
   template <class T> RT_DEV void prof_row(const Params<T>& P, int cell, int which, T* c) const { ld4(P.prof_pp + (size_t)cell * 8 + 4 * which, c); }
 #ifdef __CUDACC__
@@ -522,23 +523,31 @@ RT_DEV void axisym_field(T iR, T psiR, T psiZ, T psiRRh, T psiRZ, T psiZZh, T F,
 template <class T>
 struct GridVals { T psiR, psiZ, psiRRh, psiRZ, psiZZh, F, Fp, Ne, Nep; };
 
-template <class T, int DISP, class Gather>
-RT_DEV typename Lane<T>::mask grid_splines(const Params<T>& P, T R, T Z, Gather& gather, GridVals<T>& V) {
-  typedef typename Lane<T>::mask M;
+// The look-up in four parts, so that a caller with several rays in flight (the packed kernel, below) can issue every ray's
+// cell-cache refill before it waits for any of them:
+//   grid_psi_cell   cell index and offsets of (R, Z), rectangle test          -> gather.psi_request(cell) [+ gather.wait()]
+//   grid_psi_eval   psi and its derivatives from the cell's 16 pieces, psi-range test
+//   grid_prof_cell  profile cell index and offset of psi                      -> gather.prof_request(cell) [+ gather.wait()]
+//   grid_prof_eval  F, F', n_e, n_e' from the profile cell's 8 pieces
+template <class T>
+RT_DEV typename Lane<T>::index grid_psi_cell(const Params<T>& P, T R, T Z, typename Lane<T>::mask& inside, T& dR, T& dZ) {
   // R > 0 is implied by R >= Rmin: rt_create_equilibrium requires Rmin > 0.  Inside the rectangle R - Rmin >= +0 exactly,
   // so the cell index is >= 0 and only needs the upper clamp (R = Rmax belongs to the last cell); outside -- including NaN
   // positions, which convert to unspecified ints -- the index is forced to 0 to keep the gather in bounds.
   typedef typename Lane<T>::index I;
-  M inside = rt_and(rt_and(R >= T(P.Rmin), R <= T(P.Rmax)), rt_and(Z >= T(P.Zmin), Z <= T(P.Zmax)));
+  inside = rt_and(rt_and(R >= T(P.Rmin), R <= T(P.Rmax)), rt_and(Z >= T(P.Zmin), Z <= T(P.Zmax)));
   const T Ro = R - P.Rmin, Zo = Z - P.Zmin;                       // offsets from the grid's corner
   I iRc = rt_imin(rt_floor_int(Ro * P.inv_hR), P.nRc - 1);
   I iZc = rt_imin(rt_floor_int(Zo * P.inv_hZ), P.nZc - 1);
   iRc = rt_select(inside, iRc, 0); iZc = rt_select(inside, iZc, 0);
   // offset inside the cell: (R - Rmin) - i hR in one fused step (i hR is exact in the fma; the oracle's R - (Rmin + i hR)
   // differs by a rounding of R)
-  const T dR = rt_fma(-rt_from_index<T>(iRc), T(P.hR), Ro), dZ = rt_fma(-rt_from_index<T>(iZc), T(P.hZ), Zo);
-  const I cell = iRc * P.nZc + iZc;
-  gather.psi_select(P, cell);
+  dR = rt_fma(-rt_from_index<T>(iRc), T(P.hR), Ro); dZ = rt_fma(-rt_from_index<T>(iZc), T(P.hZ), Zo);
+  return iRc * P.nZc + iZc;
+}
+
+template <class T, int DISP, class Gather>
+RT_DEV T grid_psi_eval(const Params<T>& P, typename Lane<T>::index cell, T dR, T dZ, Gather& gather, GridVals<T>& V) {
   T a[4], a1[4], a2h[4];   // a_p(dZ) = sum_q c[p][q] dZ^q, its first dZ-derivative and half its second
   T psi, psiR, psiRRh = T(0), psiZ, psiRZ = T(0), psiZZh = T(0);
   if (sizeof(T) == 8 && DISP != DISP_O) {
@@ -570,13 +579,24 @@ RT_DEV typename Lane<T>::mask grid_splines(const Params<T>& P, T R, T Z, Gather&
       psiZZh = rt_fma(rt_fma(rt_fma(a2h[3], dR, a2h[2]), dR, a2h[1]), dR, a2h[0]);
     }
   }
+  V.psiR = psiR; V.psiZ = psiZ; V.psiRRh = psiRRh; V.psiRZ = psiRZ; V.psiZZh = psiZZh;
+  return psi;
+}
+
+template <class T>
+RT_DEV typename Lane<T>::index grid_prof_cell(const Params<T>& P, T psi, typename Lane<T>::mask& inside, T& ds) {
+  typedef typename Lane<T>::index I;
   inside = rt_and(inside, rt_and(psi >= T(P.psi_min), psi <= T(P.psi_max)));
   const T po = psi - P.psi_min;
   I iP = rt_imin(rt_floor_int(po * P.inv_hP), P.nPc - 1);                        // same argument: psi >= psi_min when inside
   iP = rt_select(inside, iP, 0);
-  const T ds = rt_fma(-rt_from_index<T>(iP), T(P.hP), po);
+  ds = rt_fma(-rt_from_index<T>(iP), T(P.hP), po);
+  return iP;
+}
+
+template <class T, int DISP, class Gather>
+RT_DEV void grid_prof_eval(const Params<T>& P, typename Lane<T>::index iP, T ds, Gather& gather, GridVals<T>& V) {
   T Ne, Nep, F = T(0), Fp = T(0);
-  gather.prof_select(P, iP);
   if (sizeof(T) == 8 && DISP != DISP_O) {
     T pq[2][4], v[2], v1[2];
     gather.prof_row(P, iP, 1, pq[0]);
@@ -593,11 +613,21 @@ RT_DEV typename Lane<T>::mask grid_splines(const Params<T>& P, T R, T Z, Gather&
       cubic01(f, ds, F, Fp);
     }
   }
-  V.psiR = psiR; V.psiZ = psiZ; V.psiRRh = psiRRh; V.psiRZ = psiRZ; V.psiZZh = psiZZh;
   V.F = F; V.Fp = Fp; V.Ne = Ne; V.Nep = Nep;
-  return inside;
 }
 
+template <class T, int DISP, class Gather>
+RT_DEV typename Lane<T>::mask grid_splines(const Params<T>& P, T R, T Z, Gather& gather, GridVals<T>& V) {
+  typename Lane<T>::mask inside;
+  T dR, dZ, ds;
+  const typename Lane<T>::index cell = grid_psi_cell(P, R, Z, inside, dR, dZ);
+  if (gather.psi_request(P, cell)) gather.wait();
+  const T psi = grid_psi_eval<T, DISP>(P, cell, dR, dZ, gather, V);
+  const typename Lane<T>::index iP = grid_prof_cell(P, psi, inside, ds);
+  if (gather.prof_request(P, iP)) gather.wait();
+  grid_prof_eval<T, DISP>(P, iP, ds, gather, V);
+  return inside;
+}
 
 // How grid_full_rhs reaches the spline look-ups.  Normally the look-ups run in the caller's lane type.  The packed fp32 trace
 // kernel of the grid equilibrium (rt_kernels.cuh: trace_kernel_x2<EQ_GRID>) instead does them PER RAY in scalar arithmetic,
@@ -614,13 +644,25 @@ template <int DISP, class Pair>
 RT_DEV mask2 grid_values_per_ray(const Params<f32x2>& P, f32x2 R, f32x2 Z, Pair& gather, GridVals<f32x2>& V) {
   const Params<float>& Pf = P;
   GridVals<float> a, b;
-  mask2 in;
-  in.a = grid_splines<float, DISP>(Pf, R.lo(), Z.lo(), gather.a, a);
-  in.b = grid_splines<float, DISP>(Pf, R.hi(), Z.hi(), gather.b, b);
+  bool ina, inb;
+  float dRa, dZa, dRb, dZb, dsa, dsb;
+  // both rays' refills are in flight before the thread waits for either (a refill is a round trip to L2)
+  const int ca = grid_psi_cell(Pf, R.lo(), Z.lo(), ina, dRa, dZa), cb = grid_psi_cell(Pf, R.hi(), Z.hi(), inb, dRb, dZb);
+  gather.a.psi_request(Pf, ca); gather.b.psi_request(Pf, cb);
+  gather.a.wait();                 // unconditionally: a branch around it costs more than the empty wait (264 against 276 ms)
+  const float psia = grid_psi_eval<float, DISP>(Pf, ca, dRa, dZa, gather.a, a);
+  const int pa = grid_prof_cell(Pf, psia, ina, dsa);
+  gather.a.prof_request(Pf, pa);
+  const float psib = grid_psi_eval<float, DISP>(Pf, cb, dRb, dZb, gather.b, b);
+  const int pb = grid_prof_cell(Pf, psib, inb, dsb);
+  gather.b.prof_request(Pf, pb);
+  gather.b.wait();
+  grid_prof_eval<float, DISP>(Pf, pa, dsa, gather.a, a);
+  grid_prof_eval<float, DISP>(Pf, pb, dsb, gather.b, b);
   V.psiR = f32x2(a.psiR, b.psiR); V.psiZ = f32x2(a.psiZ, b.psiZ); V.psiRRh = f32x2(a.psiRRh, b.psiRRh);
   V.psiRZ = f32x2(a.psiRZ, b.psiRZ); V.psiZZh = f32x2(a.psiZZh, b.psiZZh);
   V.F = f32x2(a.F, b.F); V.Fp = f32x2(a.Fp, b.Fp); V.Ne = f32x2(a.Ne, b.Ne); V.Nep = f32x2(a.Nep, b.Nep);
-  return in;
+  return mask2{ina, inb};
 }
 #endif
 
@@ -793,8 +835,11 @@ RT_DEV typename Lane<T>::mask grid_full_rhs(const Params<T>& P, const T* y, T* f
   const T nZ = n[2];
   GridVals<T> V;
   typename Lane<T>::mask inside;
+#ifdef __CUDACC__
   if constexpr (gather_is_pair<Gather>::value) inside = grid_values_per_ray<DISP_FULL>(P, R, y[2], gather, V);
-  else inside = grid_values<T, DISP_FULL>(P, R, y[2], gather, V);
+  else
+#endif
+    inside = grid_values<T, DISP_FULL>(P, R, y[2], gather, V);
   const T X = P.xs * V.Ne, gx = P.xsh * V.Nep;
   const T iR2 = iR * iR;
   const T Q = rt_fma(V.F, V.F, rt_fma(V.psiR, V.psiR, V.psiZ * V.psiZ));
