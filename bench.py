@@ -49,18 +49,18 @@ UNIT = "ray-steps/s"
 # (its Newton refinement is NOT counted).  FP_INSTR_PER_RAY_STEP is what the FP64 / FP32 pipe actually issues per
 # ray-step (FMA, MUL, ADD, SETP instructions, refinements included).  Both tables are counted from the compiled kernels by
 # paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
-FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 247, (4, "f64"): 707, (5, "f64"): 1200,
-                      (1, "f32"): 117, (2, "f32"): 117, (3, "f32"): 250, (4, "f32"): 711, (5, "f32"): 1200}
-FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 197, (4, "f64"): 553, (5, "f64"): 820,
-                         (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 178, (4, "f32"): 484, (5, "f32"): 775}
+FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 243, (4, "f64"): 707, (5, "f64"): 1200,
+                      (1, "f32"): 117, (2, "f32"): 117, (3, "f32"): 246, (4, "f32"): 711, (5, "f32"): 1200}
+FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 193, (4, "f64"): 553, (5, "f64"): 820,
+                         (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 174, (4, "f32"): 484, (5, "f32"): 775}
 # FP_RF3_PER_RAY_STEP: how many of those instructions read THREE DISTINCT registers from the register file.  Such an instruction
 # occupies the FP64 pipe for 3 cycles instead of 2 (scalar FP32: 1.56 slots instead of 1; packed f32x2: 3 cycles instead of 2) -- measured by
 # rt_fma_peak_shape, shapes 2 / 6 (profiles/r1_fma_peak_shapes.md, r2_fma_peak_shapes.md) -- so the pipe time of a ray-step is
 # (instr + RF3_EXTRA * rf3) issue slots of the FMA microbenchmark; `pipe_model_frac` is that time over the measured kernel
 # time.  The fp32 kernels of the analytic equilibria (configs 1-4) are the packed two-rays-per-thread
 # kernels (trace_kernel_x2); their counts are per ray (a packed instruction = one slot per ray).
-FP_RF3_PER_RAY_STEP = {(1, "f64"): 27, (2, "f64"): 27, (3, "f64"): 42, (4, "f64"): 134, (5, "f64"): 312,
-                       (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 45, (4, "f32"): 143, (5, "f32"): 258}
+FP_RF3_PER_RAY_STEP = {(1, "f64"): 27, (2, "f64"): 27, (3, "f64"): 37, (4, "f64"): 134, (5, "f64"): 312,
+                       (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 42, (4, "f32"): 143, (5, "f32"): 258}
 RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1: 63.9 / 42.7, 123.2 / 78.8; packed 127.9 / 84.9
 PACKED = {(c, "f32") for c in (1, 2, 3, 4, 5)}           # (config, precision) pairs that run trace_kernel_x2
 # The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from
@@ -70,7 +70,7 @@ ORBIT_KERNEL = (2, "orbit")
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed `ncu --set full`
-# captures of this build: profiles/r2_cfg4_f64_ncu_f.md (headline), profiles/r2_other_configs_ncu_f.md (the others)
+# captures of this build: profiles/r2_cfg4_f64_ncu_g.md (headline), profiles/r2_other_configs_ncu_g.md (the others)
 NCU_DRAM_BYTES = {(4, "f64"): 5.988e9, (2, "f64"): 6.99e7, (2, "f32"): 2.53e7, (3, "f64"): 1.26e7, (4, "f32"): 2.963e9,
                   (5, "f64"): 1.826e9, (5, "f32"): 9.24e8, ("orbit4", "f64"): 5.98e9}
 

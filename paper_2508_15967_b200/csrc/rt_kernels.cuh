@@ -25,6 +25,8 @@ namespace rt {
 // does not spill (profiles/r1_tuning.md).  So the register cap (`__maxnreg__`) is simply the smallest one without spills
 // inside the step, with 64-thread blocks so that the register file divides evenly:
 //   fp64, analytic equilibria   120 registers -> 8 blocks = 16 warps per SM
+//   fp64, linear slab, O / X     72 registers -> 14 blocks = 28 warps per SM (the stage is a short chain through three
+//                                reciprocals: config 3 11.52 ms at 120 registers, 10.88 ms at 72; spills at 64)
 //   fp64, grid equilibrium      128 registers -> 8 blocks = 16 warps per SM (the profile pieces live in 16 of them)
 //   fp32                         72 registers -> 14 blocks = 28 warps per SM (the grid kernel's LDS latency likes warps:
 //                                321 ms at 72 registers, 344 ms at 128)
@@ -34,6 +36,11 @@ constexpr int AUX_BLOCK = 128;
 template <class T, int EQ> struct TraceShape { static constexpr int BLOCK = 64, MAXNREG = 72; };
 template <int EQ> struct TraceShape<double, EQ> { static constexpr int BLOCK = 64, MAXNREG = 120; };
 template <> struct TraceShape<double, EQ_GRID> { static constexpr int BLOCK = 64, MAXNREG = 128; };
+// register cap of trace_kernel<T, EQ, DISP>: the class's, except for the short O- / X-mode stages over the linear slab
+template <class T, int EQ, int DISP>
+constexpr int trace_maxnreg() {
+  return (sizeof(T) == 8 && EQ == EQ_LINEAR && DISP != DISP_FULL) ? 72 : TraceShape<T, EQ>::MAXNREG;
+}
 
 template <class T>
 struct TraceArgs {
@@ -292,7 +299,7 @@ struct RowStore {
 // RESUME: the chunk kernel of rt_trace_until -- each ray's status at entry comes from A.status_in (a separate
 // instantiation, so that the plain kernels' register allocation is untouched).
 template <class T, int EQ, int DISP, bool PW, bool RESUME = false>
-__global__ void __maxnreg__((TraceShape<T, EQ>::MAXNREG + (PW ? 16 : 0) + (RESUME ? 8 : 0)))
+__global__ void __maxnreg__((trace_maxnreg<T, EQ, DISP>() + (PW ? 16 : 0) + (RESUME ? 8 : 0)))
 trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ TraceArgs<T> A) {
   constexpr int BLOCK = TraceShape<T, EQ>::BLOCK;
   const long long N = A.n_rays;

@@ -394,7 +394,7 @@ RT_DEV void disp_partials(const Params<T>& P, T X, T Y2, T u, T v, T& DX, T& DY2
 template <class T>
 struct Coef {
   T A, C, Ax, Ab, r;
-  T YD;                              // Y2 DYn (full determinant only)
+  T YD;                              // Y2 DYn
   typename Lane<T>::mask fast;       // SERIES: Y2 < Params::y2cap, i.e. the series of the ion terms is exact to rounding here
 };
 
@@ -438,7 +438,8 @@ RT_DEV Coef<T> disp_coefs(const Params<T>& P, T X, T b2, T G, T v) {
     const T DS = rt_fma(T(-2), S, v);
     const T DXn = rt_fma(sig, DS, -q1);
     const T DYn = rt_fma(Xsp, DS, -q2);
-    const T s = rt_fma(v, S, -rt_fma(Y2, DYn, X * DXn));
+    c.YD = Y2 * DYn;
+    const T s = rt_fma(v, S, -rt_fma(X, DXn, c.YD));
     c.r = rt_rcp(s);
     c.A = S;
     c.C = T(0);
@@ -481,6 +482,7 @@ template <class T>
 struct Local {
   T X, hgX[3];   // X and HALF its gradient
   T B[3], b2, hgb2[3], G, gG[3];
+  T ix;          // linear slab: 1/x
   T nl[3];       // n in the local frame
   T cph, sph;    // axisymmetric kinds: e1 = (cph, sph, 0), e2 = (-sph, cph, 0)
 };
@@ -680,6 +682,7 @@ RT_DEV typename Lane<T>::mask equilibrium(const Params<T>& P, const T* x, const 
     L.X = (x[0] - P.x_foot) * P.lin_gx;                                    // grad X = (lin_gx, 0, 0)
     if (DISP != DISP_O) {
       const T ix = rt_rcp(x[0]);
+      L.ix = ix;
       const T Bz = (SC ? P.sB0R0 : P.B0R0) * ix;
       L.B[2] = Bz;
       L.b2 = Bz * Bz;
@@ -916,12 +919,10 @@ RT_DEV typename Lane<T>::mask ray_rhs(const Params<T>& P, const T* y, T* f, T& r
     fast = rt_and(fast, c.fast);
     f[0] = c.A * n[0]; f[1] = c.A * n[1]; f[2] = c.A * n[2];               // A n is frame-independent
     if (EQ == EQ_LINEAR) {
-      T fn = rt_fma(c.Ab, L.hgb2[0], c.Ax * P.lin_gxh);
-      if (DISP == DISP_FULL) {
-        f[2] = rt_fma(c.C, L.B[2], f[2]);
-        fn = rt_fma(-c.C, L.gG[0], fn);
-      }
-      f[3] = fn; f[4] = T(0); f[5] = T(0);
+      // B = (c/x) z^:  (1/2) d|B'|^2/dx = -Y2/x and d(n.B')/dx = -(n.B')/x, so the curvature terms collapse as in
+      // tokamak_full_rhs:  Ab (1/2) dY2/dx - C d(n.B')/dx = -(Ab Y2 - C (n.B'))/x = -Y2 DYn / x
+      if (DISP == DISP_FULL) f[2] = rt_fma(c.C, L.B[2], f[2]);
+      f[3] = rt_fma(-c.YD, L.ix, c.Ax * P.lin_gxh); f[4] = T(0); f[5] = T(0);
       return inside;
     }
     // axisymmetric kinds: assemble in (R^, phi^, Z^), rotate to Cartesian
