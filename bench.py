@@ -60,7 +60,7 @@ FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 193, (4, "f
 # time.  The fp32 kernels of the analytic equilibria (configs 1-4) are the packed two-rays-per-thread
 # kernels (trace_kernel_x2); their counts are per ray (a packed instruction = one slot per ray).
 FP_RF3_PER_RAY_STEP = {(1, "f64"): 27, (2, "f64"): 27, (3, "f64"): 37, (4, "f64"): 134, (5, "f64"): 312,
-                       (1, "f32"): 33, (2, "f32"): 33, (3, "f32"): 42, (4, "f32"): 143, (5, "f32"): 258}
+                       (1, "f32"): 32, (2, "f32"): 32, (3, "f32"): 42, (4, "f32"): 143, (5, "f32"): 258}
 RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1: 63.9 / 42.7, 123.2 / 78.8; packed 127.9 / 84.9
 PACKED = {(c, "f32") for c in (1, 2, 3, 4, 5)}           # (config, precision) pairs that run trace_kernel_x2
 # The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from

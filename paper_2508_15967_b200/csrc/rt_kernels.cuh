@@ -390,6 +390,9 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
 // (16 warps per SM instead of 28) and the kernel, which is bound by the LDS data pipe and the latency of the look-up
 // chain rather than by issue slots, runs 2-3 % slower than trace_kernel<float, EQ_GRID, ...>.
 template <int EQ> struct TraceShape2 { static constexpr int BLOCK = 64, MAXNREG = 128; };
+// the slabs' short stages like more warps (config 2 fp32 6.00 -> 5.86 ms at 80 registers, config 3 fp32 4.90 -> 4.76 ms at 96)
+template <> struct TraceShape2<EQ_PARABOLIC> { static constexpr int BLOCK = 64, MAXNREG = 80; };
+template <> struct TraceShape2<EQ_LINEAR> { static constexpr int BLOCK = 64, MAXNREG = 96; };
 
 template <int EQ, int DISP>
 __global__ void __maxnreg__((TraceShape2<EQ>::MAXNREG))
