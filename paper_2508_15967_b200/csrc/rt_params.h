@@ -24,7 +24,7 @@ constexpr double kEps0 = 8.8541878188e-12;  // F/m
 //   del' = mu^4 e2^2 - e1^2 -> mu^4 - e1^2                  dropped: mu^4 (2z - z^2)/(1-z)^2
 // stays below `tol` (a quarter ulp of the working precision) relative to the smallest magnitude the electron term
 // e1 = 1/(1 - Y2) (resp. e1^2) takes on [0, Y2]: 1/max(1, Y2 - 1).  The bounds grow with Y2, so bisection finds the cap.
-// Deuterium, fp64: Y2 < 3.6 (w > 0.53 W_ce); electrons only (mu = 0): no limit.
+// Deuterium, fp64: Y2 < 3.3 (w > 0.55 W_ce); electrons only (mu = 0): no limit.
 inline double series_cap(double mu, double tol) {
   if (!(mu > 0.0)) return 1.7e308;
   auto ok = [&](double Y2) {

@@ -30,6 +30,9 @@ int shim_fit_bicubic(const double* R, const double* Z, const double* f, int nR, 
   return (int)out.size();
 }
 
+// the largest Y2 up to which the hot loop evaluates the ion terms of the Stix elements by their series (rt_params.h)
+double shim_series_cap(double mu, double tol) { return rt::series_cap(mu, tol); }
+
 void shim_fold_params(const rt_equilibrium_desc* d, double rho_max, double omega, int fp32, double* out) {
   if (fp32) fold_to<float>(d, rho_max, omega, out); else fold_to<double>(d, rho_max, omega, out);
 }

@@ -302,6 +302,68 @@ def test_stage_rhs_at_parallel_propagation(rt, oracle, where, prec):
     eq.close()
 
 
+# --------------------------------------------------------------------------------- ion terms: series and exact elements
+M_E = 9.1093837139e-31
+
+
+@pytest.fixture(scope="module")
+def series_cap(tmp_path_factory):
+    """rt_params.h: series_cap through the CPU shim -- the Y2 below which the kernels take the ion terms from their series."""
+    from helpers import build_host_shim
+    lib = build_host_shim(tmp_path_factory.mktemp("shim"))
+    return lambda mu, prec: lib.shim_series_cap(mu, 2.0**-54 if prec == "f64" else 2.0**-25)
+
+
+@pytest.mark.parametrize("cfg,prec,mass,regime", [
+    (4, "f64", 1500.0, "crossing"), (4, "f64", 935.0, "exact"), (4, "f32", 27.0, "crossing"), (4, "f32", 16.8, "exact"),
+    (5, "f64", 1500.0, "crossing"), (5, "f32", 27.0, "crossing"), (5, "f32", 16.8, "exact"),
+    (3, "f64", 1780.0, "crossing"), (3, "f64", 935.0, "exact"), (3, "f32", 32.0, "crossing")])
+def test_ion_terms_by_series_and_exactly(rt, oracle, series_cap, cfg, prec, mass, regime):
+    """The step loop evaluates the ion terms of the Stix elements by their series while every stage has Y2 below a cap
+    folded on the host, and repeats a step with the exact elements (second step loop) otherwise.
+    BASELINE's configs (deuterium) never leave the fast loop, so the switch is driven here by a lighter ion species
+    (`mass` electron masses), chosen so that the cap lies INSIDE the range of Y2 the rays see ("crossing": they start in
+    the fast loop and change to the exact one on the way -- and try the fast loop again at every sample) or BELOW it
+    ("exact": the second loop from the first step).  Either way the result is the oracle's, which knows no series."""
+    # config 3 is an fp64 workload in BASELINE.json; in fp32 its 3000 steps toward a cut-off end 1.6e-4 from the oracle with ANY
+    # ion mass (the per-call constants rounded to fp32 are a relative 6e-8 change of the problem, which the turn amplifies), so
+    # the fp32 case stops at 900 steps, before the turn and after the switch
+    n_steps = {3: 3000 if prec == "f64" else 900, 4: 1000, 5: 500}[cfg]
+    w = inputs.config(cfg, n_rays=128 * 3 + 9, n_steps=n_steps)
+    w.eq = dict(w.eq, ion_mass=mass * M_E, ion_charge=1.0)
+    oeq = oracle.Equilibrium(w.eq)
+    k0, _ = oracle.launch(oeq, w.disp, w.x0, w.dirs, w.omega, w.branch)
+    assert np.isfinite(k0).all()
+    stride = n_steps // 10
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, w.omega, n_steps, w.dt, stride, traj=True)
+    assert (ref["status"] == 0).all()
+    # Y2 = (W_ce / w)^2 along the oracle's rays against the cap of this species and precision
+    tr = ref["traj"]
+    Y2 = np.stack([oracle.diagnostics(oeq, tr[m, :3], tr[m, 3:], w.omega)[3] ** 2 for m in range(tr.shape[0])])
+    cap = series_cap(M_E / (mass * M_E), prec)
+    if regime == "crossing":
+        starts_fast = Y2[0] < 0.98 * cap
+        ends_exact = Y2.max(axis=0) > 1.02 * cap
+        assert starts_fast.mean() > 0.9 and (starts_fast & ends_exact).mean() > 0.25, (cap, Y2[0].min(), Y2.max())
+    else:
+        assert (Y2[0] > 1.5 * cap).all()
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, w.disp, _dev(w.x0, prec), _dev(k0, prec), w.omega, n_steps, w.dt, stride, traj=True)
+    got = _host(out["traj"])
+    for m in range(got.shape[0]):
+        ex, ek = rel_err_xk(got[m], tr[m])
+        assert ex < TOL[prec] and ek < TOL[prec], (cfg, prec, mass, m, ex, ek)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    # one stage on both sides of the cap (rt_rhs switches per point)
+    m = got.shape[0] // 2
+    f_ref = _rhs_ref(oracle, oeq, w.disp, tr[m, :3], tr[m, 3:], w.omega)[0]
+    f = _host(rt.rhs(eq, w.disp, _dev(tr[m, :3], prec), _dev(tr[m, 3:], prec), w.omega)[1])
+    for sl in (slice(0, 3), slice(3, 6)):
+        err = np.linalg.norm(f[sl] - f_ref[sl], axis=0) / np.linalg.norm(f_ref[sl], axis=0)
+        assert err.max() < (1e-11 if prec == "f64" else 2e-4), (cfg, prec, mass, err.max())
+    eq.close()
+
+
 # --------------------------------------------------------------------------------- full sizes, sampled rays
 @pytest.mark.parametrize("cfg,prec", [(2, "f64"), (2, "f32"), (3, "f64"), (4, "f64"), (5, "f64"), (5, "f32")])
 def test_full_size_sampled_parity(rt, oracle, cfg, prec):

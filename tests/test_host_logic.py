@@ -18,15 +18,8 @@ CSRC = HERE.parent / "paper_2508_15967_b200" / "csrc"
 
 @pytest.fixture(scope="module")
 def shim(tmp_path_factory):
-    so = tmp_path_factory.mktemp("spline") / "libspline_shim.so"
-    subprocess.run(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", str(HERE / "host_shim.cpp"),
-                    str(CSRC / "spline_fit.cpp"), "-o", str(so)], check=True)
-    lib = ctypes.CDLL(str(so))
-    P = ctypes.c_void_p
-    lib.shim_fit_cubic.argtypes = [P, P, ctypes.c_long, ctypes.c_int, P]
-    lib.shim_fit_bicubic.argtypes = [P, P, P, ctypes.c_int, ctypes.c_int, P]
-    lib.shim_fold_params.argtypes = [P, ctypes.c_double, ctypes.c_double, ctypes.c_int, P]
-    return lib
+    from helpers import build_host_shim
+    return build_host_shim(tmp_path_factory.mktemp("spline"))
 
 
 def _fit1(lib, x, y, stride=1):
@@ -140,3 +133,41 @@ def test_constant_folding_matches_the_definitions(shim, fp32):
     desc, keep = binding.make_desc(w1.eq)
     shim.shim_fold_params(ctypes.addressof(desc), 0.98, w1.omega, fp32, out.ctypes.data)
     assert out[0] == pytest.approx(0.5, rel=rtol) and out[9] == pytest.approx(0.5 / 1.0**2, rel=rtol)    # X = 1/2 (1 + r^2/L^2)
+
+
+@pytest.mark.parametrize("tol", [2.0**-54, 2.0**-25])
+@pytest.mark.parametrize("mu", [1 / 3670.48, 1 / 1836.15, 1 / 935.0, 1e-2, 0.0596, 0.3])
+def test_series_cap_bounds_the_dropped_ion_terms(shim, mu, tol):
+    """The hot loop replaces the ion terms of the Stix elements (Eq. 8-9) by their series in z = mu^2 Y2 for
+    Y2 below a host-folded cap (rt_params.h: series_cap).  With 40-digit arithmetic: below the cap each of the four sums
+    sig, sig', del, del' differs from its exact value by at most `tol` (a quarter ulp of the working precision) relative
+    to the electron term it is added to, whatever that term's size on [0, cap] (its smallest magnitude is what the cap
+    is folded against); and the cap is maximal: 2 % above it one of the bounds fails."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    cap = shim.shim_series_cap(mu, tol)
+    assert cap > 0 and np.isfinite(cap)
+    m = mp.mpf(mu)
+
+    def worst(Y2):
+        Y2 = mp.mpf(Y2)
+        z = m * m * Y2
+        e2 = 1 / (1 - z)
+        # exact ion parts and their series (disp_coefs, SERIES)
+        pairs = [(m * e2, m + m**3 * Y2, 1), (m**3 * e2**2, m**3, 2), (m * m * e2, m * m + m**4 * Y2, 1), (m**4 * e2**2, m**4, 2)]
+        # smallest magnitude of the electron term e1 = 1 / (1 - Y2) (power p) over [0, Y2]: 1 / max(1, Y2 - 1)^p
+        floor = 1 / max(mp.mpf(1), Y2 - 1)
+        return max(abs(ex - se) / floor**p for ex, se, p in pairs)
+
+    for f in (1e-3, 0.1, 0.5, 0.9, 0.999):
+        assert worst(f * cap) <= tol, (mu, tol, f)
+    assert worst(1.02 * cap) > tol
+    assert mu * mu * cap < 0.5
+
+
+def test_series_cap_without_ions_and_for_deuterium(shim):
+    """Electrons only: the series is exact, no limit.  Deuterium in fp64: Y2 < 3.3, i.e. every frequency above 0.55 of the
+    electron cyclotron frequency runs the fast loop."""
+    assert shim.shim_series_cap(0.0, 2.0**-54) > 1e300
+    cap = shim.shim_series_cap(1 / 3670.48, 2.0**-54)
+    assert 3.2 < cap < 3.5
