@@ -51,6 +51,10 @@ UNIT = "ray-steps/s"
 # paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
 FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 243, (4, "f64"): 707, (5, "f64"): 1200,
                       (1, "f32"): 117, (2, "f32"): 117, (3, "f32"): 246, (4, "f32"): 711, (5, "f32"): 1200}
+# FLOPS_EXECUTED_PER_RAY_STEP: flops as the kernel executes them (2 per fused multiply-add, 1 per multiply / add, Newton
+# refinements included) -- SURVEY.md section 8(d)'s own numerator, what ncu's op_dfma / op_dmul / op_dadd counters add up to.
+FLOPS_EXECUTED_PER_RAY_STEP = {(1, "f64"): 135, (2, "f64"): 135, (3, "f64"): 303, (4, "f64"): 843, (5, "f64"): 1288,
+                               (1, "f32"): 113, (2, "f32"): 113, (3, "f32"): 234, (4, "f32"): 687, (5, "f32"): 1184}
 FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 193, (4, "f64"): 553, (5, "f64"): 820,
                          (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 174, (4, "f32"): 484, (5, "f32"): 775}
 # FP_RF3_PER_RAY_STEP: how many of those instructions read THREE DISTINCT registers from the register file.  Such an instruction
@@ -65,14 +69,14 @@ RF3_EXTRA = {"f64": 0.5, "f32": 0.563, "f32x2": 0.507}   # shape 0 / shape 2 - 1
 PACKED = {(c, "f32") for c in (1, 2, 3, 4, 5)}           # (config, precision) pairs that run trace_kernel_x2
 # The second ensemble workload (rt_orbit on config 4's tokamak): the same three counts per PARTICLE-step, from
 # sass_count.py's orbit_kernel rows (pinned by the same test).
-ORBIT_COUNTS = {"f64": dict(flops=238, instr=184, rf3=50), "f32": dict(flops=238, instr=162, rf3=50)}
+ORBIT_COUNTS = {"f64": dict(flops=238, instr=184, rf3=50, executed=286), "f32": dict(flops=238, instr=162, rf3=50, executed=230)}
 ORBIT_KERNEL = (2, "orbit")
 # (equilibrium kind, dispersion kind) of rt_math.cuh behind each config: the key sass_count.py reports under
 KERNEL_OF_CONFIG = {1: (0, 0), 2: (0, 0), 3: (1, 1), 4: (2, 2), 5: (3, 2)}
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed `ncu --set full`
 # captures of this build: profiles/r2_cfg4_f64_ncu_g.md (headline), profiles/r2_other_configs_ncu_g.md (the others)
-NCU_DRAM_BYTES = {(4, "f64"): 5.988e9, (2, "f64"): 6.99e7, (2, "f32"): 2.53e7, (3, "f64"): 1.26e7, (4, "f32"): 2.963e9,
-                  (5, "f64"): 1.826e9, (5, "f32"): 9.24e8, ("orbit4", "f64"): 5.98e9}
+NCU_DRAM_BYTES = {(4, "f64"): 5.986e9, (2, "f64"): 6.64e7, (2, "f32"): 2.55e7, (3, "f64"): 1.26e7, (4, "f32"): 2.964e9,
+                  (5, "f64"): 1.832e9, (5, "f32"): 9.14e8, ("orbit4", "f64"): 5.976e9}
 
 WORKLOAD_NAMES = {
     1: "cfg1: O-mode, parabolic slab, 1024 rays x 1000 steps, full trajectory",
@@ -348,11 +352,18 @@ def time_steps(torch, job: Job, steps: int, warmup: int, flush, barrier=None):
 
 
 def fractions(counts: dict, units: float, kernel_ms: float, fma_rate: float, flavour: str) -> dict:
-    """The three fractions of DESIGN.md section 6 for one kernel launch of `units` ray-steps (particle-steps);
-    flavour = 'f64' | 'f32' | 'f32x2' selects the cost of a three-register instruction."""
+    """The fractions of DESIGN.md section 6 for one kernel launch of `units` ray-steps (particle-steps);
+    flavour = 'f64' | 'f32' | 'f32x2' selects the cost of a three-register instruction.
+    roofline_frac  algorithmic flops (a division or square root = 1) against 2 x the FMA rate -- the strict figure;
+    frac_executed  flops as executed against the same peak (SURVEY.md section 8(d)'s formula; what ncu's counters give);
+    frac_ceiling   the largest roofline_frac THIS instruction stream allows: flops / (2 x pipe slots), a multiply or add
+                   filling half of its slot, a three-register instruction taking a slot and a half;
+    pipe_frac, pipe_model_frac  pipe slots issued (plain / with the three-register cost) against the FMA rate."""
     per_s = units / (kernel_ms * 1e-3)
-    return {"roofline_frac": counts["flops"] * per_s / (2.0 * fma_rate), "pipe_frac": counts["instr"] * per_s / fma_rate,
-            "pipe_model_frac": (counts["instr"] + RF3_EXTRA[flavour] * counts["rf3"]) * per_s / fma_rate}
+    slots = counts["instr"] + RF3_EXTRA[flavour] * counts["rf3"]
+    return {"roofline_frac": counts["flops"] * per_s / (2.0 * fma_rate),
+            "frac_executed": counts["executed"] * per_s / (2.0 * fma_rate), "frac_ceiling": counts["flops"] / (2.0 * slots),
+            "pipe_frac": counts["instr"] * per_s / fma_rate, "pipe_model_frac": slots * per_s / fma_rate}
 
 
 def flavour(cfg: int, prec: str) -> str:
@@ -430,7 +441,7 @@ def run_ours(args) -> int:
         del x0h, k0h, hout
 
     counts = {"flops": FLOPS_PER_RAY_STEP[(cfg, prec)], "instr": FP_INSTR_PER_RAY_STEP[(cfg, prec)],
-              "rf3": FP_RF3_PER_RAY_STEP[(cfg, prec)]}
+              "rf3": FP_RF3_PER_RAY_STEP[(cfg, prec)], "executed": FLOPS_EXECUTED_PER_RAY_STEP[(cfg, prec)]}
     fr = fractions(counts, job.ray_steps, kernel_ms, peak_after, flavour(cfg, prec))
     launch_residual = job.launch_residual
     peak = 2.0 * peak_after
@@ -439,7 +450,9 @@ def run_ours(args) -> int:
                 "kernel": "rt::trace_kernel_x2 (packed f32x2, two rays per thread)" if (cfg, prec) in PACKED
                 else f"rt::trace_kernel<{'double' if prec == 'f64' else 'float'}>",
                 "kernel_ms": kernel_ms, "flops_per_ray_step": counts["flops"], "fp_instr_per_ray_step": counts["instr"],
-                "fp_rf3_per_ray_step": counts["rf3"], "pipe_frac": fr["pipe_frac"], "pipe_model_frac": fr["pipe_model_frac"],
+                "fp_rf3_per_ray_step": counts["rf3"], "flops_executed_per_ray_step": counts["executed"],
+                "frac_executed": fr["frac_executed"], "frac_ceiling": fr["frac_ceiling"],
+                "pipe_frac": fr["pipe_frac"], "pipe_model_frac": fr["pipe_model_frac"],
                 "peak_source": f"rt_fma_peak({prec}) measured in this process after the timed region: "
                                f"{peak_after / 1e12:.3f} T{'D' if prec == 'f64' else 'F'}FMA/s at {peak_mhz:.0f} MHz "
                                f"(before: {peak_before / 1e12:.3f})"}
@@ -456,7 +469,8 @@ def run_ours(args) -> int:
             j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 1000 + c, scan=scan)
             _, kms = time_steps(torch, j, 3, 1, flush)
             pk, _ = rt.fma_peak(p, 100.0)
-            cn = {"flops": FLOPS_PER_RAY_STEP[(c, p)], "instr": FP_INSTR_PER_RAY_STEP[(c, p)], "rf3": FP_RF3_PER_RAY_STEP[(c, p)]}
+            cn = {"flops": FLOPS_PER_RAY_STEP[(c, p)], "instr": FP_INSTR_PER_RAY_STEP[(c, p)], "rf3": FP_RF3_PER_RAY_STEP[(c, p)],
+                  "executed": FLOPS_EXECUTED_PER_RAY_STEP[(c, p)]}
             extra.append({"workload": f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else ""),
                           "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
                           "traffic": NCU_DRAM_BYTES.get((c, p)) if not scan else None,
