@@ -28,8 +28,8 @@ namespace rt {
 //   fp64, linear slab, O / X     72 registers -> 14 blocks = 28 warps per SM (the stage is a short chain through three
 //                                reciprocals: config 3 11.52 ms at 120 registers, 10.88 ms at 72; spills at 64)
 //   fp64, grid equilibrium      128 registers -> 8 blocks = 16 warps per SM (the profile pieces live in 16 of them)
-//   fp32                         72 registers -> 14 blocks = 28 warps per SM (the grid kernel's LDS latency likes warps:
-//                                321 ms at 72 registers, 344 ms at 128)
+//   fp32, scalar kernels         72 registers -> 14 blocks = 28 warps per SM (the grid kernel's LDS latency likes warps:
+//                                321 ms at 72 registers, 344 ms at 128); the packed fp32 kernels: TraceShape2 below
 // The grid equilibrium keeps ONE copy of the stage code (stage loop not unrolled: unrolled it needs >= 168 registers and
 // is slower at every cap, profiles/r1_tuning.md).  The diagnostic kernels (rhs, launch, diag) use plain 128-thread blocks.
 constexpr int AUX_BLOCK = 128;
@@ -385,10 +385,11 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
 // the two kernels give bit-identical rays; what changes is the instruction stream: one FFMA2 / FMUL2 / FADD2 issue slot
 // serves two rays, and MUFU seeds, domain tests and table look-ups are done per half.  A lane whose ray is frozen keeps
 // computing on its frozen state and is masked out of every update.
-// The packed kernels exist for the analytic equilibria.  For the grid equilibrium the same approach was measured and
-// dropped (profiles/r2_tuning.md): with two rays per thread the per-ray shared-memory cell cache needs 128 registers
-// (16 warps per SM instead of 28) and the kernel, which is bound by the LDS data pipe and the latency of the look-up
-// chain rather than by issue slots, runs 2-3 % slower than trace_kernel<float, EQ_GRID, ...>.
+// The packed kernels exist for every dispersion function over the analytic equilibria and for the full determinant over the
+// grid equilibrium.  Over the grid the spline look-ups are NOT packed (rt_math.cuh: grid_values_per_ray): each ray of the
+// thread has its own scalar shared-memory cell cache and its look-ups run in scalar arithmetic, the nine results are packed
+// and everything after them runs packed -- fully packed look-ups were measured and dropped (profiles/r2_tuning.md: pairing
+// every spline piece with the other ray's costs ~100 register moves per stage).
 template <int EQ> struct TraceShape2 { static constexpr int BLOCK = 64, MAXNREG = 128; };
 // the slabs' short stages like more warps (config 2 fp32 6.00 -> 5.86 ms at 80 registers, config 3 fp32 4.90 -> 4.76 ms at 96)
 template <> struct TraceShape2<EQ_PARABOLIC> { static constexpr int BLOCK = 64, MAXNREG = 80; };

@@ -246,7 +246,7 @@ struct GatherDirect {
   template <class T> RT_DEV void prof_row(const Params<T>& P, int cell, int which, T* c) const { ld4(P.prof_pp + (size_t)cell * 8 + 4 * which, c); }
 #ifdef __CUDACC__
   // per-half look-ups of the packed type (the grid branch of equilibrium<> has to compile for every T; the packed trace
-  // kernels themselves are instantiated for the analytic equilibria only)
+  // kernel of the grid equilibrium does its look-ups per ray in scalar arithmetic instead: grid_values_per_ray)
   RT_DEV void psi_row(const Params<f32x2>& P, int2v cell, int p, f32x2* c) const {
     float a[4], b[4];
     ld4(P.psi_pp + (size_t)cell.a * 16 + 4 * p, a); ld4(P.psi_pp + (size_t)cell.b * 16 + 4 * p, b);

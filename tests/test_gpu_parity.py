@@ -364,6 +364,29 @@ def test_ion_terms_by_series_and_exactly(rt, oracle, series_cap, cfg, prec, mass
     eq.close()
 
 
+@pytest.mark.parametrize("cfg,disp", [(1, "omode"), (3, "omode"), (4, "omode"), (5, "omode")])
+def test_omode_rays_off_the_dispersion_surface(rt, oracle, cfg, disp):
+    """Reading A4: the full D is differentiated (O-mode: W = -2 (v + X) = -2 (1 + D), not -2), so launch states off the
+    dispersion surface are legitimate input and must follow the oracle exactly as on-shell ones do.  Wave vectors pushed off
+    D = 0 by relative 1e-11 ... 1e-2, mixed with on-shell rays inside every warp, on every equilibrium."""
+    w, oeq, k0 = _workload(oracle, cfg, 128 * 2 + 37, 400, disp)
+    rng = np.random.default_rng(77)
+    scale = 1.0 + rng.choice([0.0, 1e-11, 1e-9, 1e-8, 1e-6, 1e-3, 1e-2], size=k0.shape[1]) * rng.choice([-1.0, 1.0], size=k0.shape[1])
+    k0 = k0 * scale
+    D0 = np.abs(oracle.dispersion_value(oeq, disp, w.x0, k0, w.omega))
+    assert (D0 < 2.0**-30).sum() > 50 and (D0 > 2.0**-26).sum() > 50          # on-shell and clearly off-shell rays, both present
+    ref = oracle.trace(oeq, disp, w.x0, k0, w.omega, 400, w.dt, 100, traj=True)
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, disp, _dev(w.x0), _dev(k0), w.omega, 400, w.dt, 100, traj=True)
+    got = _host(out["traj"])
+    for m in range(got.shape[0]):
+        ex, ek = rel_err_xk(got[m], ref["traj"][m])
+        assert ex < 1e-10 and ek < 1e-10, (cfg, m, ex, ek)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    _check_residual(oracle, oeq, w, got, _host(out["residual"]), ref["residual"], "f64")
+    eq.close()
+
+
 # --------------------------------------------------------------------------------- full sizes, sampled rays
 @pytest.mark.parametrize("cfg,prec", [(2, "f64"), (2, "f32"), (3, "f64"), (4, "f64"), (5, "f64"), (5, "f32")])
 def test_full_size_sampled_parity(rt, oracle, cfg, prec):
