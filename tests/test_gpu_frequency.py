@@ -227,3 +227,36 @@ def test_store_paths_at_ragged_sizes(rt, oracle, n_rays, prec):
     np.testing.assert_array_equal(_host(out2["final"]), tr[-1])
     np.testing.assert_array_equal(_host(out2["residual"]), _host(out["residual"])[-1])
     eq.close()
+
+
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_low_frequency_scan_straddles_the_ion_series_range(rt, oracle, cfg):
+    """Deuterium plasma of configs 4 / 5 at 20-28 GHz, one frequency per ray, second root of the biquadratic: Y2 = (W_ce / w)^2
+    at launch runs from 2.3 to 4.7, on both sides of the 3.35 below which the fp64 kernels take the ion terms of the Stix elements
+    from their series (rt_params.h: series_cap).  Inside one warp some rays stay in the fast step loop, some
+    are in the exact one from the first step and some change over on the way in -- all must follow the oracle."""
+    n_rays, n_steps, stride = 64 * 5 + 37, 400, 100
+    w = inputs.config(cfg, n_rays=n_rays, n_steps=n_steps)
+    om = 2 * np.pi * np.random.default_rng(4242).uniform(20e9, 28e9, n_rays)
+    oeq = oracle.Equilibrium(w.eq)
+    k0, D0 = oracle.launch(oeq, w.disp, w.x0, w.dirs, om, 1)
+    assert np.isfinite(k0).all() and np.abs(D0).max() < 2e-15
+    ref = oracle.trace(oeq, w.disp, w.x0, k0, om, n_steps, w.dt, stride, traj=True)
+    assert (ref["status"] == 0).all()
+    Y2 = np.stack([oracle.diagnostics(oeq, ref["traj"][m, :3], ref["traj"][m, 3:], om)[3] ** 2 for m in range(ref["traj"].shape[0])])
+    assert (Y2.max(axis=0) < 3.3).mean() > 0.2 and (Y2[0] > 3.4).mean() > 0.2 and ((Y2[0] < 3.3) & (Y2.max(axis=0) > 3.4)).mean() > 0.1
+    eq = rt.create_equilibrium(w.eq)
+    out = rt.trace(eq, w.disp, _dev(w.x0), _dev(k0), _dev(om), n_steps, w.dt, stride, traj=True)
+    tr = _host(out["traj"])
+    for m in range(tr.shape[0]):
+        ex, ek = rel_err_xk(tr[m], ref["traj"][m])
+        assert ex < 1e-10 and ek < 1e-10, (cfg, m, ex, ek)
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    # the scalar-frequency kernel on the rays of one frequency bin, wholly beyond the range (every step in the exact loop)
+    sel = np.argsort(om)[:64]
+    k0s, _ = oracle.launch(oeq, w.disp, w.x0[:, sel], w.dirs[:, sel], om[sel[0]], 1)
+    refs = oracle.trace(oeq, w.disp, w.x0[:, sel], k0s, om[sel[0]], n_steps, w.dt)
+    outs = rt.trace(eq, w.disp, _dev(w.x0[:, sel]), _dev(k0s), float(om[sel[0]]), n_steps, w.dt)
+    ex, ek = rel_err_xk(_host(outs["final"]), refs["final"])
+    assert ex < 1e-10 and ek < 1e-10 and np.array_equal(_host(outs["status"]), refs["status"]), (ex, ek)
+    eq.close()
