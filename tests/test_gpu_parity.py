@@ -388,7 +388,7 @@ def test_omode_rays_off_the_dispersion_surface(rt, oracle, cfg, disp):
 
 
 # --------------------------------------------------------------------------------- full sizes, sampled rays
-@pytest.mark.parametrize("cfg,prec", [(2, "f64"), (2, "f32"), (3, "f64"), (4, "f64"), (5, "f64"), (5, "f32")])
+@pytest.mark.parametrize("cfg,prec", [(2, "f64"), (2, "f32"), (3, "f64"), (4, "f64"), (4, "f32"), (5, "f64"), (5, "f32")])
 def test_full_size_sampled_parity(rt, oracle, cfg, prec):
     """BASELINE.json's full sizes in the launch configuration bench.py times (one rt_trace call over the whole ensemble,
     launch states from rt_launch, the config's output mode); 192 sampled rays are checked one by one against the oracle.
