@@ -119,6 +119,43 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
                   int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj, void* out_final,
                   void* out_residual, int32_t* out_status);
 
+/* rt_trace_host for callers that must not allocate device memory when they call the library.  rt_trace_host stages the
+ * rays and their results in device buffers it gets from cudaMalloc (and creates two streams on first use).  Some host
+ * programs cannot afford that:
+ *   - a code that took all of the GPU's memory into its own pool at start-up (a simulation with a fixed arena, an ML
+ *     framework's caching allocator): a cudaMalloc made behind its back fails, or succeeds only until the pool grows;
+ *   - a code with a latency budget (a control loop around the ray tracer, a service with other streams in flight):
+ *     cudaMalloc and cudaFree stall the whole device for a time nobody bounds;
+ *   - a job whose device memory is accounted for once, before the run (a fixed slice of a shared GPU).
+ * This entry point therefore takes its staging space from ONE array of RT_NOALLOC_SCRATCH_BYTES (64 MiB) that is part of
+ * the library image: every GPU on which the process uses the library holds those 64 MiB from the moment the library's
+ * code is loaded there until the process exits, whether or not this function is ever called.  The call itself makes no
+ * cudaMalloc / cudaFree, creates no stream or event, and calls no routine that allocates.
+ *
+ * Arguments and results are those of rt_trace_host (HOST buffers, pageable or pinned; the same kernels, so the same
+ * bits), plus
+ *   cuda_stream   the stream the two copies in, the kernel and the copies out are enqueued on (NULL: the default
+ *                 stream); the call waits for that stream before it returns, so the results are in host memory then.
+ * The whole call has to fit in the array at once -- there is no chunking here: with es = 8 (fp64) or 4 (fp32) bytes and
+ * every section rounded up to 256 bytes,
+ *   6 n_rays es  +  [out_traj] 6 n_saved n_rays es  +  [out_final] 6 n_rays es  +  [out_residual] n_res n_rays es
+ *                +  [out_status] 4 n_rays   <=  RT_NOALLOC_SCRATCH_BYTES
+ * (config 1 of BASELINE.json, 1024 rays with all 1001 samples in fp64, takes 55 MiB; final states only: 2^19 rays in
+ * fp64).  A larger call is refused with RT_ERR_INVALID and a message that states both byte counts; nothing is enqueued.
+ *
+ * First call on a device: the library looks up the array's device address there (cudaGetSymbolAddress, with that device
+ * current) and keeps it; this may make the CUDA runtime load the library's code onto the device.  Make that first call
+ * outside any stream capture, before the part of the program that must not stall.
+ * The array is shared by every call made on that device in this process and still holds what the previous call left in it.
+ * Nothing in it has to start at zero (the copies and the kernel write every byte that is read back), so nothing is
+ * cleared.  Two calls whose GPU work overlaps -- two host threads, or two streams -- would write over each other's rays:
+ * calls on one device must not run at the same time.  Other entry points never touch the array.
+ * Errors: as rt_trace_host; RT_ERR_INVALID when the call does not fit; RT_ERR_CUDA. */
+#define RT_NOALLOC_SCRATCH_BYTES (64ll << 20)
+int rt_trace_host_noalloc(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                          int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj,
+                          void* out_final, void* out_residual, int32_t* out_status, void* cuda_stream);
+
 /* Launch conditions ("fix w, x, k_y, k_z; Newton-solve ... to |D| < 1e-15; the initial guess selects
  * the root").  For each ray: given the position x0 and a unit direction dir, find |n| on D = 0 -- closed form
  * (O: n^2 = 1-X; X: n^2 = RL/S; full: root of Stix's biquadratic A n^4 - B n^2 + C, branch 0 = the root nearer P,

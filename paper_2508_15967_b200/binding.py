@@ -24,7 +24,7 @@ DISP_KINDS = {"omode": 0, "xmode": 1, "cold_full": 2}
 PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
-SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_trace_until", "rt_launch", "rt_launch_w",
+SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_trace_host_noalloc", "rt_trace_until", "rt_launch", "rt_launch_w",
            "rt_launch_kx", "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_launch_count", "rt_last_error", "rt_version")
 NDIAG = 10
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
@@ -97,6 +97,7 @@ def load() -> ctypes.CDLL:
         lib.rt_launch_kx.argtypes = [P, I32, P, P, D, P, I64, I32, D, P, P, P, P]
         lib.rt_orbit.argtypes = [P, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_trace_host.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P]
+        lib.rt_trace_host_noalloc.argtypes = [P, I32, I32, P, P, D, I64, I64, D, I64, P, P, P, P, P]
         lib.rt_launch.argtypes = [P, I32, I32, P, P, D, I64, P, P, P]
         lib.rt_rhs.argtypes = [P, I32, I32, P, P, D, I64, P, P, P, P]
         lib.rt_reduce.argtypes = [I32, P, P, I64, P, P]
@@ -309,6 +310,54 @@ def trace_host(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: fl
     _check(lib.rt_trace_host(eq.handle, _disp(disp), prec, hp(x0), hp(k0), float(omega), n, int(n_steps), float(dt),
                              int(save_stride), hp(o.get("traj") if traj else None), hp(o.get("final") if final else None),
                              hp(o.get("residual") if residual else None), hp(o.get("status") if status else None)))
+    return o
+
+
+NOALLOC_SCRATCH_BYTES = 64 << 20          # RT_NOALLOC_SCRATCH_BYTES (include/rt.h)
+
+
+def trace_host_noalloc(eq: Equilibrium, disp, x0, k0, omega: float, n_steps: int, dt: float, save_stride: int = 1, *,
+                       traj=False, final=True, residual=True, status=True, out: dict | None = None) -> dict:
+    """``rt_trace_host_noalloc``: ``trace_host`` for a program that must not allocate device memory when it calls the
+    library -- one that keeps the whole GPU in its own memory pool, one that cannot stand the device-wide stall of a
+    cudaMalloc / cudaFree in the middle of its run, or one whose device memory is fixed before it starts.  The rays and
+    their results are staged in a 64 MiB array built into the library (``NOALLOC_SCRATCH_BYTES``) instead of in buffers
+    from cudaMalloc, so the whole call has to fit in it at once: a larger one raises ``RtError`` (``RT_ERR_INVALID``).
+    x0, k0 and the outputs are HOST arrays (numpy, or CPU torch tensors) as for ``trace_host``, and the results are the
+    same bits.  The work is enqueued on torch's current stream (numpy arrays: on the default stream) and the call returns
+    when the results are in host memory.  Make the first call on each device outside any stream capture;
+    never run two calls at the same time on one device -- they share the array (include/rt.h has the details).
+    Only the C call is allocation-free: host output arrays that are not passed in through ``out`` are created here."""
+    lib = load()
+    is_torch = not isinstance(x0, np.ndarray)
+    if is_torch:
+        import torch
+        if x0.is_cuda or k0.is_cuda or not x0.is_contiguous() or not k0.is_contiguous():
+            raise ValueError("trace_host_noalloc wants contiguous CPU tensors")
+        prec = _prec_of(x0)
+        empty = lambda shape, dtype=x0.dtype: torch.empty(shape, dtype=dtype)
+        i32 = torch.int32
+        hp = lambda a: None if a is None else ctypes.c_void_p(a.data_ptr())
+    else:
+        x0, k0 = np.ascontiguousarray(x0), np.ascontiguousarray(k0)
+        prec = {np.dtype(np.float64): 0, np.dtype(np.float32): 1}[x0.dtype]
+        empty = lambda shape, dtype=x0.dtype: np.empty(shape, dtype=dtype)
+        i32 = np.int32
+        hp = lambda a: None if a is None else ctypes.c_void_p(a.ctypes.data)
+    n = x0.shape[1]
+    if tuple(x0.shape) != (3, n) or tuple(k0.shape) != (3, n) or k0.dtype != x0.dtype:
+        raise ValueError("x0, k0 must both be [3, n] of the same dtype")
+    n_saved = n_steps // save_stride + 1 if traj else 0
+    o = {} if out is None else out
+    shapes = {"traj": (n_saved, 6, n), "final": (6, n), "residual": (n_saved, n) if traj else (n,), "status": (n,)}
+    wanted = {"traj": traj, "final": final, "residual": residual, "status": status}
+    for key, want in wanted.items():
+        if want and key not in o:
+            o[key] = empty(shapes[key], i32) if key == "status" else empty(shapes[key])
+    arg = lambda key: hp(o[key]) if wanted[key] else None
+    _check(lib.rt_trace_host_noalloc(eq.handle, _disp(disp), prec, hp(x0), hp(k0), float(omega), n, int(n_steps), float(dt),
+                                     int(save_stride), arg("traj"), arg("final"), arg("residual"), arg("status"),
+                                     _stream() if is_torch else None))
     return o
 
 

@@ -397,6 +397,39 @@ struct UntilCleanup {
 };
 }  // namespace
 
+// ---- rt_trace_host_noalloc's staging space ------------------------------------------------------------------------------
+// Device memory that belongs to the library image instead of coming from cudaMalloc (include/rt.h says who needs that and
+// why).  Each GPU that loads this module holds the array until the process exits.  In HOST code the name below is only a
+// stand-in for the symbol, not a device address: handing it to a kernel or to cudaMemcpy as if it were a pointer faults
+// (or, on a machine where the GPU can reach host memory, quietly uses the wrong bytes).  Host code gets the real address
+// from cudaGetSymbolAddress, once per device with that device current (noalloc_scratch below), and passes THAT on.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[RT_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[kNoallocMaxDevices] = {};          // the array's device address on each device; NULL = not looked up yet
+
+// The array's address on the CURRENT device.  The first call per device does the look-up (and may thereby make the runtime
+// load the module there); later calls only read the table.
+int noalloc_scratch(unsigned char** out) {
+  int dev = -1;
+  RT_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoallocMaxDevices)
+    return fail(RT_ERR_UNSUPPORTED, "rt_trace_host_noalloc: device ordinal " + std::to_string(dev) + " is beyond the " +
+                                        std::to_string(kNoallocMaxDevices) + " devices this entry point keeps an address for");
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    RT_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p) return fail(RT_ERR_CUDA, "cudaGetSymbolAddress returned a NULL address for the staging array");
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = static_cast<unsigned char*>(g_noalloc_ptr[dev]);
+  return RT_OK;
+}
+}  // namespace
+
 // ==== C ABI ===========================================================================================================
 extern "C" {
 
@@ -635,6 +668,73 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
 #undef RT_CUDA_DRAIN
   RT_CUDA(cudaStreamSynchronize(eq->streams[0]));
   RT_CUDA(cudaStreamSynchronize(eq->streams[1]));
+  return RT_OK;
+}
+
+// rt_trace_host without a single allocation (include/rt.h): the rays and their results are staged in g_noalloc_scratch,
+// the whole call at once, on the caller's stream.  Nothing here may call cudaMalloc / cudaFree or create a stream or event.
+int rt_trace_host_noalloc(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,
+                          int64_t n_rays, int64_t n_steps, double dt, int64_t save_stride, void* out_traj,
+                          void* out_final, void* out_residual, int32_t* out_status, void* cuda_stream) {
+  int rc = check_trace_args(eq, disp, precision, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj);
+  if (rc) return rc;
+  if (n_rays == 0) return RT_OK;
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  const long long n_saved = out_traj ? n_steps / save_stride + 1 : 0;
+  const long long n_res = out_residual ? (out_traj ? n_saved : 1) : 0;
+  const long long cap = RT_NOALLOC_SCRATCH_BYTES;
+  // sections of the array, each starting on a 256-byte boundary (the kernel writes its samples with 128-bit stores)
+  auto padded = [](size_t bytes) { return (bytes + 255) / 256 * 256; };
+  size_t need = 0;
+  bool fits = n_rays <= cap && n_saved <= cap;              // keeps the products below inside 64 bits
+  size_t off_k = 0, off_traj = 0, off_fin = 0, off_res = 0, off_stat = 0;
+  if (fits) {
+    const size_t row3 = padded(3 * (size_t)n_rays * es);
+    off_k = row3;
+    off_traj = off_k + row3;
+    off_fin = off_traj + padded((size_t)n_saved * 6 * (size_t)n_rays * es);
+    off_res = off_fin + (out_final ? padded(6 * (size_t)n_rays * es) : 0);
+    off_stat = off_res + padded((size_t)n_res * (size_t)n_rays * es);
+    need = off_stat + (out_status ? padded((size_t)n_rays * 4) : 0);
+    fits = need <= (size_t)cap;
+  }
+  if (!fits)
+    return fail(RT_ERR_INVALID,
+                "rt_trace_host_noalloc: this call needs " + (need ? std::to_string(need) : std::string("far more than 2^26")) +
+                    " bytes of device staging space but the library's static array holds RT_NOALLOC_SCRATCH_BYTES = " +
+                    std::to_string(cap) + "; trace fewer rays or samples per call, or use rt_trace_host (which allocates)");
+  unsigned char* base = nullptr;
+  if ((rc = noalloc_scratch(&base))) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  void* dx = base;
+  void* dk = base + off_k;
+  void* t = out_traj ? base + off_traj : nullptr;
+  void* f = out_final ? base + off_fin : nullptr;
+  void* r = out_residual ? base + off_res : nullptr;
+  int32_t* s = out_status ? reinterpret_cast<int32_t*>(base + off_stat) : nullptr;
+  // from the first enqueued copy on, an error return first waits for the stream: a copy into the caller's buffers may
+  // still be in flight
+#define RT_CUDA_WAIT(call)                                                                \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) { cudaStreamSynchronize(st); return cuda_fail(e_, #call); }    \
+  } while (0)
+  const size_t in_bytes = 3 * (size_t)n_rays * es;
+  RT_CUDA_WAIT(cudaMemcpyAsync(dx, x0, in_bytes, cudaMemcpyHostToDevice, st));
+  RT_CUDA_WAIT(cudaMemcpyAsync(dk, k0, in_bytes, cudaMemcpyHostToDevice, st));
+  if (precision == RT_F64)
+    rc = trace_device<double>(eq, disp, dx, dk, omega, nullptr, n_rays, n_steps, dt, save_stride, t, f, r, s, st);
+  else
+    rc = trace_device<float>(eq, disp, dx, dk, omega, nullptr, n_rays, n_steps, dt, save_stride, t, f, r, s, st);
+  if (rc) { cudaStreamSynchronize(st); return rc; }
+  if (out_traj)
+    RT_CUDA_WAIT(cudaMemcpyAsync(out_traj, t, (size_t)n_saved * 6 * (size_t)n_rays * es, cudaMemcpyDeviceToHost, st));
+  if (out_final) RT_CUDA_WAIT(cudaMemcpyAsync(out_final, f, 6 * (size_t)n_rays * es, cudaMemcpyDeviceToHost, st));
+  if (out_residual)
+    RT_CUDA_WAIT(cudaMemcpyAsync(out_residual, r, (size_t)n_res * (size_t)n_rays * es, cudaMemcpyDeviceToHost, st));
+  if (out_status) RT_CUDA_WAIT(cudaMemcpyAsync(out_status, s, (size_t)n_rays * 4, cudaMemcpyDeviceToHost, st));
+#undef RT_CUDA_WAIT
+  RT_CUDA(cudaStreamSynchronize(st));
   return RT_OK;
 }
 
