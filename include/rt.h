@@ -246,7 +246,12 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
  * there is no host round trip between chunks, and the call returns as soon as the graph is enqueued on `cuda_stream`
  * (which must not be capturing).  A frozen ray stays frozen (and bit for bit unchanged) across chunks.
  *   x0, k0         DEVICE [3][n_rays] launch state (not modified)
- *   chunk_steps    >= 1;  max_chunks >= 0 (0: report the launch state);  tol > 0, +inf switches the |D| criterion off
+ *   chunk_steps    >= 1;  max_chunks >= 0;  tol > 0, +inf switches the |D| criterion off
+ *                  max_chunks == 0 reports the launch state: 0 chunks, the active count and max |D| of the launch state,
+ *                  and reason 0 -- the stop tests are made at the end of a chunk, so none is made (not even when max |D|
+ *                  at launch already exceeds tol).  n_rays == 0 with max_chunks > 0 reports 1 chunk, 0 active rays,
+ *                  reason 1 (the loop's first chunk over an empty ensemble finds no active ray); with max_chunks == 0:
+ *                  0 chunks, reason 0.  Both as the oracle's loop does (oracle/rt_oracle.cpp: oracle_trace_until).
  *   out_final      DEVICE [6][n_rays]: the state, advanced in place chunk by chunk; required
  *   out_residual   DEVICE [n_rays] |D| at the current state; required      out_status  DEVICE int32 [n_rays]; required
  *   out_info       DEVICE int64 [RT_UNTIL_INFO_WORDS], 8-byte aligned; on completion
@@ -254,6 +259,10 @@ int rt_reduce(int precision, const void* residual, const int32_t* status, int64_
  *                    [3] reason: 0 = max_chunks reached, 1 = every ray frozen, 2 = max |D| > tol (1 wins over 2)
  *                    [4..9] the last reduction as rt_reduce writes it (doubles);  [10..15] reserved
  * State rows hold k in rad/m; an active ray's k is re-rounded once per chunk by the exchange k <-> n = c k / w.
+ * fp32: the chunks run the one-ray-per-thread kernel (as rt_trace_w does), rt_trace / rt_trace_host the packed
+ * two-rays-per-thread kernel.  The two evaluate the same formulas but are not bit-identical (the compiler contracts some
+ * multiply-add pairs of the scalar code): one fp32 chunk equals rt_trace over the same steps to ~2e-6 relative, not bit for
+ * bit.  fp64 has one kernel: one chunk equals rt_trace exactly.
  * Errors: RT_ERR_INVALID (as rt_trace, and chunk_steps < 1, max_chunks < 0, tol not > 0, a NULL output), UNSUPPORTED, CUDA. */
 #define RT_UNTIL_INFO_WORDS 16
 int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void* x0, const void* k0, double omega,

@@ -757,9 +757,9 @@ int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   long long* info = reinterpret_cast<long long*>(out_info);
   double* red = reinterpret_cast<double*>(info + 4);
-  if (n_rays == 0) {                               // nothing to advance: 0 chunks, 0 active rays, "every ray frozen"
-    RT_CUDA(cudaMemsetAsync(info, 0, RT_UNTIL_INFO_WORDS * 8, st));
-    rt::until_decide_kernel<<<1, 1, 0, st>>>(info, tol, 0, 0, 0);
+  if (n_rays == 0) {                               // an empty ensemble: the loop's first chunk (if one may run) finds no
+    RT_CUDA(cudaMemsetAsync(info, 0, RT_UNTIL_INFO_WORDS * 8, st));      // active ray -- 1 chunk, "every ray frozen"
+    rt::until_decide_kernel<<<1, 1, 0, st>>>(info, tol, max_chunks, 0, max_chunks > 0 ? 1 : 0);
     ++g_launches;
     RT_CUDA(cudaGetLastError());
     return RT_OK;
@@ -811,7 +811,7 @@ int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void
   u.capturing = true;
   if ((rc = chunk(chunk_steps, u.cs, out_status))) return rc;
   if ((rc = launch_reduce(precision, out_residual, out_status, n_rays, red, u.cs))) return rc;
-  rt::until_decide_kernel<<<1, 1, 0, u.cs>>>(info, tol, max_chunks, cond, 1);
+  rt::until_decide_kernel<<<1, 1, 0, u.cs>>>(info, tol, max_chunks, cond, 3);
   ++g_launches;
   RT_CUDA(cudaGetLastError());
   u.capturing = false;

@@ -381,10 +381,14 @@ trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ Trace
 
 // ---- fp32, two rays per thread: packed f32x2 arithmetic (rt_math.cuh: f32x2) ------------------------------------------
 // Thread t of a block traces rays 2 (block * BLOCK + t) and the next one, one in each half of every f32x2 value; a warp
-// owns 64 consecutive rays.  Same arithmetic per ray as trace_kernel<float, ...> (the IEEE fp32 operation on each half), so
-// the two kernels give bit-identical rays; what changes is the instruction stream: one FFMA2 / FMUL2 / FADD2 issue slot
-// serves two rays, and MUFU seeds, domain tests and table look-ups are done per half.  A lane whose ray is frozen keeps
-// computing on its frozen state and is masked out of every update.
+// owns 64 consecutive rays.  Same formulas per ray as trace_kernel<float, ...> (the IEEE fp32 operation on each half), and a
+// ray's result does not depend on which half or thread it rides in -- but the two kernels are NOT bit-identical to each
+// other: where the scalar code has a multiply followed by an add the compiler may contract the pair into one FFMA, while
+// the packed code keeps the two instructions it was written with (measured: one 40-step chunk differs by <= 2e-6 relative,
+// tests/test_gpu_until.py).  So an fp32 result depends on the entry point: rt_trace / rt_trace_host run this kernel, rt_trace_w
+// and rt_trace_until the scalar one (include/rt.h says so at rt_trace_until).  What changes here is the instruction stream:
+// one FFMA2 / FMUL2 / FADD2 issue slot serves two rays, and MUFU seeds, domain tests and table look-ups are done per half.
+// A lane whose ray is frozen keeps computing on its frozen state and is masked out of every update.
 // The packed kernels exist for every dispersion function over the analytic equilibria and for the full determinant over the
 // grid equilibrium.  Over the grid the spline look-ups are NOT packed (rt_math.cuh: grid_values_per_ray): each ray of the
 // thread has its own scalar shared-memory cell cache and its look-ups run in scalar arithmetic, the nine results are packed
@@ -837,19 +841,24 @@ reduce_kernel(const T* __restrict__ res, const int32_t* __restrict__ status, lon
 // sets the WHILE condition on the device -- no host round trip between chunks.
 //   info[0] chunks run   info[1] rays still active (status 0)   info[2] max |D| (bit pattern of a double)
 //   info[3] reason: 0 max_chunks reached, 1 every ray frozen, 2 max |D| > tol        info[4..9]: reduce_kernel's out[6]
+// mode: bit 0 = a chunk has just run (count it), bit 1 = set the WHILE condition (the launch inside the graph's body).
+// The stop tests belong to the end of a chunk: with max_chunks == 0 no chunk runs, none is made and the reason is 0
+// whatever the launch state looks like (as the oracle's loop, which is never entered then).
 __global__ void until_decide_kernel(long long* __restrict__ info, double tol, long long max_chunks,
-                                    cudaGraphConditionalHandle cond, int in_graph) {
+                                    cudaGraphConditionalHandle cond, int mode) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   const double* red = reinterpret_cast<const double*>(info + 4);
-  const long long chunks = info[0] + (in_graph ? 1 : 0);
+  const long long chunks = info[0] + ((mode & 1) ? 1 : 0);
   const long long n_active = (long long)red[3];
   const double max_D = red[0];
   long long reason = 0;
   bool go = chunks < max_chunks;
-  if (n_active == 0) { reason = 1; go = false; }
-  else if (max_D > tol) { reason = 2; go = false; }
+  if (max_chunks > 0) {
+    if (n_active == 0) { reason = 1; go = false; }
+    else if (max_D > tol) { reason = 2; go = false; }
+  }
   info[0] = chunks; info[1] = n_active; info[2] = __double_as_longlong(max_D); info[3] = reason;
-  if (in_graph) cudaGraphSetConditional(cond, go ? 1u : 0u);
+  if (mode & 2) cudaGraphSetConditional(cond, go ? 1u : 0u);
 }
 
 // Roofline denominator: FMA_CHAINS independent accumulators per thread, each a dependent chain of fused multiply-adds.

@@ -124,9 +124,9 @@ def test_degenerate_calls_and_argument_errors(rt, oracle):
     plain32 = rt.trace(eq, w.disp, x32, k32, w.omega, 40, w.dt)
     assert torch.equal(one32["status"], plain32["status"])
     assert float(((one32["final"] - plain32["final"]).abs() / plain32["final"].abs().amax(dim=1, keepdim=True)).max()) < 2e-6
-    e = torch.empty((3, 0), dtype=torch.float64, device="cuda")                          # zero rays
-    z = rt.until_info(rt.trace_until(eq, w.disp, e, e.clone(), w.omega, 10, 5, w.dt)["info"])
-    assert (z["chunks"], z["n_active"], z["reason"]) == (0, 0, 1)
+    e = torch.empty((3, 0), dtype=torch.float64, device="cuda")                          # zero rays: as the oracle's loop over an
+    z = rt.until_info(rt.trace_until(eq, w.disp, e, e.clone(), w.omega, 10, 5, w.dt)["info"])   # empty ensemble (one chunk, then
+    assert (z["chunks"], z["n_active"], z["reason"]) == (1, 0, 1)                        # "every ray frozen"); see the test below
     for bad in (dict(chunk_steps=0), dict(max_chunks=-1), dict(tol=0.0), dict(tol=float("nan"))):
         kw = dict(chunk_steps=10, max_chunks=3, tol=float("inf"))
         kw.update(bad)
@@ -156,4 +156,43 @@ def test_the_call_returns_before_the_loop_has_finished(rt, oracle):
     ev.synchronize()
     assert torch.equal(out["final"], ref["final"]) and torch.equal(out["info"][:4], ref["info"][:4])
     assert rt.until_info(out["info"])["chunks"] == 10
+    eq.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_edge_contracts_equal_the_oracles(rt, oracle, prec):
+    """The two corners where the loop does not run as usual, against oracle.trace_until (not against typed values):
+    max_chunks = 0 reports the launch state and makes NO stop test -- reason 0 ("max_chunks reached") even when max |D| at
+    launch already exceeds tol; an empty ensemble with max_chunks > 0 goes through the loop once (1 chunk, no active ray,
+    reason 1), with max_chunks = 0 not at all."""
+    import torch
+    n = 64 + 13
+    w, oeq, k0 = _case(oracle, 4, n)
+    k0 = k0 * 1.001                                   # off the dispersion surface: |D| ~ 1e-5 at launch, above tol
+    tol = 1e-6
+    eq = rt.create_equilibrium(w.eq)
+    ref = oracle.trace_until(oeq, w.disp, w.x0, k0, w.omega, 10, 0, w.dt, tol)
+    assert (ref["chunks"], ref["n_active"], ref["reason"]) == (0, n, 0) and ref["max_D"] > 10 * tol
+    out = rt.trace_until(eq, w.disp, _dev(w.x0, prec), _dev(k0, prec), w.omega, 10, 0, w.dt, tol)
+    info = rt.until_info(out["info"])
+    assert (info["chunks"], info["n_active"], info["reason"]) == (ref["chunks"], ref["n_active"], ref["reason"])
+    assert abs(info["max_D"] - ref["max_D"]) <= (1e-12 if prec == "f64" else 1e-3) * ref["max_D"] + RES_ATOL[prec]
+    assert np.array_equal(_host(out["status"]), ref["status"])
+    launch_state = _host(torch.cat([_dev(w.x0, prec), _dev(k0, prec)]))      # x rows as given; k rows go through k -> n -> k
+    assert np.array_equal(_host(out["final"])[:3], launch_state[:3])
+    assert np.allclose(_host(out["final"])[3:], launch_state[3:], rtol=4 * (2.2e-16 if prec == "f64" else 1.2e-7), atol=0)
+    assert np.allclose(_host(out["final"]), ref["final"], rtol=4 * (2.2e-16 if prec == "f64" else 1.2e-7), atol=0)
+    # one chunk from the same launch state does stop on the tolerance (reason 2): the test is made after a chunk, never before
+    ref1 = oracle.trace_until(oeq, w.disp, w.x0, k0, w.omega, 10, 3, w.dt, tol)
+    info1 = rt.until_info(rt.trace_until(eq, w.disp, _dev(w.x0, prec), _dev(k0, prec), w.omega, 10, 3, w.dt, tol)["info"])
+    assert (ref1["chunks"], ref1["reason"]) == (1, 2)
+    assert (info1["chunks"], info1["n_active"], info1["reason"]) == (ref1["chunks"], ref1["n_active"], ref1["reason"])
+    # no rays
+    e = torch.empty((3, 0), dtype=torch.float64 if prec == "f64" else torch.float32, device="cuda")
+    for max_chunks in (0, 1, 5):
+        ref0 = oracle.trace_until(oeq, w.disp, np.empty((3, 0)), np.empty((3, 0)), w.omega, 10, max_chunks, w.dt, tol)
+        got0 = rt.until_info(rt.trace_until(eq, w.disp, e, e.clone(), w.omega, 10, max_chunks, w.dt, tol)["info"])
+        assert (got0["chunks"], got0["n_active"], got0["reason"], got0["max_D"]) == \
+               (ref0["chunks"], ref0["n_active"], ref0["reason"], ref0["max_D"]), max_chunks
+    assert (ref0["chunks"], ref0["reason"]) == (1, 1)
     eq.close()
