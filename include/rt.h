@@ -86,7 +86,9 @@ typedef struct rt_equilibrium rt_equilibrium;   /* opaque; owns its device table
  * upload the cell-major coefficient tables.  *out receives the handle.  Errors: INVALID, NOMEM, CUDA. */
 int rt_create_equilibrium(const rt_equilibrium_desc* desc, rt_equilibrium** out);
 
-/* Free the handle and everything it owns.  NULL is accepted.  Synchronises the device. */
+/* Free the handle and everything it owns.  NULL is accepted.  Waits, on the handle's own device, for the work that may still
+ * use the handle: rt_trace_host's streams and the rt_trace_until loops launched through it; for RT_EQ_GRID_RZ also for the
+ * whole device (kernels on the callers' streams may still read its tables).  Other handles' work is not waited for. */
 int rt_destroy(rt_equilibrium* eq);
 
 /* The hot path (Eq. 2-3): trace n_rays rays for n_steps RK4 steps of size dt.
@@ -272,7 +274,9 @@ int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void
 /* The measurement entry points (the roofline denominator rt_fma_peak and its instruction-shape variants) are declared in
  * include/rt_bench.h: they are part of the library, not of the ray-tracing interface. */
 
-/* Number of kernel launches this library has enqueued on the calling process so far (for bench.py's gpu_launches). */
+/* Number of kernel launches this library has enqueued on the calling process so far (for bench.py's gpu_launches).  The three
+ * kernels in the body of rt_trace_until's device-side loop are counted once per call -- when they are recorded -- not once
+ * per chunk: how often the loop ran is only known on the device (out_info[0]). */
 int64_t rt_launch_count(void);
 
 const char* rt_last_error(void);

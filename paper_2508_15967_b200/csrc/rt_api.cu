@@ -69,8 +69,10 @@ rt::Params<T> make_params(const rt_equilibrium* eq, double omega) {
 
 // The grid kind's tables (and the host pipeline's workspace) live on the device that was current when they were created:
 // a call made with another device current would dereference foreign memory.
-int check_device(const rt_equilibrium* eq) {
-  if (!eq || !(eq->psi_pp64 || eq->slot[0])) return RT_OK;
+// Only calls that touch that memory are checked: the analytic kinds' kernels take every constant by value, so an analytic
+// handle works on any device -- except in rt_trace_host (uses_workspace), once its workspace exists.
+int check_device(const rt_equilibrium* eq, bool uses_workspace = false) {
+  if (!eq || !(eq->psi_pp64 || (uses_workspace && eq->slot[0]))) return RT_OK;
   int dev = -1;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cudaGetDevice"); }
@@ -334,13 +336,12 @@ namespace {
 int launch_reduce(int precision, const void* residual, const int32_t* status, long long n, double* out, cudaStream_t st) {
   RT_CUDA(cudaMemsetAsync(out, 0, 6 * sizeof(double), st));
   if (n == 0) return RT_OK;
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0, v = 0;
-    RT_CUDA(cudaGetDevice(&dev));
-    RT_CUDA(cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev));
-    sms = v > 0 ? v : 1;
-  }
+  // the SM count of the device this launch goes to, asked for every time: an attribute query costs well under a microsecond,
+  // is allowed during stream capture, and a cached value would be the first caller's device on a multi-GPU process
+  int dev = 0, sms = 0;
+  RT_CUDA(cudaGetDevice(&dev));
+  RT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (sms < 1) sms = 1;
   long long blocks = (n + 255) / 256;
   if (blocks > (long long)sms * 8) blocks = (long long)sms * 8;
   if (precision == RT_F64)
@@ -361,16 +362,19 @@ struct PendingGraph {
   cudaGraphExec_t ex;
   cudaGraph_t g;
   cudaEvent_t done;
+  const rt_equilibrium* owner;     // the handle whose call launched it (its kernels may read that handle's device tables)
 };
 std::mutex g_pending_mu;
 std::vector<PendingGraph> g_pending;
 
-void release_finished_graphs(bool wait) {
+// Releases every parked graph that has finished.  wait_for != NULL (rt_destroy): the graphs launched through that handle are
+// waited for; the other handles' graphs are only polled, so destroying one handle never blocks on another one's loop.
+void release_finished_graphs(const rt_equilibrium* wait_for) {
   std::lock_guard<std::mutex> lock(g_pending_mu);
   size_t keep = 0;
   for (size_t i = 0; i < g_pending.size(); ++i) {
     PendingGraph& p = g_pending[i];
-    const cudaError_t q = wait ? cudaEventSynchronize(p.done) : cudaEventQuery(p.done);
+    const cudaError_t q = (wait_for && p.owner == wait_for) ? cudaEventSynchronize(p.done) : cudaEventQuery(p.done);
     if (q == cudaErrorNotReady) { g_pending[keep++] = p; continue; }
     if (q != cudaSuccess) cudaGetLastError();
     cudaGraphExecDestroy(p.ex);
@@ -522,9 +526,19 @@ int rt_create_equilibrium(const rt_equilibrium_desc* desc, rt_equilibrium** out)
 
 int rt_destroy(rt_equilibrium* eq) {
   if (!eq) return RT_OK;
-  if (eq->psi_pp64 || eq->slot[0] || eq->streams[0]) cudaDeviceSynchronize();
-  release_finished_graphs(true);
+  // with the HANDLE's device current (not whichever the caller happens to have): wait for what may still use the handle's
+  // memory -- its own two streams (rt_trace_host), the convergence loops launched through it, and, for the grid kind, the
+  // kernels that callers' streams may still be running against its device tables (those streams are unknown here, hence the
+  // device-wide wait for that kind only).  An analytic handle owns no device memory that a kernel reads: no device-wide wait.
+  int cur = -1;
+  const bool owns = eq->psi_pp64 || eq->slot[0] || eq->streams[0];
+  const bool switched = owns && cudaGetDevice(&cur) == cudaSuccess && cur != eq->device && cudaSetDevice(eq->device) == cudaSuccess;
+  for (int s = 0; s < 2; ++s)
+    if (eq->streams[s]) cudaStreamSynchronize(eq->streams[s]);
+  if (eq->psi_pp64) cudaDeviceSynchronize();
+  release_finished_graphs(eq);
   free_handle(eq);
+  if (switched) cudaSetDevice(cur);
   return RT_OK;
 }
 
@@ -598,6 +612,7 @@ int rt_trace_host(rt_equilibrium* eq, int disp, int precision, const void* x0, c
   int rc = check_trace_args(eq, disp, precision, x0, k0, omega, n_rays, n_steps, dt, save_stride, out_traj);
   if (rc) return rc;
   if (n_rays == 0) return RT_OK;
+  if ((rc = check_device(eq, true))) return rc;
   const size_t es = (precision == RT_F64) ? 8 : 4;
   const long long n_saved = out_traj ? n_steps / save_stride + 1 : 0;
   const long long n_res = out_residual ? (out_traj ? n_saved : 1) : 0;
@@ -785,7 +800,7 @@ int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void
     return RT_OK;
   }
   // graph:  {copy x0, k0 into out_final; zero out_status and out_info}  ->  WHILE (cond) { chunk; reduce; decide }
-  release_finished_graphs(false);
+  release_finished_graphs(nullptr);
   UntilCleanup u;
   RT_CUDA(cudaGraphCreate(&u.g, 0));
   cudaGraphNode_t pro[4];
@@ -822,7 +837,7 @@ int rt_trace_until(const rt_equilibrium* eq, int disp, int precision, const void
   RT_CUDA(cudaEventRecord(u.done, st));
   {
     std::lock_guard<std::mutex> lock(g_pending_mu);
-    g_pending.push_back({u.ex, u.g, u.done});
+    g_pending.push_back({u.ex, u.g, u.done, eq});
   }
   u.ex = nullptr; u.g = nullptr; u.done = nullptr;        // now owned by the pending list
   return RT_OK;
