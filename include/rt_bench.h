@@ -4,7 +4,8 @@
  * microbenchmark of >= 8 independent dependent-chain DFMA (resp. FFMA) accumulators per thread ... reporting FMA/s and the
  * SM clock observed").  rt_fma_peak is that microbenchmark; rt_fma_peak_shape runs it at other instruction shapes and
  * occupancies, the evidence behind DESIGN.md section 6's operand-port model of the FP64 / FP32 pipe.  Both are
- * synchronous, allocate and free their own scratch, and use the current device.  Return codes as in rt.h. */
+ * synchronous, allocate and free their own scratch, and use the current device.  rt_math_probe exposes the hot loop's
+ * reciprocal / square-root routines to a unit test.  Return codes as in rt.h. */
 #ifndef RT_B200_RT_BENCH_H
 #define RT_B200_RT_BENCH_H
 
@@ -35,6 +36,14 @@ int rt_fma_peak(int precision, double min_ms, double* fma_per_s, double* sm_cloc
  * / fma_per_s NULL (all checked before the first CUDA call); RT_ERR_CUDA when no device is usable. */
 int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms, double* fma_per_s,
                       double* sm_clock_mhz);
+
+/* Unit-test hook: the hot loop's own reciprocal, reciprocal square root and square root (a MUFU seed plus one Newton
+ * step in fp64, the bare seed in fp32; csrc/rt_math.cuh) applied to an array, so that their rounding error can be measured
+ * directly (tests/test_gpu_math.py; DESIGN.md section 7 has the bounds).  Asynchronous on `cuda_stream`, allocates nothing.
+ *   fn   0: 1/x    1: 1/sqrt(x)    2: sqrt(x)
+ *   x    DEVICE [n] of `precision`;   out  DEVICE [n] of `precision`
+ * Errors: RT_ERR_INVALID (unknown precision / fn, n < 0, a NULL, misaligned or host pointer), RT_ERR_CUDA. */
+int rt_math_probe(int precision, int fn, const void* x, int64_t n, void* out, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -25,7 +25,7 @@ PRECISIONS = {"f64": 0, "f32": 1}
 
 # every symbol include/rt.h declares (tests check the library exports each of them)
 SYMBOLS = ("rt_create_equilibrium", "rt_destroy", "rt_trace", "rt_trace_w", "rt_trace_host", "rt_trace_host_noalloc", "rt_trace_until", "rt_launch", "rt_launch_w",
-           "rt_launch_kx", "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_launch_count", "rt_last_error", "rt_version")
+           "rt_launch_kx", "rt_diagnostics", "rt_orbit", "rt_rhs", "rt_reduce", "rt_fma_peak", "rt_fma_peak_shape", "rt_math_probe", "rt_launch_count", "rt_last_error", "rt_version")
 NDIAG = 10
 DIAG_ROWS = ("n_e", "B", "X", "Y", "S", "D", "P", "R", "L", "n_par2")
 
@@ -103,6 +103,7 @@ def load() -> ctypes.CDLL:
         lib.rt_reduce.argtypes = [I32, P, P, I64, P, P]
         lib.rt_fma_peak.argtypes = [I32, D, ctypes.POINTER(D), ctypes.POINTER(D)]
         lib.rt_fma_peak_shape.argtypes = [I32, I32, I32, D, ctypes.POINTER(D), ctypes.POINTER(D)]
+        lib.rt_math_probe.argtypes = [I32, I32, P, I64, P, P]
         lib.rt_launch_count.restype = I64
         lib.rt_last_error.restype = ctypes.c_char_p
         lib.rt_version.restype = ctypes.c_char_p
@@ -498,3 +499,19 @@ def fma_peak_shape(precision="f64", shape: int = 0, blocks_per_sm: int = 4, min_
     p = PRECISIONS[precision] if isinstance(precision, str) else int(precision)
     _check(lib.rt_fma_peak_shape(p, int(shape), int(blocks_per_sm), float(min_ms), ctypes.byref(rate), ctypes.byref(mhz)))
     return rate.value, mhz.value
+
+
+MATH_FNS = {"rcp": 0, "rsqrt": 1, "sqrt": 2}
+
+
+def math_probe(fn, x):
+    """``rt_math_probe``: the hot loop's own 1/x, 1/sqrt(x) or sqrt(x) (``fn`` = "rcp" / "rsqrt" / "sqrt") applied to the
+    CUDA tensor ``x`` (float64 or float32, 1-D contiguous); returns a tensor like ``x``.  A unit-test hook."""
+    import torch
+    lib = load()
+    if not (x.is_cuda and x.is_contiguous() and x.dim() == 1):
+        raise ValueError("math_probe wants a contiguous 1-D CUDA tensor")
+    out = torch.empty_like(x)
+    _check(lib.rt_math_probe(_prec_of(x), MATH_FNS[fn] if isinstance(fn, str) else int(fn), _ptr(x), x.numel(), _ptr(out),
+                             _stream()))
+    return out

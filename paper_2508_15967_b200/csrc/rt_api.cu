@@ -1034,4 +1034,23 @@ int rt_fma_peak_shape(int precision, int shape, int blocks_per_sm, double min_ms
   return rc;
 }
 
+int rt_math_probe(int precision, int fn, const void* x, int64_t n, void* out, void* cuda_stream) {
+  if (precision != RT_F64 && precision != RT_F32) return fail(RT_ERR_INVALID, "unknown precision");
+  if (fn < 0 || fn > 2) return fail(RT_ERR_INVALID, "fn must be 0 (rcp), 1 (rsqrt) or 2 (sqrt)");
+  if (n < 0) return fail(RT_ERR_INVALID, "n must be >= 0");
+  if (n == 0) return RT_OK;
+  int rc;
+  const size_t es = (precision == RT_F64) ? 8 : 4;
+  if ((rc = require_device_ptr(x, "x", false, es)) || (rc = require_device_ptr(out, "out", false, es))) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const unsigned grid = grid_for(n, rt::AUX_BLOCK);
+  if (precision == RT_F64)
+    rt::math_probe_kernel<double><<<grid, rt::AUX_BLOCK, 0, st>>>(fn, static_cast<const double*>(x), n, static_cast<double*>(out));
+  else
+    rt::math_probe_kernel<float><<<grid, rt::AUX_BLOCK, 0, st>>>(fn, static_cast<const float*>(x), n, static_cast<float*>(out));
+  ++g_launches;
+  RT_CUDA(cudaGetLastError());
+  return RT_OK;
+}
+
 }  // extern "C"

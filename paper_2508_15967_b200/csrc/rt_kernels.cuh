@@ -954,6 +954,17 @@ fma_peak_packed_kernel(float* __restrict__ sink, long long iters, float a, float
   if (threadIdx.x == 0 && blockIdx.x == 0) { clk[0] = (unsigned long long)(c1 - c0); clk[1] = t1 - t0; }
 }
 
+// Unit-test hook for the hot loop's own reciprocal / square-root routines (rt_math.cuh), which no output of the path shows
+// in isolation: out[i] = f(x[i]) with f = 0 rt_rcp, 1 rt_rsqrt, 2 rt_sqrt_fast, in the precision of T.
+template <class T>
+__global__ void __launch_bounds__(AUX_BLOCK)
+math_probe_kernel(int fn, const T* __restrict__ x, long long n, T* __restrict__ out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const T v = x[i];
+  out[i] = (fn == 0) ? rt_rcp(v) : (fn == 1) ? rt_rsqrt(v) : rt_sqrt_fast(v);
+}
+
 #endif  // __CUDACC__
 
 }  // namespace rt
