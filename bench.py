@@ -199,17 +199,20 @@ def oracle_rate(cfg: int, target_s: float, n_threads: int = 0):
     return run_once, n, n_steps, cores
 
 
-def cpu_baseline(cfg: int) -> dict:
-    """the oracle timed (a) on one thread and (b) on every host core, core count and CPU model stated."""
-    run_once, n, n_steps, cores = oracle_rate(cfg, target_s=12.0)
+def cpu_baseline(cfg: int, target_s: float = 12.0, single_thread_s: float = 6.0) -> dict:
+    """the oracle timed (a) on every host core and (b) on one thread (single_thread_s = 0: leg (a) only), core
+    count and CPU model stated.  The single-thread leg is reported in scalar keys beside the all-cores ones."""
+    run_once, n, n_steps, cores = oracle_rate(cfg, target_s=target_s)
     t = run_once()
-    run1, n1, _, _ = oracle_rate(cfg, target_s=6.0, n_threads=1)
-    t1 = run1()
-    return {"value": n * n_steps / t, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": round(t, 2),
-            "sample": f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps (fp64, OpenMP over rays)",
-            "single_thread": {"value": n1 * n_steps / t1, "unit": UNIT, "cores": 1, "seconds": round(t1, 2),
-                              "sample": f"first {n1} rays of the same launch set x {n_steps} steps"},
-            "cpu_model": cpu_model()}
+    out = {"value": n * n_steps / t, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": round(t, 2),
+           "sample": f"first {n} rays of config {cfg}'s seeded launch set x {n_steps} steps (fp64, OpenMP over rays)",
+           "cpu_model": cpu_model()}
+    if single_thread_s > 0:
+        run1, n1, _, _ = oracle_rate(cfg, target_s=single_thread_s, n_threads=1)
+        t1 = run1()
+        out.update({"single_thread_value": n1 * n_steps / t1, "single_thread_seconds": round(t1, 2),
+                    "single_thread_sample": f"first {n1} rays of the same launch set x {n_steps} steps, one thread"})
+    return out
 
 
 def workload_config(cfg: int, scaling: str) -> dict:
@@ -277,6 +280,21 @@ class Job:
         return self.rt.trace(self.eq, w.disp, self.x0, self.k0, self.omega, w.n_steps, w.dt, self.stride, traj=self.traj,
                              out=self.out)
 
+    def parity_sample(self, n_sampled: int = 192) -> dict:
+        """The launch state (the bytes the kernel read), final state and status of `n_sampled` rays of the LAST timed step --
+        first / last rays, a warp boundary and seeded draws, as tests/test_gpu_parity.py samples them -- copied to the host for
+        `sampled_parity` (which runs after every GPU measurement is done: the oracle is never called inside a timed region)."""
+        torch = self.torch
+        rng = np.random.default_rng(4242 + self.cfg)
+        n = self.n
+        idx = np.unique(np.concatenate([np.arange(min(8, n)), np.arange(max(0, n - 8), n), np.array([127, 128, 129]) % n,
+                                        rng.integers(0, n, n_sampled - 19)]))
+        d = torch.from_numpy(idx).cuda()
+        host = lambda t: t.cpu().numpy().astype(np.float64)
+        return {"kind": "rays", "cfg": self.cfg, "x0": host(self.x0[:, d]), "k0": host(self.k0[:, d]),
+                "omega": host(self.omega[d]) if torch.is_tensor(self.omega) else self.omega,
+                "final": host(self.out["final"][:, d]), "status": self.out["status"][d].cpu().numpy()}
+
     def host_buffers(self):
         torch, w = self.torch, self.w
         x0h, k0h = self.x0.cpu().pin_memory(), self.k0.cpu().pin_memory()
@@ -305,7 +323,7 @@ class OrbitJob:
     trajectories every 10 steps.  Same interface as Job as far as time_steps needs it."""
 
     def __init__(self, rt, torch, prec: str):
-        self.rt, self.prec = rt, prec
+        self.rt, self.torch, self.prec = rt, torch, prec
         self.w = w = inputs.orbit_config(4)
         self.eq = rt.create_equilibrium(w.eq)
         dt = torch.float64 if prec == "f64" else torch.float32
@@ -322,9 +340,38 @@ class OrbitJob:
         return self.rt.orbit(self.eq, self.x0, self.v0, w.charge_over_mass, w.n_steps, w.dt, w.save_stride, traj=True,
                              out=self.out)
 
+    def parity_sample(self, n_sampled: int = 192) -> dict:
+        torch, n = self.torch, self.w.n
+        idx = np.unique(np.concatenate([np.arange(8), np.arange(n - 8, n), [127, 128, 129],
+                                        np.random.default_rng(4242).integers(0, n, n_sampled - 19)]))
+        d = torch.from_numpy(idx).cuda()
+        host = lambda t: t.cpu().numpy().astype(np.float64)
+        return {"kind": "orbits", "x0": host(self.x0[:, d]), "k0": host(self.v0[:, d]), "final": host(self.out["final"][:, d]),
+                "status": self.out["status"][d].cpu().numpy()}
+
     def close(self):
         self.out = {}
         self.eq.close()
+
+
+def sampled_parity(sample: dict) -> dict:
+    """the sampled rays of one timed launch against the CPU oracle, from the very launch states the
+    kernel read (fp32 runs: the fp32-rounded ones).  Errors are per-ray 2-norms relative to the oracle's (reading A15),
+    maxima over the rays that end active on both sides; a ray whose status differs is counted, not measured."""
+    import oracle
+    oracle.build()
+    if sample["kind"] == "orbits":
+        w = inputs.orbit_config(4, n=8)
+        ref = oracle.orbit(oracle.Equilibrium(w.eq), sample["x0"], sample["k0"], w.charge_over_mass, w.n_steps, w.dt)
+    else:
+        w = inputs.config(sample["cfg"], n_rays=8)
+        ref = oracle.trace(oracle.Equilibrium(w.eq), w.disp, sample["x0"], sample["k0"], sample["omega"], w.n_steps, w.dt)
+    got, same = sample["final"], sample["status"] == ref["status"]
+    ok = same & (ref["status"] == 0)
+    rel = lambda a, b: float((np.linalg.norm(a - b, axis=0) / np.linalg.norm(b, axis=0)).max()) if a.shape[1] else 0.0
+    second = "max_rel_err_v" if sample["kind"] == "orbits" else "max_rel_err_k"
+    return {"max_rel_err_x": rel(got[:3, ok], ref["final"][:3, ok]), second: rel(got[3:, ok], ref["final"][3:, ok]),
+            "status_mismatches": int((~same).sum()), "n_sampled": int(same.size), "n_compared": int(ok.sum())}
 
 
 def time_steps(torch, job: Job, steps: int, warmup: int, flush, barrier=None):
@@ -364,6 +411,30 @@ def fractions(counts: dict, units: float, kernel_ms: float, fma_rate: float, fla
     return {"roofline_frac": counts["flops"] * per_s / (2.0 * fma_rate),
             "frac_executed": counts["executed"] * per_s / (2.0 * fma_rate), "frac_ceiling": counts["flops"] / (2.0 * slots),
             "pipe_frac": counts["instr"] * per_s / fma_rate, "pipe_model_frac": slots * per_s / fma_rate}
+
+
+def kernel_resources(kernel: str) -> dict:
+    """Registers and spill bytes of one kernel instantiation, parsed from the ptxas report the build writes beside the
+    library (librt_b200.ptxas.txt); `kernel` is the mangled-name prefix.  SURVEY 8(d) item (4)."""
+    import re
+    from paper_2508_15967_b200 import build as rt_build
+    try:
+        text = (rt_build.LIB.parent / "librt_b200.ptxas.txt").read_text()
+    except OSError:
+        return {"registers": None, "spill_bytes": None}
+    m = re.search(r"Function properties for " + re.escape(kernel) + r"\w*\n\s*(\d+) bytes stack frame, (\d+) bytes spill stores, "
+                  r"(\d+) bytes spill loads\nptxas info\s*: Used (\d+) registers", text)
+    if not m:
+        return {"registers": None, "spill_bytes": None}
+    return {"registers": int(m.group(4)), "spill_bytes": int(m.group(2)) + int(m.group(3)), "stack_bytes": int(m.group(1))}
+
+
+def trace_kernel_symbol(cfg: int, prec: str, scan: bool = False) -> str:
+    """Mangled-name prefix of the kernel rt_trace / rt_trace_w launches for a config (rt_api.cu: launch_trace)."""
+    e, d = KERNEL_OF_CONFIG[cfg]
+    if (cfg, prec) in PACKED and not scan:
+        return f"_ZN2rt15trace_kernel_x2ILi{e}ELi{d}EEE"
+    return f"_ZN2rt12trace_kernelI{'d' if prec == 'f64' else 'f'}Li{e}ELi{d}ELb{int(scan)}ELb0EEE"
 
 
 def flavour(cfg: int, prec: str) -> str:
@@ -414,6 +485,8 @@ def run_ours(args) -> int:
     launches = rt.launch_count() - launches0 - args.warmup
     peak_after, peak_mhz = rt.fma_peak(prec, 200.0)
 
+    want_oracle = rank == 0 and world == 1 and not args.no_cpu_baseline
+    headline_sample = job.parity_sample() if want_oracle else None
     # a reduction over the last step's outputs: the run's own correctness summary (max |D|, status counts)
     red = rt.reduce(job.out["residual"].reshape(-1)).cpu().tolist()[:3] + rt.reduce(None, job.out["status"]).cpu().tolist()[3:]
 
@@ -461,20 +534,30 @@ def run_ours(args) -> int:
         job.close()
         del job
         torch.cuda.empty_cache()
-        extra = []
-        for c, p, scan in ((2, "f64", False), (2, "f32", False), (3, "f64", False), (4, "f32", False), (5, "f64", False),
-                           (5, "f32", False), (4, "f64", True)):
-            if (c, p) == (cfg, prec) and not scan:
+        extra, samples = [], []
+        # the last tuple entry: a divisor of the config's ray count -- the per-rank size of a strong-scaling run over that many
+        # GPUs, timed on this one GPU (rays never communicate, so this IS the per-rank time)
+        table = [(1, "f64", False, 1), (1, "f32", False, 1), (2, "f64", False, 1), (2, "f32", False, 1), (3, "f64", False, 1),
+                 (4, "f32", False, 1), (5, "f64", False, 1), (5, "f32", False, 1), (4, "f64", True, 1), (4, "f32", True, 1)]
+        table += [(c, "f64", False, d) for c in (4, 5) for d in (2, 4, 8)]
+        for c, p, scan, div in table:
+            if (c, p) == (cfg, prec) and not scan and div == 1:
                 continue
-            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0], 1000 + c, scan=scan)
+            j = Job(rt, torch, c, p, inputs.FULL_SIZES[c][0] // div, 1000 + c, scan=scan)
             _, kms = time_steps(torch, j, 3, 1, flush)
             pk, _ = rt.fma_peak(p, 100.0)
             cn = {"flops": FLOPS_PER_RAY_STEP[(c, p)], "instr": FP_INSTR_PER_RAY_STEP[(c, p)], "rf3": FP_RF3_PER_RAY_STEP[(c, p)],
                   "executed": FLOPS_EXECUTED_PER_RAY_STEP[(c, p)]}
-            extra.append({"workload": f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else ""),
-                          "dtype": p, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT, "kernel_ms": kms,
-                          "traffic": NCU_DRAM_BYTES.get((c, p)) if not scan else None,
+            name = f"cfg{c}" + (" with one frequency per ray (rt_trace_w, w_i = w0 (1 +- 10 %))" if scan else "")
+            if div > 1:
+                name += f" at n_rays / {div} = {j.n} rays (the per-rank size of a {div}-GPU strong-scaling run, on one GPU)"
+            if c == 1:
+                name += " -- 1024 rays = 16 blocks on 148 SMs: latency-bound, the fractions say how empty the chip is"
+            extra.append({"workload": name, "dtype": p, "n_rays": j.n, "value": j.ray_steps / (kms * 1e-3), "unit": UNIT,
+                          "kernel_ms": kms, "traffic": NCU_DRAM_BYTES.get((c, p)) if not scan and div == 1 else None,
+                          **kernel_resources(trace_kernel_symbol(c, p, scan)),
                           **fractions(cn, j.ray_steps, kms, pk, flavour(c, p) if not scan else p)})
+            samples.append(j.parity_sample() if want_oracle and div == 1 else None)
             j.close()
             del j
             torch.cuda.empty_cache()
@@ -486,14 +569,29 @@ def run_ours(args) -> int:
                                       "every 10 steps + energy drift (rt_orbit)", "dtype": p,
                           "value": j.ray_steps / (kms * 1e-3), "unit": "particle-steps/s", "kernel_ms": kms,
                           "kernel": "rt::orbit_kernel", "traffic": NCU_DRAM_BYTES.get(("orbit4", p)),
+                          **kernel_resources(f"_ZN2rt12orbit_kernelI{'d' if p == 'f64' else 'f'}Li2EEE"),
                           **fractions(ORBIT_COUNTS[p], j.ray_steps, kms, pk, p)})
+            samples.append(j.parity_sample() if want_oracle else None)
             j.close()
             del j
             torch.cuda.empty_cache()
 
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    # every GPU measurement is done: now the oracle legs (the only place this arm calls oracle/)
+    cpu, parity = None, None
+    if want_oracle:
         cpu = cpu_baseline(cfg)
+        parity = sampled_parity(headline_sample)
+        if extra:
+            per_cfg = {}                   # the oracle timed on a ~3 s sample of each other config too, all cores
+            for row, smp in zip(extra, samples):
+                if smp is None:
+                    continue
+                row["parity"] = sampled_parity(smp)
+                if smp["kind"] == "rays":
+                    c = smp["cfg"]
+                    if c not in per_cfg:
+                        per_cfg[c] = cpu_baseline(c, target_s=3.0, single_thread_s=0.0)
+                    row["cpu_baseline"] = per_cfg[c]
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -501,8 +599,10 @@ def run_ours(args) -> int:
                 "dtype": prec, "data": "synthetic", "config": workload_config(cfg, args.scaling),
                 "run": {"launch_states": "rt_launch kernel, max |D0| = %.1e" % launch_residual,
                         "rays_this_rank": n_rays if args.scaling == "weak" else list(sharding.ray_range(n_rays, rank, world))},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-                "checks": {"max_abs_D": red[0], "mean_abs_D": red[1] / max(red[2], 1.0), "status_counts": red[3:6]},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+                "roofline": {**roofline, **kernel_resources(trace_kernel_symbol(cfg, prec))},
+                "checks": {"max_abs_D": red[0], "mean_abs_D": red[1] / max(red[2], 1.0), "status_counts": red[3:6],
+                           "parity": parity},
                 "cpu_baseline": cpu, "other_configs": extra}
         print(json.dumps(line))
     if dist:

@@ -42,6 +42,14 @@ constexpr int trace_maxnreg() {
   return (sizeof(T) == 8 && EQ == EQ_LINEAR && DISP != DISP_FULL) ? 72 : TraceShape<T, EQ>::MAXNREG;
 }
 
+// extra registers of the per-ray-frequency (PW) kernels, which hold the frequency-dependent constants per thread: 16, and 24
+// for the fp64 full determinant over the analytic equilibria (at 136 the tokamak instantiation spilled 8 bytes in its
+// prologue; 144 registers are the same 7 blocks per SM)
+template <class T, int EQ, int DISP>
+constexpr int pw_extra_regs() {
+  return (sizeof(T) == 8 && DISP == DISP_FULL && EQ != EQ_GRID) ? 24 : 16;
+}
+
 template <class T>
 struct TraceArgs {
   const T* x0;
@@ -299,7 +307,7 @@ struct RowStore {
 // RESUME: the chunk kernel of rt_trace_until -- each ray's status at entry comes from A.status_in (a separate
 // instantiation, so that the plain kernels' register allocation is untouched).
 template <class T, int EQ, int DISP, bool PW, bool RESUME = false>
-__global__ void __maxnreg__((trace_maxnreg<T, EQ, DISP>() + (PW ? 16 : 0) + (RESUME ? 8 : 0)))
+__global__ void __maxnreg__((trace_maxnreg<T, EQ, DISP>() + (PW ? pw_extra_regs<T, EQ, DISP>() : 0) + (RESUME ? 8 : 0)))
 trace_kernel(const __grid_constant__ Params<T> P0, const __grid_constant__ TraceArgs<T> A) {
   constexpr int BLOCK = TraceShape<T, EQ>::BLOCK;
   const long long N = A.n_rays;

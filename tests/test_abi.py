@@ -217,3 +217,16 @@ def test_flop_tables_match_the_compiled_kernels(lib):
     import re
     spilled = [max(int(x) for x in re.findall(r"(\d+) bytes spill stores", b)) for b in traces]
     assert max(spilled) <= 64, spilled
+
+
+def test_no_trace_or_orbit_kernel_spills(lib):
+    """north_star: "register spills at zero".  Every instantiation of the step-loop kernels -- trace_kernel (per-ray frequency and
+    resume variants included), trace_kernel_x2, orbit_kernel -- in the ptxas report the build writes beside the library."""
+    report = binding.LIB_PATH.parent / "librt_b200.ptxas.txt"
+    if not report.exists() or report.stat().st_mtime < binding.LIB_PATH.stat().st_mtime - 600:
+        rt_build.build(force=True)
+    rows = re.findall(r"Function properties for (_ZN2rt(?:12trace_kernel|15trace_kernel_x2|12orbit_kernel)I\w+)\n\s*(\d+) bytes stack "
+                      r"frame, (\d+) bytes spill stores, (\d+) bytes spill loads", report.read_text())
+    assert len(rows) >= 60, len(rows)
+    spilled = {name: (int(a), int(b), int(c)) for name, a, b, c in rows if int(a) or int(b) or int(c)}
+    assert not spilled, spilled
