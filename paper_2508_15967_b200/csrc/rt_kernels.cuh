@@ -544,13 +544,20 @@ RT_DEV bool orbit_rhs(const Params<T>& P, T qm, const T* y, T* f, Gather& gather
 }
 
 // One classical RK4 step of the orbit equations; same acceptance rule and return codes as rk4_step.
+// fp32 (COMP): the POSITION is carried as the unevaluated sum y[0..2] + xlo[0..2].  A step moves a particle by ~1e-3 m at
+// |x| ~ 2 m, so a plain fp32 update loses ~0.2 um per step; over 1000 steps that random walk reaches several um, the field
+// seen by the particle is off by dB/B = dR/R ~ 3e-6, and the gyro-phase (~100 rad) by ~2e-4 -- the velocity error that
+// bench.py's sampled parity showed (2.2e-4, over north_star's 1e-4).  So the step's increment is summed on its own and
+// added to (y, xlo) with a Fast2Sum (|y| >> |increment| for positions): 12 FADD per step.  Velocities rotate through zero
+// and their rounding only random-walks the phase (~2e-6): they keep the plain update.  fp64 is untouched (xlo unused).
 template <class T, int EQ, class Gather>
-RT_DEV int orbit_step(const Params<T>& P, T qm, T h, T* y, Gather& gather) {
+RT_DEV int orbit_step(const Params<T>& P, T qm, T h, T* y, T* xlo, Gather& gather) {
+  constexpr bool COMP = sizeof(T) == 4;
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0), h3 = h * T(1.0 / 3.0);
   constexpr int NA = (EQ == EQ_LINEAR) ? 5 : 6;          // active components (slab: v_z is constant)
   T k[6], acc[6], ys[6];
 #pragma unroll
-  for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = y[j]; ys[j] = y[j]; }
+  for (int j = 0; j < 6; ++j) { k[j] = T(0); acc[j] = (COMP && j < 3) ? T(0) : y[j]; ys[j] = y[j]; }
   bool ok = true;
   auto stage = [&](int st) {
     const T a = (st == 0) ? T(0) : ((st == 3) ? h : hh);
@@ -569,12 +576,26 @@ RT_DEV int orbit_step(const Params<T>& P, T qm, T h, T* y, Gather& gather) {
     for (int st = 0; st < 4; ++st) stage(st);
   }
   if (!ok) return 1;
+  T nlo[3] = {T(0), T(0), T(0)};
+  if constexpr (COMP) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const T t = acc[j] + xlo[j];       // the step's increment plus what earlier steps could not represent
+      const T s = y[j] + t;
+      nlo[j] = t - (s - y[j]);           // Fast2Sum: exact for |y| >= |t|
+      acc[j] = s;
+    }
+  }
   bool fin = true;
 #pragma unroll
   for (int j = 0; j < 6; ++j) fin = fin && rt_finite(acc[j]);
   if (!fin) return 2;
 #pragma unroll
   for (int j = 0; j < 6; ++j) y[j] = acc[j];
+  if constexpr (COMP) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) xlo[j] = nlo[j];
+  }
   return 0;
 }
 
@@ -614,6 +635,7 @@ orbit_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ OrbitA
     y[c] = valid ? A.x0[c * N + i] : T(0);
     y[3 + c] = valid ? A.v0[c * N + i] : T(1);
   }
+  T xlo[3] = {T(0), T(0), T(0)};          // fp32: low parts of the position (orbit_step)
   const T inv_e0 = T(1) / rt_fma(y[3], y[3], rt_fma(y[4], y[4], y[5] * y[5]));
   int status = valid ? 0 : 3;
   auto save = [&](T* rows6, T* drift_row) {
@@ -631,7 +653,7 @@ orbit_kernel(const __grid_constant__ Params<T> P, const __grid_constant__ OrbitA
   for (long long m = 1; m <= n_outer; ++m) {
 #pragma unroll 1
     for (long long s = 0; s < n_inner; ++s)
-      if (status == 0) status = orbit_step<T, EQ>(P, A.qm, A.h, y, gather);
+      if (status == 0) status = orbit_step<T, EQ>(P, A.qm, A.h, y, xlo, gather);
     if (A.traj) save(A.traj + m * 6 * A.n, A.drift ? A.drift + m * A.n : nullptr);
   }
   if (A.fin || (!A.traj && A.drift)) save(A.fin, A.traj ? nullptr : A.drift);

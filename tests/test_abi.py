@@ -199,7 +199,8 @@ def test_flop_tables_match_the_compiled_kernels(lib):
         assert got["executed"] == bench.FLOPS_EXECUTED_PER_RAY_STEP[(cfg, prec)], (cfg, prec, got)
     for prec, c in bench.ORBIT_COUNTS.items():
         got = counted[(prec, *bench.ORBIT_KERNEL)]
-        assert (got["flops"], got["instr"], got["rf3"], got["executed"]) == (c["flops"], c["instr"], c["rf3"], c["executed"]), (prec, got)
+        assert (got["flops"] - c.get("compensation", 0), got["instr"], got["rf3"], got["executed"]) == \
+               (c["flops"], c["instr"], c["rf3"], c["executed"]), (prec, got)
     # spills would show up as local-memory traffic: no trace kernel may execute a local load / store inside a ray-step,
     # and what ptxas parks outside the step loop (store staging: once per ray) stays below 64 bytes
     assert all(r["local"] == 0 for r in counted.values()), {k: r["local"] for k, r in counted.items() if r["local"]}

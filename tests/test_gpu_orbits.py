@@ -3,8 +3,10 @@ particles in the equilibria of configs 3, 4, 5 -- against oracle.orbit on the sa
 
 Tolerances: per-particle 2-norms of x and of v.  Both sides apply the same discrete map (same ODE,
 tableau, dt), so they differ by rounding only: 1e-10 in fp64 like the rays.  In fp32 the velocity rotates through
-Phi = W t ~ 80-100 rad in 1000 steps, and a relative rounding delta of B, dt or q/m (6e-8 each in fp32, about ten of them
-per stage, not all independent from step to step) turns it by Phi * delta: a few 1e-5 each, 1e-4 observed; the bar is 5e-4.
+Phi = W t ~ 80-100 rad in 1000 steps, so a relative error delta of the field seen by the particle turns it by Phi * delta.
+With a plain fp32 position update delta reached ~3e-6 (positions random-walk by ~0.2 um per step) and the velocities ended
+2.2e-4 off; orbit_kernel<float> now sums positions with compensation (rt_kernels.cuh: orbit_step) and bench.py's sampled
+parity shows 6e-6.  The bar is north_star's 1e-4.
 The energy drift is a difference of O(1) numbers: absolute 64 ulp against the drift formula evaluated at the kernel's own
 states.
 """
@@ -16,7 +18,7 @@ from helpers import rel_err_xk
 from test_gpu_parity import _dev, _host, rt  # noqa: F401
 
 pytestmark = pytest.mark.gpu
-TOL = {"f64": 1e-10, "f32": 5e-4}
+TOL = {"f64": 1e-10, "f32": 1e-4}
 DRIFT_ATOL = {"f64": 64 * 2.2e-16, "f32": 64 * 1.2e-7}
 
 
