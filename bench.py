@@ -48,7 +48,7 @@ UNIT = "ray-steps/s"
 # formulation, one RK4 step = 4 right-hand sides + the tableau; a fused multiply-add counts 2, a division or square root 1
 # (its Newton refinement is NOT counted).  FP_INSTR_PER_RAY_STEP is what the FP64 / FP32 pipe actually issues per
 # ray-step (FMA, MUL, ADD, SETP instructions, refinements included).  Both tables are counted from the compiled kernels by
-# paper_2508_15967_b200/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
+# tests/sass_count.py and pinned to it by tests/test_abi.py::test_flop_tables_match_the_compiled_kernels.
 FLOPS_PER_RAY_STEP = {(1, "f64"): 115, (2, "f64"): 115, (3, "f64"): 243, (4, "f64"): 707, (5, "f64"): 1200,
                       (1, "f32"): 117, (2, "f32"): 117, (3, "f32"): 246, (4, "f32"): 711, (5, "f32"): 1200}
 # FLOPS_EXECUTED_PER_RAY_STEP: flops as the kernel executes them (2 per fused multiply-add, 1 per multiply / add, Newton
@@ -59,7 +59,7 @@ FP_INSTR_PER_RAY_STEP = {(1, "f64"): 75, (2, "f64"): 75, (3, "f64"): 193, (4, "f
                          (1, "f32"): 70, (2, "f32"): 70, (3, "f32"): 174, (4, "f32"): 484, (5, "f32"): 775}
 # FP_RF3_PER_RAY_STEP: how many of those instructions read THREE DISTINCT registers from the register file.  Such an instruction
 # occupies the FP64 pipe for 3 cycles instead of 2 (scalar FP32: 1.56 slots instead of 1; packed f32x2: 3 cycles instead of 2) -- measured by
-# rt_fma_peak_shape, shapes 2 / 6 (profiles/r1_fma_peak_shapes.md, r2_fma_peak_shapes.md) -- so the pipe time of a ray-step is
+# rt_fma_peak_shape, shapes 2 / 6 (profiles/r2_fma_peak_shapes.md) -- so the pipe time of a ray-step is
 # (instr + RF3_EXTRA * rf3) issue slots of the FMA microbenchmark; `pipe_model_frac` is that time over the measured kernel
 # time.  The fp32 kernels of the analytic equilibria (configs 1-4) are the packed two-rays-per-thread
 # kernels (trace_kernel_x2); their counts are per ray (a packed instruction = one slot per ray).

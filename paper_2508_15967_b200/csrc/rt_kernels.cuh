@@ -905,7 +905,7 @@ __global__ void until_decide_kernel(long long* __restrict__ info, double tol, lo
 //            of FFMA2, each instruction two fused multiply-adds: what the chip's FP32 FMA pipe delivers at best;
 //   SHAPE 6 (fp32 only): shape 2 with packed accumulators (three distinct 64-bit register pairs per FFMA2).
 // On B200 the DFMA rate is 63.7 / 58 / 42.7 per clock per SM for shapes 0 / 1 / 2: an FP64 instruction that reads three
-// registers from the register file occupies the pipe for 3 cycles instead of 2 (profiles/r1_fma_peak_shapes.md).  FP32:
+// registers from the register file occupies the pipe for 3 cycles instead of 2 (profiles/r2_fma_peak_shapes.md).  FP32:
 // 123.2 / 117 / 78.8 scalar, 127.9 / 84.9 packed (shapes 5 / 6): the same port limit, two FMAs per issue slot.
 constexpr int FMA_CHAINS = 16;
 constexpr int FMA_BLOCK = 256;

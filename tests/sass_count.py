@@ -1,7 +1,7 @@
 """Count the floating-point work of one ray-step (particle-step) in the compiled ``trace_kernel`` and ``orbit_kernel``
 instantiations (``cuobjdump -sass``).
 
-    python -m paper_2508_15967_b200.sass_count            # table for every trace kernel in librt_b200.so
+    python tests/sass_count.py            # table for every trace kernel in librt_b200.so
 
 A ray-step is one pass through the body of the kernel's step loop (the loops that hold FP-pipe instructions are nested:
 sample loop > step loop, and for the grid equilibrium > the rolled stage loop, which runs 4 times per step).
@@ -12,7 +12,7 @@ Reported per kernel:
 * ``rf3``       how many of them read THREE DISTINCT registers from the register file (constants, immediates, RZ and operands
                 served by the operand-reuse cache -- flagged ``.reuse`` in the same slot of the preceding instruction --
                 do not count).  Such an instruction occupies the FP64 pipe for 3 cycles instead of 2 (FP32: 1.56
-                instead of 1; ``rt_fma_peak_shape`` shape 2, profiles/r1_fma_peak_shapes.md), so the pipe time of a
+                instead of 1; ``rt_fma_peak_shape`` shape 2, profiles/r2_fma_peak_shapes.md), so the pipe time of a
                 ray-step is 2 instr + rf3 cycles per warp and scheduler;
 * ``executed``  flops as executed, a fused multiply-add counted as 2;
 * ``mufu``      MUFU seeds (reciprocals and reciprocal square roots), ``rsqrt`` of them square roots;
@@ -40,7 +40,7 @@ import subprocess
 from collections import Counter
 from pathlib import Path
 
-LIB = Path(__file__).resolve().parent / "librt_b200.so"
+LIB = Path(__file__).resolve().parent.parent / "paper_2508_15967_b200" / "librt_b200.so"
 _INS = re.compile(r"\s+/\*([0-9a-f]+)\*/\s+(?:@!?U?P\w+\s+)?([A-Z0-9_.]+)(.*?);")
 _FP = {"d": ("DFMA", "DMUL", "DADD", "DSETP"), "f": ("FFMA", "FMUL", "FADD", "FSETP")}
 _FP2 = ("FFMA2", "FMUL2", "FADD2")       # packed f32x2: one instruction serves both rays of a thread

@@ -186,7 +186,7 @@ def test_flop_tables_match_the_compiled_kernels(lib):
     """bench.py's algorithmic-flop and FP-instruction tables are counted from the SASS of the trace kernels
     (sass_count.py); a kernel change that alters the counts must update the tables."""
     import bench
-    from paper_2508_15967_b200 import sass_count
+    import sass_count
     if sass_count.cuobjdump() is None:
         pytest.skip("cuobjdump not available")
     counted = sass_count.count_kernels()

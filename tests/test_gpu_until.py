@@ -64,9 +64,20 @@ def test_runs_to_max_chunks_and_matches_the_plain_trace(rt, oracle, cfg, prec):
     act = ref["status"] == 0
     ex, ek = rel_err_xk(_host(out["final"])[:, act], ref["final"][:, act])
     assert ex < TOL[prec] and ek < TOL[prec], (ex, ek)
-    if (~act).any():                                    # frozen rays: same step of freezing (a step is ~1e-3 m)
+    if (~act).any():                                    # frozen rays: same step of freezing (a one-step difference is ~1e-3)
         ex, ek = rel_err_xk(_host(out["final"])[:, ~act], ref["final"][:, ~act])
-        assert ex < 1e-4 and ek < 1e-4, (ex, ek)
+        if cfg == 4:                                    # analytic tokamak: the bar of every other ray
+            bx = bk = TOL[prec]
+        else:                                           # grid edge (n_e -> 0, the determinant's two roots merge): 50 x the ORACLE's
+            sx = sk = 0.0                               # own sensitivity to a 1e-15 perturbation of the launch positions, capped
+            for seed in (0, 1, 2):                      # at 1e-5 -- the bound test_rays_leaving_the_domain_freeze_identically derives
+                x1 = w.x0 * (1.0 + 1e-15 * np.random.default_rng(seed).normal(size=w.x0.shape))
+                ref1 = oracle.trace_until(oeq, w.disp, x1, k0, w.omega, chunk, max_chunks, w.dt)
+                same = (~act) & (ref1["status"] == ref["status"])
+                a, b = rel_err_xk(ref1["final"][:, same], ref["final"][:, same])
+                sx, sk = max(sx, a), max(sk, b)
+            bx, bk = min(1e-5, max(TOL[prec], 50 * sx)), min(1e-5, max(TOL[prec], 50 * sk))
+        assert ex < bx and ek < bk, (ex, ek, bx, bk)
         # ... and frozen means frozen bit for bit: they froze in the first few chunks, so a run that stops 4 chunks earlier
         # leaves them in exactly the same state (their k rows do not go through the k <-> n exchange again)
         early = rt.trace_until(eq, w.disp, x0d, k0d, w.omega, chunk, max_chunks - 4, w.dt)
